@@ -1,0 +1,174 @@
+/*
+ * eldr_moe.h -- C ABI of the B200 (sm_100a) batched-decode MoE layer with fused ELDR expert-signature
+ * accumulation.  Source of the method: "ELDR: Expert-Locality-Aware Decode Routing for PD-Disaggregated
+ * MoE Serving" (arxiv/paper_2607_00466), cited below as PAPER.md:<line> (section).
+ *
+ * What the path computes (section 3.1: "the gate partitions the batch among experts ... each
+ * step fetches the weights of every expert the batch activates"; "standard top-k gating"):
+ *
+ *   z[t,e]   = sum_h x[t,h] * gate_w[e,h] (+ gate_bias[e])                       gate GEMV, fp32
+ *   p[t,:]   = softmax_E(z[t,:]);  ids[t,:] = the k experts with the largest z (ties -> lower id),
+ *              z-descending;  w[t,j] = p[t,ids_j] / sum_i p[t,ids_i]  if renormalize, else p[t,ids_j]
+ *   U        = { e : some token chose e }   (the active-expert union, ascending id)
+ *   out[t,:] = sum_j w[t,j] * W2_e ( silu(W1_e x_t) * (W3_e x_t) ),  e = ids[t,j]   (SwiGLU, no bias)
+ *              + sum_s FFN_shared_s(x_t)                               (always-on shared experts, weight 1)
+ *   only experts in U (and the shared experts) are read from HBM, each exactly once per call.
+ *
+ * Signature (section 4.2.2 step 1 "Count"; section 4.4):
+ *   for every recorded token t and each of its k ids e:
+ *     sig_req  [token_req[t],   layer, e] += 1      int32 [R , L, E]   per-request counts c_r(l,e)
+ *     sig_block[token_block[t], layer, e] += 1      int8  [NB, L, E]   "one int8 per (block, MoE layer, expert)"
+ *   so that  s_r = sum_{b in B(r)} sig_block[b].
+ *
+ * Conventions for every entry point
+ *   - Pointers are DEVICE pointers unless the name starts with h_ (host).  The caller owns every buffer;
+ *     the library never allocates, frees or retains device memory (it caches only TMA descriptors, by value).
+ *   - All work is enqueued on `stream`; no host synchronisation, no hidden streams
+ *     (except eldr_moe_decode_layer_host, which is synchronous by contract).
+ *   - Layouts are row-major, dense.  bf16 tensors are passed as uint16_t bit patterns (eldr_bf16).
+ *     Device pointers must be 16-byte aligned.
+ *   - Return value: ELDR_OK (0) or a negative eldr_status_t.  No exceptions cross the ABI.
+ *     T == 0 is a no-op returning ELDR_OK.  NaN/Inf inputs are outside the contract (ids stay in [0,E)).
+ *   - token_req[t] < 0 / token_block[t] < 0 mean "do not record this token" (padding).
+ *   - Shared experts are not gate selections: they are never counted in signatures nor in n_active.
+ */
+#ifndef ELDR_MOE_H_
+#define ELDR_MOE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef uint16_t eldr_bf16;          /* bfloat16 bit pattern */
+typedef void*    eldr_stream_t;      /* cudaStream_t */
+
+typedef enum {
+  ELDR_OK                   =  0,
+  ELDR_ERR_INVALID_ARG      = -1,    /* null pointer, bad shape field, misaligned pointer, k > E, block size > 127 */
+  ELDR_ERR_UNSUPPORTED      = -2,    /* shape outside what the kernels support (see each function) */
+  ELDR_ERR_WORKSPACE_SMALL  = -3,
+  ELDR_ERR_CUDA             = -4     /* a CUDA runtime / driver call or a launch failed */
+} eldr_status_t;
+
+typedef struct {                     /* passed by const pointer, HOST memory */
+  int32_t hidden;                    /* H, multiple of 8 (16-byte bf16 vectors)                      */
+  int32_t inter;                     /* I, multiple of 8                                              */
+  int32_t n_experts;                 /* E routed experts, 1..256                                      */
+  int32_t top_k;                     /* k, 1..min(E,16)                                               */
+  int32_t n_shared;                  /* always-on shared experts, 0..8                                */
+  int32_t renormalize;               /* 1: w /= sum over the top-k (all BASELINE configs); 0: w = p   */
+  int32_t n_layers;                  /* L, row stride of the signature tensors                        */
+  int32_t kv_block_size;             /* tokens per KV block, 1..127 (int8 cells)        */
+} eldr_moe_shape_t;
+
+/* Byte offsets of the intermediates eldr_moe_decode_layer leaves in `workspace` (for per-kernel parity
+ * tests and profiling; the contents are valid until the next call that uses the workspace). */
+typedef struct {
+  size_t z;          /* float   [T,E]            gate logits incl. bias                                 */
+  size_t cnt;        /* int32   [E]              pairs routed to each expert                             */
+  size_t off;        /* int32   [E+1]            exclusive scan of cnt                                   */
+  size_t perm;       /* int32   [T*k]            pair index (t*k+slot) at each sorted position           */
+  size_t pair_pos;   /* int32   [T*k]            inverse of perm                                         */
+  size_t work;       /* int32x4 [E+n_shared]     {expert, x_row0, out_row0, m} per streamed expert       */
+  size_t n_work;     /* int32   [1]              n_active + n_shared                                     */
+  size_t x_perm;     /* bf16    [T*k + T, H]     x gathered in sorted order, then a plain copy of x      */
+  size_t h;          /* bf16    [T*(k+ns), I]    silu(W1 x)*(W3 x) per sorted pair, then shared experts  */
+  size_t y;          /* float   [T*(k+ns), H]    W2 h per sorted pair, then shared experts               */
+  size_t total;      /* bytes needed                                                                    */
+} eldr_moe_ws_layout_t;
+
+/* Gate + softmax top-k + renormalise (+ fused signature accumulation) for T tokens of one layer.
+ * Operation: z, ids, w as defined above ("The gate scores experts using the token's hidden
+ * representation and dispatches the token to the top-scoring experts").  Any T >= 0.
+ *   x [T,H] bf16 in; gate_w [E,H] fp32 in; gate_bias [E] fp32 in or NULL;
+ *   topk_ids [T,k] int32 out; topk_w [T,k] fp32 out;
+ *   token_req/token_block [T] int32 in or NULL; sig_req [R,L,E] int32 in/out or NULL;
+ *   sig_block [NB,L,E] int8 in/out or NULL (accumulated in place; caller zeroes / resets);
+ *   workspace: at least eldr_moe_workspace_bytes(shape, T) bytes (holds z). */
+int32_t eldr_moe_gate_topk(const eldr_moe_shape_t* shape, int32_t layer, int32_t T,
+                           const eldr_bf16* x, const float* gate_w, const float* gate_bias,
+                           int32_t* topk_ids, float* topk_w,
+                           const int32_t* token_req, const int32_t* token_block,
+                           int32_t* sig_req, int8_t* sig_block,
+                           void* workspace, size_t workspace_bytes, eldr_stream_t stream);
+
+/* One decode step of one MoE layer: gate -> top-k (+signature) -> token->expert permutation with union
+ * compaction -> grouped SwiGLU FFN streaming each ACTIVE expert's weights once -> weighted combine.
+ *   w13 [E,2I,H] bf16: rows 0..I-1 = w1 (SiLU branch), rows I..2I-1 = w3;  w2 [E,H,I] bf16;
+ *   shared_w13 [n_shared,2I,H], shared_w2 [n_shared,H,I] (NULL iff n_shared == 0);
+ *   out [T,H] bf16 (rounded once, RNE, from the fp32 combine);
+ *   topk_ids/topk_w: outputs, or INPUTS if force_routing != 0 (ids must be distinct per token, in [0,E));
+ *   active_experts [E] int32 out: first n_active entries = U ascending, rest -1;  n_active [1] int32 out.
+ *   T in 0..1024 (decode batches; larger T -> ELDR_ERR_UNSUPPORTED).
+ * Fast path (TMA + mma) needs H % 64 == 0 and I % 64 == 0; other shapes run a plain CUDA-core path. */
+int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* shape, int32_t layer, int32_t T,
+                              const eldr_bf16* x, const float* gate_w, const float* gate_bias,
+                              const eldr_bf16* w13, const eldr_bf16* w2,
+                              const eldr_bf16* shared_w13, const eldr_bf16* shared_w2,
+                              eldr_bf16* out,
+                              int32_t* topk_ids, float* topk_w, int32_t force_routing,
+                              int32_t* active_experts, int32_t* n_active,
+                              const int32_t* token_req, const int32_t* token_block,
+                              int32_t* sig_req, int8_t* sig_block,
+                              void* workspace, size_t workspace_bytes, eldr_stream_t stream);
+
+/* Same step with the per-step inputs and results in HOST memory (pinned for async copies): copies h_x and
+ * the token maps to the device, runs eldr_moe_decode_layer, copies out / ids / weights / n_active back and
+ * synchronises `stream` before returning.  Weights, gate, signature tables and workspace stay on the device.
+ * `workspace` must hold eldr_moe_workspace_bytes_host(shape, T) bytes (layer workspace + staging). */
+int32_t eldr_moe_decode_layer_host(const eldr_moe_shape_t* shape, int32_t layer, int32_t T,
+                                   const eldr_bf16* h_x, const float* gate_w, const float* gate_bias,
+                                   const eldr_bf16* w13, const eldr_bf16* w2,
+                                   const eldr_bf16* shared_w13, const eldr_bf16* shared_w2,
+                                   eldr_bf16* h_out, int32_t* h_topk_ids, float* h_topk_w,
+                                   int32_t* h_n_active,
+                                   const int32_t* h_token_req, const int32_t* h_token_block,
+                                   int32_t* sig_req, int8_t* sig_block,
+                                   void* workspace, size_t workspace_bytes, eldr_stream_t stream);
+
+/* Signature accumulation alone, from already-computed top-k ids (prefill-shaped calls: "Each
+ * forward accumulates the new tokens' expert picks into the matching rows in a single GPU pass").
+ * Exact integer adds; the result does not depend on the order of tokens.  Any T >= 0. */
+int32_t eldr_signature_accumulate(const eldr_moe_shape_t* shape, int32_t layer, int32_t T,
+                                  const int32_t* topk_ids, const int32_t* token_req,
+                                  const int32_t* token_block, int32_t* sig_req, int8_t* sig_block,
+                                  eldr_stream_t stream);
+
+/* PAPER.md:253 "a reused block resets its signature": zero the L*E cells of each listed row (ids < 0 skipped). */
+int32_t eldr_signature_reset_blocks(const eldr_moe_shape_t* shape, const int32_t* block_ids, int32_t n,
+                                    int8_t* sig_block, eldr_stream_t stream);
+
+/* PAPER.md:253 "s_r = sum_{b in B(r)} sig[b]", "retrieving a request's signature sums its
+ * blocks' rows into its [L,E] signature": for request i, sums rows block_ids[req_off[i] .. req_off[i+1])
+ * of sig_block into sig_out[i] ([n_req,L,E] int32, overwritten). */
+int32_t eldr_signature_readout(const eldr_moe_shape_t* shape, const int32_t* block_ids,
+                               const int32_t* req_off, int32_t n_req, const int8_t* sig_block,
+                               int32_t* sig_out, eldr_stream_t stream);
+
+size_t  eldr_moe_workspace_bytes(const eldr_moe_shape_t* shape, int32_t max_T);
+size_t  eldr_moe_workspace_bytes_host(const eldr_moe_shape_t* shape, int32_t max_T);
+int32_t eldr_moe_workspace_layout(const eldr_moe_shape_t* shape, int32_t T, eldr_moe_ws_layout_t* layout);
+
+/* Per-kernel device timing of eldr_moe_decode_layer (measurement aid, off by default, per host thread).
+ * When enabled, the call records a CUDA event on `stream` before each of its kernels and after the last.
+ * eldr_moe_profile_read waits for the last call's events and writes the ELDR_PROFILE_SLOTS durations in
+ * milliseconds to HOST memory: [0] gate GEMV, [1] top-k/signature/permutation, [2] gather,
+ * [3] FFN w1/w3, [4] FFN w2, [5] combine (0 for a kernel that did not run). */
+#define ELDR_PROFILE_SLOTS 6
+int32_t eldr_moe_profile_enable(int32_t on);
+int32_t eldr_moe_profile_read(float* h_ms);
+
+/* Number of kernels the last eldr_moe_decode_layer call on this thread enqueued (bench accounting). */
+int32_t eldr_moe_last_launch_count(void);
+
+const char* eldr_status_string(int32_t status);
+/* Text of the last CUDA error seen by this thread inside the library ("" if none). */
+const char* eldr_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ELDR_MOE_H_ */

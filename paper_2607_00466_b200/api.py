@@ -1,0 +1,245 @@
+"""Thin Python binding of the C ABI in include/eldr_moe.h (argument marshalling only).
+
+Same names as the C entry points.  Every step of the path runs in the CUDA library
+(csrc/libeldr_moe.so); there is no CPU or PyTorch fallback: if the library is missing or a call
+fails, a RuntimeError is raised.  PyTorch is used for device memory and streams only.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+import torch
+
+from . import build as _build
+
+_lib = None
+
+EXPORTS = [
+    "eldr_moe_gate_topk", "eldr_moe_decode_layer", "eldr_moe_decode_layer_host",
+    "eldr_signature_accumulate", "eldr_signature_reset_blocks", "eldr_signature_readout",
+    "eldr_moe_workspace_bytes", "eldr_moe_workspace_bytes_host", "eldr_moe_workspace_layout",
+    "eldr_moe_last_launch_count", "eldr_status_string", "eldr_last_cuda_error",
+    "eldr_moe_profile_enable", "eldr_moe_profile_read",
+]
+PROFILE_SLOTS = ("gate", "route", "gather", "ffn13", "ffn2", "combine")
+
+
+class Shape(C.Structure):
+    """eldr_moe_shape_t"""
+    _fields_ = [(n, C.c_int32) for n in ("hidden", "inter", "n_experts", "top_k", "n_shared",
+                                         "renormalize", "n_layers", "kv_block_size")]
+
+
+class WsLayout(C.Structure):
+    """eldr_moe_ws_layout_t"""
+    _fields_ = [(n, C.c_size_t) for n in ("z", "cnt", "off", "perm", "pair_pos", "work", "n_work",
+                                          "x_perm", "h", "y", "total")]
+
+
+def lib_path() -> str:
+    return _build.LIB
+
+
+def load(build_if_missing: bool = False):
+    """dlopen the CUDA library.  Raises if it is not built (no fallback)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if not os.path.exists(path):
+        if build_if_missing:
+            _build.build()
+        else:
+            raise RuntimeError("CUDA library %s is not built; run `python -c 'import __graft_entry__ as g; "
+                               "g.build()'` (there is no CPU fallback)" % path)
+    lib = C.CDLL(path)
+    lib.eldr_moe_workspace_bytes.restype = C.c_size_t
+    lib.eldr_moe_workspace_bytes_host.restype = C.c_size_t
+    lib.eldr_status_string.restype = C.c_char_p
+    lib.eldr_last_cuda_error.restype = C.c_char_p
+    for n in EXPORTS:
+        getattr(lib, n)          # fail loudly if a declared symbol is missing
+    _lib = lib
+    return lib
+
+
+def make_shape(s) -> Shape:
+    return Shape(s.hidden, s.inter, s.n_experts, s.top_k, s.n_shared, s.renormalize, s.n_layers,
+                 s.kv_block_size)
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        lib = load()
+        raise RuntimeError("%s failed: %s (%d) %s" % (what, lib.eldr_status_string(rc).decode(), rc,
+                                                       lib.eldr_last_cuda_error().decode()))
+
+
+def _ptr(t: Optional[torch.Tensor], dtype=None, cuda: bool = True):
+    if t is None:
+        return C.c_void_p(0)
+    assert t.is_contiguous()
+    if dtype is not None:
+        assert t.dtype == dtype, (t.dtype, dtype)
+    assert t.is_cuda == cuda, "tensor on the wrong side of the PCIe bus"
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream():
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def bf16_from_bits(bits: np.ndarray, device="cuda") -> torch.Tensor:
+    """uint16 bf16 bit patterns (synth.py) -> torch.bfloat16 tensor (same bits)."""
+    t = torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).view(torch.bfloat16)
+    return t.to(device) if device is not None else t
+
+
+def bits_from_bf16(t: torch.Tensor) -> np.ndarray:
+    return t.detach().cpu().contiguous().view(torch.int16).numpy().view(np.uint16)
+
+
+def eldr_moe_workspace_bytes(shape, max_T: int) -> int:
+    s = make_shape(shape)
+    return int(load().eldr_moe_workspace_bytes(C.byref(s), C.c_int32(max_T)))
+
+
+def eldr_moe_workspace_bytes_host(shape, max_T: int) -> int:
+    s = make_shape(shape)
+    return int(load().eldr_moe_workspace_bytes_host(C.byref(s), C.c_int32(max_T)))
+
+
+def eldr_moe_workspace_layout(shape, T: int) -> WsLayout:
+    s = make_shape(shape)
+    L = WsLayout()
+    _check(load().eldr_moe_workspace_layout(C.byref(s), C.c_int32(T), C.byref(L)), "eldr_moe_workspace_layout")
+    return L
+
+
+def eldr_moe_last_launch_count() -> int:
+    return int(load().eldr_moe_last_launch_count())
+
+
+def eldr_moe_profile_enable(on: bool) -> None:
+    _check(load().eldr_moe_profile_enable(C.c_int32(1 if on else 0)), "eldr_moe_profile_enable")
+
+
+def eldr_moe_profile_read() -> dict:
+    """Per-kernel milliseconds of the last eldr_moe_decode_layer call (waits for it)."""
+    ms = (C.c_float * len(PROFILE_SLOTS))()
+    _check(load().eldr_moe_profile_read(ms), "eldr_moe_profile_read")
+    return dict(zip(PROFILE_SLOTS, [float(v) for v in ms]))
+
+
+def eldr_moe_gate_topk(shape, layer: int, x, gate_w, gate_bias, topk_ids, topk_w, token_req=None,
+                       token_block=None, sig_req=None, sig_block=None, workspace=None):
+    s = make_shape(shape)
+    T = x.shape[0]
+    _check(load().eldr_moe_gate_topk(
+        C.byref(s), C.c_int32(layer), C.c_int32(T), _ptr(x, torch.bfloat16), _ptr(gate_w, torch.float32),
+        _ptr(gate_bias, torch.float32), _ptr(topk_ids, torch.int32), _ptr(topk_w, torch.float32),
+        _ptr(token_req, torch.int32), _ptr(token_block, torch.int32), _ptr(sig_req, torch.int32),
+        _ptr(sig_block, torch.int8), _ptr(workspace), C.c_size_t(workspace.numel() * workspace.element_size()),
+        _stream()), "eldr_moe_gate_topk")
+
+
+def eldr_moe_decode_layer(shape, layer: int, x, gate_w, gate_bias, w13, w2, shared_w13, shared_w2, out,
+                          topk_ids, topk_w, force_routing: int, active_experts, n_active,
+                          token_req=None, token_block=None, sig_req=None, sig_block=None, workspace=None):
+    s = make_shape(shape)
+    T = x.shape[0]
+    _check(load().eldr_moe_decode_layer(
+        C.byref(s), C.c_int32(layer), C.c_int32(T), _ptr(x, torch.bfloat16), _ptr(gate_w, torch.float32),
+        _ptr(gate_bias, torch.float32), _ptr(w13, torch.bfloat16), _ptr(w2, torch.bfloat16),
+        _ptr(shared_w13, torch.bfloat16), _ptr(shared_w2, torch.bfloat16), _ptr(out, torch.bfloat16),
+        _ptr(topk_ids, torch.int32), _ptr(topk_w, torch.float32), C.c_int32(force_routing),
+        _ptr(active_experts, torch.int32), _ptr(n_active, torch.int32),
+        _ptr(token_req, torch.int32), _ptr(token_block, torch.int32), _ptr(sig_req, torch.int32),
+        _ptr(sig_block, torch.int8), _ptr(workspace), C.c_size_t(workspace.numel() * workspace.element_size()),
+        _stream()), "eldr_moe_decode_layer")
+
+
+def eldr_moe_decode_layer_host(shape, layer: int, h_x, gate_w, gate_bias, w13, w2, shared_w13, shared_w2,
+                               h_out, h_topk_ids, h_topk_w, h_n_active, h_token_req=None, h_token_block=None,
+                               sig_req=None, sig_block=None, workspace=None):
+    """h_* are HOST (pinned) tensors; everything else lives on the device.  Synchronous."""
+    s = make_shape(shape)
+    T = h_x.shape[0]
+    _check(load().eldr_moe_decode_layer_host(
+        C.byref(s), C.c_int32(layer), C.c_int32(T), _ptr(h_x, torch.bfloat16, cuda=False),
+        _ptr(gate_w, torch.float32), _ptr(gate_bias, torch.float32), _ptr(w13, torch.bfloat16),
+        _ptr(w2, torch.bfloat16), _ptr(shared_w13, torch.bfloat16), _ptr(shared_w2, torch.bfloat16),
+        _ptr(h_out, torch.bfloat16, cuda=False), _ptr(h_topk_ids, torch.int32, cuda=False),
+        _ptr(h_topk_w, torch.float32, cuda=False), _ptr(h_n_active, torch.int32, cuda=False),
+        _ptr(h_token_req, torch.int32, cuda=False), _ptr(h_token_block, torch.int32, cuda=False),
+        _ptr(sig_req, torch.int32), _ptr(sig_block, torch.int8), _ptr(workspace),
+        C.c_size_t(workspace.numel() * workspace.element_size()), _stream()), "eldr_moe_decode_layer_host")
+
+
+def eldr_signature_accumulate(shape, layer: int, topk_ids, token_req, token_block, sig_req, sig_block):
+    s = make_shape(shape)
+    T = topk_ids.shape[0]
+    _check(load().eldr_signature_accumulate(
+        C.byref(s), C.c_int32(layer), C.c_int32(T), _ptr(topk_ids, torch.int32), _ptr(token_req, torch.int32),
+        _ptr(token_block, torch.int32), _ptr(sig_req, torch.int32), _ptr(sig_block, torch.int8), _stream()),
+        "eldr_signature_accumulate")
+
+
+def eldr_signature_reset_blocks(shape, block_ids, sig_block):
+    s = make_shape(shape)
+    _check(load().eldr_signature_reset_blocks(C.byref(s), _ptr(block_ids, torch.int32),
+                                              C.c_int32(block_ids.numel()), _ptr(sig_block, torch.int8),
+                                              _stream()), "eldr_signature_reset_blocks")
+
+
+def eldr_signature_readout(shape, block_ids, req_off, sig_block, sig_out):
+    s = make_shape(shape)
+    _check(load().eldr_signature_readout(C.byref(s), _ptr(block_ids, torch.int32), _ptr(req_off, torch.int32),
+                                         C.c_int32(req_off.numel() - 1), _ptr(sig_block, torch.int8),
+                                         _ptr(sig_out, torch.int32), _stream()), "eldr_signature_readout")
+
+
+class DecodeLayer:
+    """Convenience holder of one layer's device tensors + workspace (plumbing; no arithmetic)."""
+
+    def __init__(self, shape, lw, max_T: int, device="cuda"):
+        self.shape = shape
+        self.gate_w = torch.from_numpy(lw.gate_w).to(device)
+        self.w13 = bf16_from_bits(lw.w13, device)
+        self.w2 = bf16_from_bits(lw.w2, device)
+        self.shared_w13 = bf16_from_bits(lw.shared_w13, device) if lw.shared_w13 is not None else None
+        self.shared_w2 = bf16_from_bits(lw.shared_w2, device) if lw.shared_w2 is not None else None
+        self.max_T = max_T
+        self.workspace = torch.empty(eldr_moe_workspace_bytes_host(shape, max_T), dtype=torch.uint8, device=device)
+        E, k, H = shape.n_experts, shape.top_k, shape.hidden
+        self.out = torch.empty((max_T, H), dtype=torch.bfloat16, device=device)
+        self.ids = torch.empty((max_T, k), dtype=torch.int32, device=device)
+        self.w = torch.empty((max_T, k), dtype=torch.float32, device=device)
+        self.active = torch.empty((E,), dtype=torch.int32, device=device)
+        self.n_active = torch.zeros((1,), dtype=torch.int32, device=device)
+
+    def run(self, x, gate_bias=None, layer=0, force_routing=0, token_req=None, token_block=None,
+            sig_req=None, sig_block=None):
+        T = x.shape[0]
+        eldr_moe_decode_layer(self.shape, layer, x, self.gate_w, gate_bias, self.w13, self.w2,
+                              self.shared_w13, self.shared_w2, self.out[:T], self.ids[:T], self.w[:T],
+                              force_routing, self.active, self.n_active, token_req, token_block,
+                              sig_req, sig_block, self.workspace)
+        return self.out[:T]
+
+    def ws_view(self, name: str, T: int):
+        """Typed view of one workspace intermediate (for per-kernel parity tests)."""
+        L = eldr_moe_workspace_layout(self.shape, T)
+        s = self.shape
+        k, E, H, I, ns = s.top_k, s.n_experts, s.hidden, s.inter, s.n_shared
+        spec = {"z": (torch.float32, (T, E)), "cnt": (torch.int32, (E,)), "off": (torch.int32, (E + 1,)),
+                "perm": (torch.int32, (T * k,)), "pair_pos": (torch.int32, (T * k,)),
+                "work": (torch.int32, (E + ns, 4)), "n_work": (torch.int32, (1,)),
+                "x_perm": (torch.bfloat16, (T * k + T, H)), "h": (torch.bfloat16, (T * (k + ns), I)),
+                "y": (torch.float32, (T * (k + ns), H))}[name]
+        off = getattr(L, name)
+        n = int(np.prod(spec[1])) * torch.empty((), dtype=spec[0]).element_size()
+        return self.workspace[off: off + n].view(spec[0]).view(spec[1])

@@ -1,0 +1,465 @@
+// C ABI of the B200 decode-MoE layer (include/eldr_moe.h): argument validation, workspace carving, TMA
+// descriptor construction and kernel launches.  No device allocation, no host synchronisation (except the
+// *_host entry point, synchronous by contract).
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+
+#include "eldr_moe.h"
+#include "ffn_stream.cuh"
+#include "gate_route.cuh"
+
+namespace {
+
+using namespace eldr;
+
+thread_local char g_err[256] = "";
+thread_local int g_launches = 0;
+
+// optional per-kernel event timing (eldr_moe_profile_enable)
+thread_local bool g_prof_on = false;
+thread_local cudaEvent_t g_prof_ev[ELDR_PROFILE_SLOTS + 1];
+thread_local bool g_prof_ev_made = false;
+thread_local int g_prof_mark[ELDR_PROFILE_SLOTS + 1];   // event index recorded before kernel slot i (-1: not run)
+thread_local int g_prof_n = 0;
+
+void prof_begin() {
+  if (!g_prof_on) return;
+  if (!g_prof_ev_made) {
+    for (auto& e : g_prof_ev) cudaEventCreate(&e);
+    g_prof_ev_made = true;
+  }
+  for (auto& m : g_prof_mark) m = -1;
+  g_prof_n = 0;
+}
+// record "kernel `slot` starts here" (slot == ELDR_PROFILE_SLOTS: end of the call)
+void prof_mark(int slot, cudaStream_t st) {
+  if (!g_prof_on) return;
+  cudaEventRecord(g_prof_ev[g_prof_n], st);
+  g_prof_mark[slot] = g_prof_n++;
+}
+
+bool cuda_ok(cudaError_t e, const char* what) {
+  if (e == cudaSuccess) return true;
+  snprintf(g_err, sizeof(g_err), "%s: %s", what, cudaGetErrorString(e));
+  return false;
+}
+bool launch_ok(const char* what) {
+  ++g_launches;
+  return cuda_ok(cudaGetLastError(), what);
+}
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+int32_t check_shape(const eldr_moe_shape_t* s) {
+  if (!s) return ELDR_ERR_INVALID_ARG;
+  if (s->hidden < 8 || s->hidden % 8 || s->inter < 8 || s->inter % 8) return ELDR_ERR_INVALID_ARG;
+  if (s->n_experts < 1 || s->n_experts > kMaxExperts) return ELDR_ERR_INVALID_ARG;
+  if (s->top_k < 1 || s->top_k > s->n_experts || s->top_k > kMaxTopK) return ELDR_ERR_INVALID_ARG;
+  if (s->n_shared < 0 || s->n_shared > 8) return ELDR_ERR_INVALID_ARG;
+  if (s->n_layers < 1) return ELDR_ERR_INVALID_ARG;
+  if (s->kv_block_size < 1 || s->kv_block_size > 127) return ELDR_ERR_INVALID_ARG;
+  return ELDR_OK;
+}
+
+void make_layout(const eldr_moe_shape_t* s, int T, eldr_moe_ws_layout_t* L) {
+  const size_t H = s->hidden, I = s->inter, E = s->n_experts, k = s->top_k, ns = s->n_shared;
+  const size_t Tz = T > 0 ? T : 1;
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + bytes, 256); return r; };
+  L->z = take(Tz * E * 4);
+  L->cnt = take(E * 4);
+  L->off = take((E + 1) * 4);
+  L->perm = take(Tz * k * 4);
+  L->pair_pos = take(Tz * k * 4);
+  L->work = take((E + ns) * 16);
+  L->n_work = take(4);
+  L->x_perm = take((Tz * k + Tz) * H * 2);
+  L->h = take(Tz * (k + ns) * I * 2);
+  L->y = take(Tz * (k + ns) * H * 4);
+  L->total = o;
+}
+
+// staging block appended to the layer workspace by eldr_moe_decode_layer_host
+struct HostStage { size_t x, req, blk, out, ids, w, active, n_active, total; };
+void make_host_stage(const eldr_moe_shape_t* s, int T, size_t base, HostStage* S) {
+  const size_t H = s->hidden, E = s->n_experts, k = s->top_k, Tz = T > 0 ? T : 1;
+  size_t o = base;
+  auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + bytes, 256); return r; };
+  S->x = take(Tz * H * 2); S->req = take(Tz * 4); S->blk = take(Tz * 4); S->out = take(Tz * H * 2);
+  S->ids = take(Tz * k * 4); S->w = take(Tz * k * 4); S->active = take(E * 4); S->n_active = take(4);
+  S->total = o;
+}
+
+int num_sms() {
+  static int n = 0;
+  if (n == 0) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
+    if (n <= 0) n = 148;
+  }
+  return n;
+}
+
+// ---------------------------------------------------------------------------- TMA descriptors
+typedef CUresult (*encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
+                                    CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                    CUtensorMapFloatOOBfill);
+
+encode_tiled_fn get_encode_fn() {
+  static encode_tiled_fn fn = nullptr;
+  static std::once_flag once;
+  std::call_once(once, [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<encode_tiled_fn>(p);
+  });
+  return fn;
+}
+
+// bf16 [rows, cols] row-major, box = box_rows x 64 columns (128 bytes), SWIZZLE_128B, OOB reads give zeros.
+// Descriptors are pure functions of (ptr, rows, cols, box_rows); a small cache avoids re-encoding the
+// static weight descriptors every step.
+struct TmapKey { const void* p; uint64_t rows, cols; uint32_t box_rows; };
+struct TmapSlot { TmapKey k; CUtensorMap m; bool used; };
+std::mutex g_tm_mu;
+TmapSlot g_tm_cache[64];
+int g_tm_next = 0;
+
+bool make_tmap(CUtensorMap* out, const void* ptr, uint64_t rows, uint64_t cols, uint32_t box_rows) {
+  {
+    std::lock_guard<std::mutex> lk(g_tm_mu);
+    for (auto& s : g_tm_cache)
+      if (s.used && s.k.p == ptr && s.k.rows == rows && s.k.cols == cols && s.k.box_rows == box_rows) {
+        *out = s.m;
+        return true;
+      }
+  }
+  encode_tiled_fn fn = get_encode_fn();
+  if (!fn) { snprintf(g_err, sizeof(g_err), "cuTensorMapEncodeTiled entry point not found"); return false; }
+  cuuint64_t gdim[2] = {cols, rows};
+  cuuint64_t gstride[1] = {cols * 2};
+  cuuint32_t box[2] = {64, box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptr), gdim, gstride, box, estr,
+                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) { snprintf(g_err, sizeof(g_err), "cuTensorMapEncodeTiled failed: %d", (int)r); return false; }
+  std::lock_guard<std::mutex> lk(g_tm_mu);
+  TmapSlot& s = g_tm_cache[g_tm_next];
+  g_tm_next = (g_tm_next + 1) % 64;
+  s.k = TmapKey{ptr, rows, cols, box_rows};
+  s.m = *out;
+  s.used = true;
+  return true;
+}
+
+template <typename K>
+bool set_smem(K kernel, size_t bytes) {
+  return cuda_ok(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes),
+                 "cudaFuncSetAttribute(smem)");
+}
+
+int32_t launch_gate_logits(const eldr_moe_shape_t* s, int T, const eldr_bf16* x, const float* gate_w,
+                           const float* gate_bias, float* z, cudaStream_t st) {
+  const size_t smem = (size_t)kGateTok * s->hidden * 2;
+  if (smem > 200 * 1024) return ELDR_ERR_UNSUPPORTED;
+  if (smem > 48 * 1024 && !set_smem(gate_logits_kernel, smem)) return ELDR_ERR_CUDA;
+  dim3 grid((s->n_experts + kGateExp - 1) / kGateExp, (T + kGateTok - 1) / kGateTok);
+  gate_logits_kernel<<<grid, 256, smem, st>>>(x, gate_w, gate_bias, z, T, s->hidden, s->n_experts);
+  return launch_ok("gate_logits_kernel") ? ELDR_OK : ELDR_ERR_CUDA;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* eldr_status_string(int32_t st) {
+  switch (st) {
+    case ELDR_OK: return "ok";
+    case ELDR_ERR_INVALID_ARG: return "invalid argument";
+    case ELDR_ERR_UNSUPPORTED: return "unsupported shape";
+    case ELDR_ERR_WORKSPACE_SMALL: return "workspace too small";
+    case ELDR_ERR_CUDA: return "CUDA error";
+    default: return "unknown status";
+  }
+}
+
+const char* eldr_last_cuda_error(void) { return g_err; }
+
+int32_t eldr_moe_profile_enable(int32_t on) {
+  g_prof_on = on != 0;
+  return ELDR_OK;
+}
+
+int32_t eldr_moe_profile_read(float* h_ms) {
+  if (!h_ms) return ELDR_ERR_INVALID_ARG;
+  for (int i = 0; i < ELDR_PROFILE_SLOTS; ++i) h_ms[i] = 0.f;
+  if (!g_prof_ev_made || g_prof_n < 2 || g_prof_mark[ELDR_PROFILE_SLOTS] < 0) return ELDR_ERR_INVALID_ARG;
+  if (!cuda_ok(cudaEventSynchronize(g_prof_ev[g_prof_mark[ELDR_PROFILE_SLOTS]]), "profile sync")) return ELDR_ERR_CUDA;
+  for (int i = 0; i < ELDR_PROFILE_SLOTS; ++i) {
+    if (g_prof_mark[i] < 0) continue;
+    // the next recorded event after this kernel's start marks its end
+    if (!cuda_ok(cudaEventElapsedTime(&h_ms[i], g_prof_ev[g_prof_mark[i]], g_prof_ev[g_prof_mark[i] + 1]), "profile elapsed"))
+      return ELDR_ERR_CUDA;
+  }
+  return ELDR_OK;
+}
+int32_t eldr_moe_last_launch_count(void) { return g_launches; }
+
+size_t eldr_moe_workspace_bytes(const eldr_moe_shape_t* shape, int32_t max_T) {
+  if (check_shape(shape) != ELDR_OK || max_T < 0) return 0;
+  eldr_moe_ws_layout_t L;
+  make_layout(shape, max_T, &L);
+  return L.total;
+}
+
+size_t eldr_moe_workspace_bytes_host(const eldr_moe_shape_t* shape, int32_t max_T) {
+  if (check_shape(shape) != ELDR_OK || max_T < 0) return 0;
+  eldr_moe_ws_layout_t L;
+  make_layout(shape, max_T, &L);
+  HostStage S;
+  make_host_stage(shape, max_T, L.total, &S);
+  return S.total;
+}
+
+int32_t eldr_moe_workspace_layout(const eldr_moe_shape_t* shape, int32_t T, eldr_moe_ws_layout_t* layout) {
+  if (check_shape(shape) != ELDR_OK || T < 0 || !layout) return ELDR_ERR_INVALID_ARG;
+  make_layout(shape, T, layout);
+  return ELDR_OK;
+}
+
+int32_t eldr_moe_gate_topk(const eldr_moe_shape_t* s, int32_t layer, int32_t T, const eldr_bf16* x,
+                           const float* gate_w, const float* gate_bias, int32_t* topk_ids, float* topk_w,
+                           const int32_t* token_req, const int32_t* token_block, int32_t* sig_req,
+                           int8_t* sig_block, void* workspace, size_t workspace_bytes, eldr_stream_t stream) {
+  g_launches = 0;
+  int32_t rc = check_shape(s);
+  if (rc != ELDR_OK) return rc;
+  if (T < 0 || layer < 0 || layer >= s->n_layers) return ELDR_ERR_INVALID_ARG;
+  if (T == 0) return ELDR_OK;
+  if (!x || !gate_w || !topk_ids || !topk_w || !workspace) return ELDR_ERR_INVALID_ARG;
+  if (!aligned16(x) || !aligned16(gate_w) || !aligned16(workspace) || !aligned16(sig_block)) return ELDR_ERR_INVALID_ARG;
+  if (workspace_bytes < align_up((size_t)T * s->n_experts * 4, 256)) return ELDR_ERR_WORKSPACE_SMALL;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  float* z = static_cast<float*>(workspace);
+  rc = launch_gate_logits(s, T, x, gate_w, gate_bias, z, st);
+  if (rc != ELDR_OK) return rc;
+  TopkArgs a{z, topk_ids, topk_w, token_req, token_block, sig_req, sig_block,
+             T, s->n_experts, s->top_k, s->n_layers, layer, s->renormalize};
+  topk_kernel<<<(T + 7) / 8, 256, 0, st>>>(a);
+  return launch_ok("topk_kernel") ? ELDR_OK : ELDR_ERR_CUDA;
+}
+
+int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t T, const eldr_bf16* x,
+                              const float* gate_w, const float* gate_bias, const eldr_bf16* w13,
+                              const eldr_bf16* w2, const eldr_bf16* shared_w13, const eldr_bf16* shared_w2,
+                              eldr_bf16* out, int32_t* topk_ids, float* topk_w, int32_t force_routing,
+                              int32_t* active_experts, int32_t* n_active, const int32_t* token_req,
+                              const int32_t* token_block, int32_t* sig_req, int8_t* sig_block,
+                              void* workspace, size_t workspace_bytes, eldr_stream_t stream) {
+  g_launches = 0;
+  int32_t rc = check_shape(s);
+  if (rc != ELDR_OK) return rc;
+  if (T < 0 || layer < 0 || layer >= s->n_layers) return ELDR_ERR_INVALID_ARG;
+  if (T == 0) return ELDR_OK;
+  if (T > 1024) return ELDR_ERR_UNSUPPORTED;
+  if (!x || !w13 || !w2 || !out || !topk_ids || !topk_w || !active_experts || !n_active || !workspace)
+    return ELDR_ERR_INVALID_ARG;
+  if (!force_routing && !gate_w) return ELDR_ERR_INVALID_ARG;
+  if (s->n_shared > 0 && (!shared_w13 || !shared_w2)) return ELDR_ERR_INVALID_ARG;
+  if (!aligned16(x) || !aligned16(gate_w) || !aligned16(w13) || !aligned16(w2) || !aligned16(shared_w13) ||
+      !aligned16(shared_w2) || !aligned16(out) || !aligned16(workspace) || !aligned16(sig_block))
+    return ELDR_ERR_INVALID_ARG;
+  eldr_moe_ws_layout_t L;
+  make_layout(s, T, &L);
+  if (workspace_bytes < L.total) return ELDR_ERR_WORKSPACE_SMALL;
+
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  uint8_t* ws = static_cast<uint8_t*>(workspace);
+  const int H = s->hidden, I = s->inter, E = s->n_experts, k = s->top_k, ns = s->n_shared;
+  float* z = reinterpret_cast<float*>(ws + L.z);
+  int32_t* perm = reinterpret_cast<int32_t*>(ws + L.perm);
+  int32_t* pair_pos = reinterpret_cast<int32_t*>(ws + L.pair_pos);
+  int4* work = reinterpret_cast<int4*>(ws + L.work);
+  int32_t* n_work = reinterpret_cast<int32_t*>(ws + L.n_work);
+  uint16_t* x_perm = reinterpret_cast<uint16_t*>(ws + L.x_perm);
+  uint16_t* hbuf = reinterpret_cast<uint16_t*>(ws + L.h);
+  float* ybuf = reinterpret_cast<float*>(ws + L.y);
+
+  prof_begin();
+  // a1: gate logits
+  if (!force_routing) {
+    prof_mark(0, st);
+    rc = launch_gate_logits(s, T, x, gate_w, gate_bias, z, st);
+    if (rc != ELDR_OK) return rc;
+  }
+  // a2-a4: top-k (+signature), permutation, union compaction -- one CTA
+  {
+    RouteArgs ra;
+    ra.tk = TopkArgs{z, topk_ids, topk_w, token_req, token_block, sig_req, sig_block,
+                     T, E, k, s->n_layers, layer, s->renormalize};
+    ra.force_routing = force_routing ? 1 : 0;
+    ra.n_shared = ns;
+    ra.cnt = reinterpret_cast<int32_t*>(ws + L.cnt);
+    ra.off = reinterpret_cast<int32_t*>(ws + L.off);
+    ra.perm = perm;
+    ra.pair_pos = pair_pos;
+    ra.work = work;
+    ra.n_work = n_work;
+    ra.active = active_experts;
+    ra.n_active = n_active;
+    const int W = (T + 31) / 32;
+    const size_t smem = (size_t)E * W * 8 + (size_t)(2 * E + 1) * 4;
+    if (smem > 48 * 1024 && !set_smem(topk_route_kernel, smem)) return ELDR_ERR_CUDA;
+    prof_mark(1, st);
+    topk_route_kernel<<<1, 1024, smem, st>>>(ra);
+    if (!launch_ok("topk_route_kernel")) return ELDR_ERR_CUDA;
+  }
+  // gather token rows in expert-sorted order (+ plain copy for the shared experts)
+  const int x_rows = T * k + (ns ? T : 0);
+  const int out_rows = T * (k + ns);
+  prof_mark(2, st);
+  gather_x_kernel<<<(x_rows + 7) / 8, 256, 0, st>>>(x, perm, x_perm, T, H, k, x_rows);
+  if (!launch_ok("gather_x_kernel")) return ELDR_ERR_CUDA;
+
+  // a5/a6: grouped SwiGLU FFN over the active experts
+  const int max_work = (E < T * k ? E : T * k) + ns;
+  FfnArgs f13{work, n_work, E, H, 2 * I, I, H, I / 64, hbuf, nullptr};
+  FfnArgs f2{work, n_work, E, I, H, I, H, (H + 127) / 128, nullptr, ybuf};
+  if (H % 64 == 0 && I % 64 == 0) {
+    CUtensorMap tm_w13, tm_sw13, tm_x, tm_w2, tm_sw2, tm_h;
+    if (!make_tmap(&tm_w13, w13, (uint64_t)E * 2 * I, H, 64)) return ELDR_ERR_CUDA;
+    if (!make_tmap(&tm_w2, w2, (uint64_t)E * H, I, 128)) return ELDR_ERR_CUDA;
+    if (ns) {
+      if (!make_tmap(&tm_sw13, shared_w13, (uint64_t)ns * 2 * I, H, 64)) return ELDR_ERR_CUDA;
+      if (!make_tmap(&tm_sw2, shared_w2, (uint64_t)ns * H, I, 128)) return ELDR_ERR_CUDA;
+    } else {
+      tm_sw13 = tm_w13;
+      tm_sw2 = tm_w2;
+    }
+    if (!make_tmap(&tm_x, x_perm, (uint64_t)x_rows, H, kFfnXBox)) return ELDR_ERR_CUDA;
+    if (!make_tmap(&tm_h, hbuf, (uint64_t)out_rows, I, kFfnXBox)) return ELDR_ERR_CUDA;
+    static bool attr_set = false;
+    if (!attr_set) {
+      if (!set_smem(ffn_stream_kernel<0>, kFfnSmemBytes) || !set_smem(ffn_stream_kernel<1>, kFfnSmemBytes))
+        return ELDR_ERR_CUDA;
+      attr_set = true;
+    }
+    const int sms = num_sms();
+    int g13 = max_work * f13.tiles_per_expert; if (g13 > sms) g13 = sms;
+    int g2 = max_work * f2.tiles_per_expert; if (g2 > sms) g2 = sms;
+    prof_mark(3, st);
+    ffn_stream_kernel<0><<<g13, kFfnThreads, kFfnSmemBytes, st>>>(tm_w13, tm_sw13, tm_x, f13);
+    if (!launch_ok("ffn_stream_kernel<w13>")) return ELDR_ERR_CUDA;
+    prof_mark(4, st);
+    ffn_stream_kernel<1><<<g2, kFfnThreads, kFfnSmemBytes, st>>>(tm_w2, tm_sw2, tm_h, f2);
+    if (!launch_ok("ffn_stream_kernel<w2>")) return ELDR_ERR_CUDA;
+  } else {
+    dim3 g13(max_work, (I + 127) / 128), g2(max_work, (H + 127) / 128);
+    prof_mark(3, st);
+    ffn13_plain_kernel<<<g13, 128, 0, st>>>(w13, shared_w13, x_perm, f13);
+    if (!launch_ok("ffn13_plain_kernel")) return ELDR_ERR_CUDA;
+    prof_mark(4, st);
+    ffn2_plain_kernel<<<g2, 128, 0, st>>>(w2, shared_w2, hbuf, f2);
+    if (!launch_ok("ffn2_plain_kernel")) return ELDR_ERR_CUDA;
+  }
+  // a7: weighted combine
+  prof_mark(5, st);
+  combine_kernel<<<(T * (H / 4) + 255) / 256, 256, 0, st>>>(ybuf, topk_w, pair_pos, out, T, H, k, ns);
+  if (!launch_ok("combine_kernel")) return ELDR_ERR_CUDA;
+  prof_mark(ELDR_PROFILE_SLOTS, st);
+  return ELDR_OK;
+}
+
+int32_t eldr_moe_decode_layer_host(const eldr_moe_shape_t* s, int32_t layer, int32_t T, const eldr_bf16* h_x,
+                                   const float* gate_w, const float* gate_bias, const eldr_bf16* w13,
+                                   const eldr_bf16* w2, const eldr_bf16* shared_w13, const eldr_bf16* shared_w2,
+                                   eldr_bf16* h_out, int32_t* h_topk_ids, float* h_topk_w, int32_t* h_n_active,
+                                   const int32_t* h_token_req, const int32_t* h_token_block, int32_t* sig_req,
+                                   int8_t* sig_block, void* workspace, size_t workspace_bytes,
+                                   eldr_stream_t stream) {
+  int32_t rc = check_shape(s);
+  if (rc != ELDR_OK) return rc;
+  if (T < 0) return ELDR_ERR_INVALID_ARG;
+  if (T == 0) return ELDR_OK;
+  if (!h_x || !h_out || !workspace) return ELDR_ERR_INVALID_ARG;
+  eldr_moe_ws_layout_t L;
+  make_layout(s, T, &L);
+  HostStage S;
+  make_host_stage(s, T, L.total, &S);
+  if (workspace_bytes < S.total) return ELDR_ERR_WORKSPACE_SMALL;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  uint8_t* ws = static_cast<uint8_t*>(workspace);
+  const size_t H = s->hidden, k = s->top_k;
+  if (!cuda_ok(cudaMemcpyAsync(ws + S.x, h_x, (size_t)T * H * 2, cudaMemcpyHostToDevice, st), "H2D x")) return ELDR_ERR_CUDA;
+  if (h_token_req && !cuda_ok(cudaMemcpyAsync(ws + S.req, h_token_req, (size_t)T * 4, cudaMemcpyHostToDevice, st), "H2D req")) return ELDR_ERR_CUDA;
+  if (h_token_block && !cuda_ok(cudaMemcpyAsync(ws + S.blk, h_token_block, (size_t)T * 4, cudaMemcpyHostToDevice, st), "H2D blk")) return ELDR_ERR_CUDA;
+  rc = eldr_moe_decode_layer(s, layer, T, reinterpret_cast<eldr_bf16*>(ws + S.x), gate_w, gate_bias, w13, w2,
+                             shared_w13, shared_w2, reinterpret_cast<eldr_bf16*>(ws + S.out),
+                             reinterpret_cast<int32_t*>(ws + S.ids), reinterpret_cast<float*>(ws + S.w), 0,
+                             reinterpret_cast<int32_t*>(ws + S.active), reinterpret_cast<int32_t*>(ws + S.n_active),
+                             h_token_req ? reinterpret_cast<int32_t*>(ws + S.req) : nullptr,
+                             h_token_block ? reinterpret_cast<int32_t*>(ws + S.blk) : nullptr, sig_req, sig_block,
+                             workspace, L.total, stream);
+  if (rc != ELDR_OK) return rc;
+  if (!cuda_ok(cudaMemcpyAsync(h_out, ws + S.out, (size_t)T * H * 2, cudaMemcpyDeviceToHost, st), "D2H out")) return ELDR_ERR_CUDA;
+  if (h_topk_ids && !cuda_ok(cudaMemcpyAsync(h_topk_ids, ws + S.ids, (size_t)T * k * 4, cudaMemcpyDeviceToHost, st), "D2H ids")) return ELDR_ERR_CUDA;
+  if (h_topk_w && !cuda_ok(cudaMemcpyAsync(h_topk_w, ws + S.w, (size_t)T * k * 4, cudaMemcpyDeviceToHost, st), "D2H w")) return ELDR_ERR_CUDA;
+  if (h_n_active && !cuda_ok(cudaMemcpyAsync(h_n_active, ws + S.n_active, 4, cudaMemcpyDeviceToHost, st), "D2H n_active")) return ELDR_ERR_CUDA;
+  if (!cuda_ok(cudaStreamSynchronize(st), "stream sync")) return ELDR_ERR_CUDA;
+  return ELDR_OK;
+}
+
+int32_t eldr_signature_accumulate(const eldr_moe_shape_t* s, int32_t layer, int32_t T, const int32_t* topk_ids,
+                                  const int32_t* token_req, const int32_t* token_block, int32_t* sig_req,
+                                  int8_t* sig_block, eldr_stream_t stream) {
+  g_launches = 0;
+  int32_t rc = check_shape(s);
+  if (rc != ELDR_OK) return rc;
+  if (T < 0 || layer < 0 || layer >= s->n_layers) return ELDR_ERR_INVALID_ARG;
+  if (T == 0) return ELDR_OK;
+  if (!topk_ids || !aligned16(sig_block)) return ELDR_ERR_INVALID_ARG;
+  const long long pairs = (long long)T * s->top_k;
+  sig_accumulate_kernel<<<(unsigned)((pairs + 255) / 256), 256, 0, static_cast<cudaStream_t>(stream)>>>(
+      topk_ids, token_req, token_block, sig_req, sig_block, T, s->n_experts, s->top_k, s->n_layers, layer);
+  return launch_ok("sig_accumulate_kernel") ? ELDR_OK : ELDR_ERR_CUDA;
+}
+
+int32_t eldr_signature_reset_blocks(const eldr_moe_shape_t* s, const int32_t* block_ids, int32_t n,
+                                    int8_t* sig_block, eldr_stream_t stream) {
+  g_launches = 0;
+  int32_t rc = check_shape(s);
+  if (rc != ELDR_OK) return rc;
+  if (n < 0) return ELDR_ERR_INVALID_ARG;
+  if (n == 0) return ELDR_OK;
+  if (!block_ids || !sig_block || !aligned16(sig_block)) return ELDR_ERR_INVALID_ARG;
+  sig_reset_kernel<<<n, 256, 0, static_cast<cudaStream_t>(stream)>>>(block_ids, sig_block,
+                                                                    s->n_layers * s->n_experts);
+  return launch_ok("sig_reset_kernel") ? ELDR_OK : ELDR_ERR_CUDA;
+}
+
+int32_t eldr_signature_readout(const eldr_moe_shape_t* s, const int32_t* block_ids, const int32_t* req_off,
+                               int32_t n_req, const int8_t* sig_block, int32_t* sig_out, eldr_stream_t stream) {
+  g_launches = 0;
+  int32_t rc = check_shape(s);
+  if (rc != ELDR_OK) return rc;
+  if (n_req < 0) return ELDR_ERR_INVALID_ARG;
+  if (n_req == 0) return ELDR_OK;
+  if (!block_ids || !req_off || !sig_block || !sig_out) return ELDR_ERR_INVALID_ARG;
+  const int cells = s->n_layers * s->n_experts;
+  dim3 grid((cells + 255) / 256 < 64 ? (cells + 255) / 256 : 64, n_req);
+  sig_readout_kernel<<<grid, 256, 0, static_cast<cudaStream_t>(stream)>>>(block_ids, req_off, sig_block, sig_out,
+                                                                       cells);
+  return launch_ok("sig_readout_kernel") ? ELDR_OK : ELDR_ERR_CUDA;
+}
+
+}  // extern "C"

@@ -1,0 +1,364 @@
+// Gate GEMV, warp-shuffle softmax top-k, fused ELDR signature accumulation, token->expert permutation
+// with union compaction, gather, combine.  (SURVEY.md 8(a) steps a1-a4, a7.)
+#pragma once
+#include "device_utils.cuh"
+
+namespace eldr {
+
+constexpr int kMaxExperts = 256;   // 8 logits per lane in the warp top-k
+constexpr int kMaxTopK = 16;
+constexpr int kGateTok = 8;        // tokens per CTA in the gate GEMV
+constexpr int kGateExp = 8;        // experts per CTA (= warps)
+
+// ------------------------------------------------------------------------------------ a1: gate GEMV
+// z[t,e] = sum_h x[t,h]*Wg[e,h] + bias[e], fp32 FMA on CUDA cores (no TF32/bf16 MMA: near-ties must not
+// flip).  CTA = 8 warps: warp w owns expert blockIdx.x*8+w against an 8-token x tile held in smem as bf16.
+__global__ void __launch_bounds__(256) gate_logits_kernel(const uint16_t* __restrict__ x,
+                                                          const float* __restrict__ gate_w,
+                                                          const float* __restrict__ gate_bias,
+                                                          float* __restrict__ z, int T, int H, int E) {
+  extern __shared__ __align__(16) uint8_t smem_raw[];
+  uint4* xs4 = reinterpret_cast<uint4*>(smem_raw);
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int t0 = blockIdx.y * kGateTok;
+  const int vec_per_row = H >> 3;
+  for (int v = tid; v < kGateTok * vec_per_row; v += 256) {
+    const int t = v / vec_per_row, c = v - t * vec_per_row;
+    uint4 val = make_uint4(0u, 0u, 0u, 0u);
+    if (t0 + t < T) val = *reinterpret_cast<const uint4*>(x + (size_t)(t0 + t) * H + (size_t)c * 8);
+    xs4[v] = val;
+  }
+  __syncthreads();
+  const int e = blockIdx.x * kGateExp + warp;
+  if (e >= E) return;
+  float acc[kGateTok];
+#pragma unroll
+  for (int t = 0; t < kGateTok; ++t) acc[t] = 0.f;
+  const float4* wrow = reinterpret_cast<const float4*>(gate_w + (size_t)e * H);
+  const uint2* xs2 = reinterpret_cast<const uint2*>(smem_raw);
+  const int q_per_row = H >> 2;
+  for (int c4 = lane; c4 < q_per_row; c4 += 32) {
+    const float4 wv = __ldg(wrow + c4);
+#pragma unroll
+    for (int t = 0; t < kGateTok; ++t) {
+      const uint2 xv = xs2[t * q_per_row + c4];
+      float a = acc[t];
+      a = fmaf(wv.x, bf16_lo(xv.x), a);
+      a = fmaf(wv.y, bf16_hi(xv.x), a);
+      a = fmaf(wv.z, bf16_lo(xv.y), a);
+      a = fmaf(wv.w, bf16_hi(xv.y), a);
+      acc[t] = a;
+    }
+  }
+#pragma unroll
+  for (int t = 0; t < kGateTok; ++t) {
+    float a = acc[t];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+    acc[t] = a;
+  }
+  if (lane == 0) {
+    const float b = gate_bias ? gate_bias[e] : 0.f;
+#pragma unroll
+    for (int t = 0; t < kGateTok; ++t)
+      if (t0 + t < T) z[(size_t)(t0 + t) * E + e] = acc[t] + b;
+  }
+}
+
+// ----------------------------------------------------------------------- a2: warp softmax top-k
+// One warp, one token.  Lane l holds logits of experts l, l+32, ...  k rounds of warp arg-max with the
+// order (z descending, id ascending); lane j ends up holding the j-th pick and its weight.
+__device__ __forceinline__ void warp_topk(const float* __restrict__ zrow, int E, int k, int renorm,
+                                          int lane, int& my_id, float& my_w) {
+  constexpr int NV = kMaxExperts / 32;
+  float v[NV];
+#pragma unroll
+  for (int i = 0; i < NV; ++i) {
+    const int e = lane + 32 * i;
+    v[i] = (e < E) ? zrow[e] : -INFINITY;
+  }
+  float zmax = v[0];
+#pragma unroll
+  for (int i = 1; i < NV; ++i) zmax = fmaxf(zmax, v[i]);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) zmax = fmaxf(zmax, __shfl_xor_sync(0xffffffffu, zmax, o));
+  float denom_all = 0.f;
+  if (!renorm) {
+#pragma unroll
+    for (int i = 0; i < NV; ++i)
+      if (lane + 32 * i < E) denom_all += expf(v[i] - zmax);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) denom_all += __shfl_xor_sync(0xffffffffu, denom_all, o);
+  }
+  float sel_val = -INFINITY;
+  int sel_id = 0;
+  for (int j = 0; j < k; ++j) {
+    float bv = -INFINITY;
+    int bi = 0x7fffffff;
+#pragma unroll
+    for (int i = 0; i < NV; ++i)
+      if (v[i] > bv) { bv = v[i]; bi = lane + 32 * i; }     // ascending id per lane: strict > keeps the lower id
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      const float ov = __shfl_xor_sync(0xffffffffu, bv, o);
+      const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+      if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+    }
+    if ((bi & 31) == lane) {
+#pragma unroll
+      for (int i = 0; i < NV; ++i)
+        if ((bi >> 5) == i) v[i] = -INFINITY;
+    }
+    if (lane == j) { sel_val = bv; sel_id = bi; }
+  }
+  sel_id = min(max(sel_id, 0), E - 1);          // NaN/Inf inputs are outside the contract; never index out of [0,E)
+  const float ev = (lane < k) ? expf(sel_val - zmax) : 0.f;
+  float denom = ev;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) denom += __shfl_xor_sync(0xffffffffu, denom, o);
+  my_id = sel_id;
+  my_w = renorm ? ev / denom : ev / denom_all;
+}
+
+// ------------------------------------------------------------------------ a3: signature increments
+// int32 request cell: atomic add.  int8 block cell: CUDA has no 8-bit atomics -> 32-bit atomic add of
+// 1 << 8*(byte in word) on the aligned word; no carry can cross because a cell never exceeds the KV
+// block size (<= 127; ids are distinct per token).  Integer adds commute => bit-exact in any order.
+__device__ __forceinline__ void sig_add(int32_t* sig_req, int8_t* sig_block, int req, int blk, int L,
+                                        int layer, int E, int e) {
+  if (sig_req != nullptr && req >= 0)
+    atomicAdd(sig_req + ((size_t)req * L + layer) * E + e, 1);
+  if (sig_block != nullptr && blk >= 0) {
+    const size_t idx = ((size_t)blk * L + layer) * E + e;
+    unsigned int* word = reinterpret_cast<unsigned int*>(sig_block + (idx & ~(size_t)3));
+    atomicAdd(word, 1u << (8u * (unsigned)(idx & 3)));
+  }
+}
+
+struct TopkArgs {
+  const float* z;            // [T,E]
+  int32_t* ids;              // [T,k]
+  float* w;                  // [T,k]
+  const int32_t* token_req;  // [T] or null
+  const int32_t* token_block;
+  int32_t* sig_req;
+  int8_t* sig_block;
+  int T, E, k, L, layer, renorm;
+};
+
+// Multi-CTA top-k (+signature) for eldr_moe_gate_topk: warp per token, any T.
+__global__ void __launch_bounds__(256) topk_kernel(TopkArgs a) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int t = blockIdx.x * 8 + warp;
+  if (t >= a.T) return;
+  int id; float w;
+  warp_topk(a.z + (size_t)t * a.E, a.E, a.k, a.renorm, lane, id, w);
+  if (lane < a.k) {
+    a.ids[(size_t)t * a.k + lane] = id;
+    a.w[(size_t)t * a.k + lane] = w;
+    sig_add(a.sig_req, a.sig_block, a.token_req ? a.token_req[t] : -1,
+            a.token_block ? a.token_block[t] : -1, a.L, a.layer, a.E, id);
+  }
+}
+
+// ------------------------------------------------- a2+a3+a4: top-k, signature, permutation, union
+struct RouteArgs {
+  TopkArgs tk;
+  int force_routing, n_shared;
+  int32_t* cnt;        // [E]
+  int32_t* off;        // [E+1]
+  int32_t* perm;       // [T*k]
+  int32_t* pair_pos;   // [T*k]
+  int4* work;          // [E+n_shared] {expert, x_row0, out_row0, m}
+  int32_t* n_work;     // [1]
+  int32_t* active;     // [E]
+  int32_t* n_active;   // [1]
+};
+
+// Single CTA (decode batches: T <= 1024).  Membership bitmask mask[e][t/32] makes the counting sort
+// deterministic and atomic-free in global memory: rank of pair (t,e) = popcount of expert e's bits below t.
+__global__ void __launch_bounds__(1024) topk_route_kernel(RouteArgs a) {
+  extern __shared__ __align__(16) uint8_t smem_raw[];
+  const int T = a.tk.T, E = a.tk.E, k = a.tk.k;
+  const int W = (T + 31) >> 5;
+  uint32_t* mask = reinterpret_cast<uint32_t*>(smem_raw);   // [E][W]
+  uint32_t* pref = mask + (size_t)E * W;                      // [E][W] exclusive prefix popcounts
+  int32_t* s_cnt = reinterpret_cast<int32_t*>(pref + (size_t)E * W);   // [E]
+  int32_t* s_off = s_cnt + E;                                 // [E+1]
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+
+  for (int i = tid; i < E * W; i += 1024) mask[i] = 0u;
+  __syncthreads();
+
+  for (int t = warp; t < T; t += 32) {
+    int id = 0; float w = 0.f;
+    if (!a.force_routing) {
+      warp_topk(a.tk.z + (size_t)t * E, E, k, a.tk.renorm, lane, id, w);
+      if (lane < k) {
+        a.tk.ids[(size_t)t * k + lane] = id;
+        a.tk.w[(size_t)t * k + lane] = w;
+      }
+    } else if (lane < k) {
+      id = min(max(a.tk.ids[(size_t)t * k + lane], 0), E - 1);
+    }
+    if (lane < k) {
+      atomicOr(&mask[id * W + (t >> 5)], 1u << (t & 31));
+      sig_add(a.tk.sig_req, a.tk.sig_block, a.tk.token_req ? a.tk.token_req[t] : -1,
+              a.tk.token_block ? a.tk.token_block[t] : -1, a.tk.L, a.tk.layer, E, id);
+    }
+  }
+  __syncthreads();
+
+  for (int e = tid; e < E; e += 1024) {
+    int run = 0;
+    for (int w = 0; w < W; ++w) {
+      pref[e * W + w] = run;
+      run += __popc(mask[e * W + w]);
+    }
+    s_cnt[e] = run;
+  }
+  __syncthreads();
+
+  if (warp == 0) {     // exclusive scan of cnt and ascending compaction of the active experts
+    constexpr int PER = kMaxExperts / 32;
+    int c[PER], csum = 0, asum = 0;
+#pragma unroll
+    for (int i = 0; i < PER; ++i) {
+      const int e = lane * PER + i;
+      c[i] = (e < E) ? s_cnt[e] : 0;
+      csum += c[i];
+      asum += (c[i] > 0);
+    }
+    int cinc = csum, ainc = asum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int cv = __shfl_up_sync(0xffffffffu, cinc, o);
+      const int av = __shfl_up_sync(0xffffffffu, ainc, o);
+      if (lane >= o) { cinc += cv; ainc += av; }
+    }
+    int coff = cinc - csum, aoff = ainc - asum;
+    const int n_act = __shfl_sync(0xffffffffu, ainc, 31);
+    const int total = __shfl_sync(0xffffffffu, cinc, 31);
+#pragma unroll
+    for (int i = 0; i < PER; ++i) {
+      const int e = lane * PER + i;
+      if (e < E) {
+        s_off[e] = coff;
+        a.off[e] = coff;
+        a.cnt[e] = c[i];
+        if (c[i] > 0) {
+          a.active[aoff] = e;
+          a.work[aoff] = make_int4(e, coff, coff, c[i]);
+          ++aoff;
+        }
+        coff += c[i];
+      }
+    }
+    for (int i = n_act + lane; i < E; i += 32) a.active[i] = -1;
+    if (lane == 0) {
+      s_off[E] = total;
+      a.off[E] = total;
+      *a.n_active = n_act;
+      *a.n_work = n_act + a.n_shared;
+    }
+    if (lane < a.n_shared) a.work[n_act + lane] = make_int4(E + lane, T * k, T * k + lane * T, T);
+  }
+  __syncthreads();
+
+  for (int p = tid; p < T * k; p += 1024) {
+    const int t = p / k;
+    const int e = min(max(a.tk.ids[p], 0), E - 1);
+    const int rank = pref[e * W + (t >> 5)] + __popc(mask[e * W + (t >> 5)] & ((1u << (t & 31)) - 1u));
+    const int pos = s_off[e] + rank;
+    a.perm[pos] = p;
+    a.pair_pos[p] = pos;
+  }
+}
+
+// x_perm[row] = x[token of sorted pair row]  (rows >= T*k: plain copy of x for the shared experts)
+__global__ void __launch_bounds__(256) gather_x_kernel(const uint16_t* __restrict__ x,
+                                                       const int32_t* __restrict__ perm,
+                                                       uint16_t* __restrict__ x_perm, int T, int H, int k,
+                                                       int n_rows) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int row = blockIdx.x * 8 + warp;
+  if (row >= n_rows) return;
+  const int t = (row < T * k) ? perm[row] / k : row - T * k;
+  const uint4* src = reinterpret_cast<const uint4*>(x + (size_t)t * H);
+  uint4* dst = reinterpret_cast<uint4*>(x_perm + (size_t)row * H);
+  for (int c = lane; c < (H >> 3); c += 32) dst[c] = __ldg(src + c);
+}
+
+// --------------------------------------------------------------------------- a7: weighted combine
+// out[t] = sum_j w[t,j]*y[pos(t,j)] (slot order) + sum_s y[shared s, t]; fp32, one RNE rounding to bf16.
+// Staged + ordered instead of fp32 atomics so that results are run-to-run bit-identical.
+__global__ void __launch_bounds__(256) combine_kernel(const float* __restrict__ y,
+                                                      const float* __restrict__ w,
+                                                      const int32_t* __restrict__ pair_pos,
+                                                      uint16_t* __restrict__ out, int T, int H, int k,
+                                                      int n_shared) {
+  const int q_per_row = H >> 2;
+  const int idx = blockIdx.x * 256 + threadIdx.x;
+  if (idx >= T * q_per_row) return;
+  const int t = idx / q_per_row, c4 = idx - t * q_per_row;
+  float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+  for (int j = 0; j < k; ++j) {
+    const int pos = pair_pos[t * k + j];
+    const float wt = w[t * k + j];
+    const float4 v = *reinterpret_cast<const float4*>(y + (size_t)pos * H + (size_t)c4 * 4);
+    acc.x = fmaf(wt, v.x, acc.x); acc.y = fmaf(wt, v.y, acc.y);
+    acc.z = fmaf(wt, v.z, acc.z); acc.w = fmaf(wt, v.w, acc.w);
+  }
+  for (int s = 0; s < n_shared; ++s) {
+    const float4 v = *reinterpret_cast<const float4*>(y + ((size_t)T * k + (size_t)s * T + t) * H + (size_t)c4 * 4);
+    acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
+  }
+  uint2 o;
+  o.x = (uint32_t)f32_to_bf16_rn(acc.x) | ((uint32_t)f32_to_bf16_rn(acc.y) << 16);
+  o.y = (uint32_t)f32_to_bf16_rn(acc.z) | ((uint32_t)f32_to_bf16_rn(acc.w) << 16);
+  *reinterpret_cast<uint2*>(out + (size_t)t * H + (size_t)c4 * 4) = o;
+}
+
+// ------------------------------------------------------------------- standalone signature kernels
+__global__ void __launch_bounds__(256) sig_accumulate_kernel(const int32_t* __restrict__ ids,
+                                                             const int32_t* __restrict__ token_req,
+                                                             const int32_t* __restrict__ token_block,
+                                                             int32_t* sig_req, int8_t* sig_block, int T, int E,
+                                                             int k, int L, int layer) {
+  const long long p = (long long)blockIdx.x * 256 + threadIdx.x;
+  if (p >= (long long)T * k) return;
+  const int t = (int)(p / k);
+  const int e = ids[p];
+  if (e < 0 || e >= E) return;
+  sig_add(sig_req, sig_block, token_req ? token_req[t] : -1, token_block ? token_block[t] : -1, L, layer, E, e);
+}
+
+__global__ void __launch_bounds__(256) sig_reset_kernel(const int32_t* __restrict__ block_ids, int8_t* sig_block,
+                                                        int row_bytes) {
+  const int b = block_ids[blockIdx.x];
+  if (b < 0) return;
+  if ((row_bytes & 3) == 0) {
+    uint32_t* row = reinterpret_cast<uint32_t*>(sig_block + (size_t)b * row_bytes);
+    for (int i = threadIdx.x; i < (row_bytes >> 2); i += 256) row[i] = 0u;
+  } else {
+    for (int i = threadIdx.x; i < row_bytes; i += 256) sig_block[(size_t)b * row_bytes + i] = 0;
+  }
+}
+
+__global__ void __launch_bounds__(256) sig_readout_kernel(const int32_t* __restrict__ block_ids,
+                                                          const int32_t* __restrict__ req_off,
+                                                          const int8_t* __restrict__ sig_block,
+                                                          int32_t* __restrict__ sig_out, int row_cells) {
+  const int r = blockIdx.y;
+  const int b0 = req_off[r], b1 = req_off[r + 1];
+  for (int c = blockIdx.x * 256 + threadIdx.x; c < row_cells; c += gridDim.x * 256) {
+    int acc = 0;
+    for (int i = b0; i < b1; ++i) {
+      const int b = block_ids[i];
+      if (b >= 0) acc += (int)sig_block[(size_t)b * row_cells + c];
+    }
+    sig_out[(size_t)r * row_cells + c] = acc;
+  }
+}
+
+}  // namespace eldr

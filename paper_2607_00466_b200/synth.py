@@ -89,12 +89,18 @@ class LayerWeights:
     shared_w2: Optional[np.ndarray]    # [n_shared,H,I] bf16 bits or None
 
 
+def make_gate_w(shape: "MoEShape", seed: int, layer: int = 0, gate_std: float = 0.05) -> np.ndarray:
+    """fp32 gate rows ~N(0,0.05), [E,H]."""
+    g = np.random.default_rng(sub_seed(seed, "gate_w", layer))
+    return (g.standard_normal((shape.n_experts, shape.hidden), dtype=np.float32)
+            * np.float32(gate_std)).astype(np.float32)
+
+
 def make_layer_weights(shape: MoEShape, seed: int, layer: int = 0,
                        w_std: float = 0.02, gate_std: float = 0.05) -> LayerWeights:
     """bf16 expert weights ~N(0,0.02), fp32 gate ~N(0,0.05) (BASELINE.json configs 1-2)."""
     H, I, E = shape.hidden, shape.inter, shape.n_experts
-    g = np.random.default_rng(sub_seed(seed, "gate_w", layer))
-    gate_w = (g.standard_normal((E, H), dtype=np.float32) * np.float32(gate_std)).astype(np.float32)
+    gate_w = make_gate_w(shape, seed, layer, gate_std)
     w13 = _normal_bf16(np.random.default_rng(sub_seed(seed, "w13", layer)), (E, 2 * I, H), w_std)
     w2 = _normal_bf16(np.random.default_rng(sub_seed(seed, "w2", layer)), (E, H, I), w_std)
     s13 = s2 = None
@@ -269,3 +275,27 @@ def hand_example(pad_h: int = 2, pad_i: int = 1):
     token_req = np.array([0, 1], np.int32)
     token_block = np.array([0, 1], np.int32)
     return shape, lw, f32_to_bf16_bits(x), token_req, token_block
+
+
+# ----------------------------------------------------------------------------------------------
+# Config 2/3 cases: (T, u) -> hiddens + gate bias.  The realised union can fall short of u by chance,
+# so seeds are rejection-sampled ONCE by oracle/find_union_seeds.py (which calls only the oracle) and
+# stored in union_seeds.json beside this file; this module only looks the accepted seed up.
+# ----------------------------------------------------------------------------------------------
+WEIGHT_SEED = 0
+
+
+def union_case(shape: MoEShape, T: int, u: int, try_seed: int):
+    """x [T,H] bf16 bits and gate_bias [E] for one (T,u) case at one try seed."""
+    x = make_hidden(T, shape.hidden, try_seed, tag="xu%d" % u)
+    bias = union_bias(shape.n_experts, u, try_seed)
+    return x, bias
+
+
+def accepted_union_seed(T: int, u: int) -> int:
+    import json
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "union_seeds.json")
+    with open(path) as f:
+        table = json.load(f)
+    return int(table["T%d_u%d" % (T, u)]["seed"])

