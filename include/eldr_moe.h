@@ -152,6 +152,13 @@ size_t  eldr_moe_workspace_bytes(const eldr_moe_shape_t* shape, int32_t max_T);
 size_t  eldr_moe_workspace_bytes_host(const eldr_moe_shape_t* shape, int32_t max_T);
 int32_t eldr_moe_workspace_layout(const eldr_moe_shape_t* shape, int32_t T, eldr_moe_ws_layout_t* layout);
 
+/* Process-wide tuning knobs (defaults are the fast settings; used by tests and profiles to compare paths).
+ *   ELDR_OPT_FFN_PATH: ELDR_FFN_TCGEN05 (default; tcgen05.mma + TMEM) or ELDR_FFN_MMA_SYNC (legacy mma.sync). */
+#define ELDR_OPT_FFN_PATH 0
+#define ELDR_FFN_MMA_SYNC 0
+#define ELDR_FFN_TCGEN05  1
+int32_t eldr_moe_set_option(int32_t key, int32_t value);
+
 /* Per-kernel device timing of eldr_moe_decode_layer (measurement aid, off by default, per host thread).
  * When enabled, the call records a CUDA event on `stream` before each of its kernels and after the last.
  * eldr_moe_profile_read waits for the last call's events and writes the ELDR_PROFILE_SLOTS durations in

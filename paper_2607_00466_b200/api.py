@@ -22,8 +22,9 @@ EXPORTS = [
     "eldr_signature_accumulate", "eldr_signature_reset_blocks", "eldr_signature_readout",
     "eldr_moe_workspace_bytes", "eldr_moe_workspace_bytes_host", "eldr_moe_workspace_layout",
     "eldr_moe_last_launch_count", "eldr_status_string", "eldr_last_cuda_error",
-    "eldr_moe_profile_enable", "eldr_moe_profile_read",
+    "eldr_moe_profile_enable", "eldr_moe_profile_read", "eldr_moe_set_option",
 ]
+OPT_FFN_PATH, FFN_MMA_SYNC, FFN_TCGEN05 = 0, 0, 1
 PROFILE_SLOTS = ("gate", "route", "gather", "ffn13", "ffn2", "combine")
 
 
@@ -121,6 +122,10 @@ def eldr_moe_workspace_layout(shape, T: int) -> WsLayout:
 
 def eldr_moe_last_launch_count() -> int:
     return int(load().eldr_moe_last_launch_count())
+
+
+def eldr_moe_set_option(key: int, value: int) -> None:
+    _check(load().eldr_moe_set_option(C.c_int32(key), C.c_int32(value)), "eldr_moe_set_option")
 
 
 def eldr_moe_profile_enable(on: bool) -> None:

@@ -10,11 +10,14 @@
 
 #include "eldr_moe.h"
 #include "ffn_stream.cuh"
+#include "ffn_umma.cuh"
 #include "gate_route.cuh"
 
 namespace {
 
 using namespace eldr;
+
+int g_ffn_path = ELDR_FFN_TCGEN05;   // process-wide tuning knob (eldr_moe_set_option)
 
 thread_local char g_err[256] = "";
 thread_local int g_launches = 0;
@@ -128,21 +131,35 @@ encode_tiled_fn get_encode_fn() {
 // bf16 [rows, cols] row-major, box = box_rows x 64 columns (128 bytes), SWIZZLE_128B, OOB reads give zeros.
 // Descriptors are pure functions of (ptr, rows, cols, box_rows); a small cache avoids re-encoding the
 // static weight descriptors every step.
-struct TmapKey { const void* p; uint64_t rows, cols; uint32_t box_rows; };
+struct TmapKey { const void* p; uint64_t rows, cols; uint32_t box_rows, kind; };
 struct TmapSlot { TmapKey k; CUtensorMap m; bool used; };
 std::mutex g_tm_mu;
 TmapSlot g_tm_cache[64];
 int g_tm_next = 0;
 
+bool tmap_lookup(const TmapKey& k, CUtensorMap* out) {
+  std::lock_guard<std::mutex> lk(g_tm_mu);
+  for (auto& s : g_tm_cache)
+    if (s.used && s.k.p == k.p && s.k.rows == k.rows && s.k.cols == k.cols && s.k.box_rows == k.box_rows &&
+        s.k.kind == k.kind) {
+      *out = s.m;
+      return true;
+    }
+  return false;
+}
+void tmap_store(const TmapKey& k, const CUtensorMap& m) {
+  std::lock_guard<std::mutex> lk(g_tm_mu);
+  TmapSlot& s = g_tm_cache[g_tm_next];
+  g_tm_next = (g_tm_next + 1) % 64;
+  s.k = k;
+  s.m = m;
+  s.used = true;
+}
+
+// bf16 [rows, cols] row-major, box = box_rows x 64 columns (128 bytes), SWIZZLE_128B, OOB reads give zeros.
 bool make_tmap(CUtensorMap* out, const void* ptr, uint64_t rows, uint64_t cols, uint32_t box_rows) {
-  {
-    std::lock_guard<std::mutex> lk(g_tm_mu);
-    for (auto& s : g_tm_cache)
-      if (s.used && s.k.p == ptr && s.k.rows == rows && s.k.cols == cols && s.k.box_rows == box_rows) {
-        *out = s.m;
-        return true;
-      }
-  }
+  const TmapKey key{ptr, rows, cols, box_rows, 2};
+  if (tmap_lookup(key, out)) return true;
   encode_tiled_fn fn = get_encode_fn();
   if (!fn) { snprintf(g_err, sizeof(g_err), "cuTensorMapEncodeTiled entry point not found"); return false; }
   cuuint64_t gdim[2] = {cols, rows};
@@ -153,12 +170,26 @@ bool make_tmap(CUtensorMap* out, const void* ptr, uint64_t rows, uint64_t cols, 
                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) { snprintf(g_err, sizeof(g_err), "cuTensorMapEncodeTiled failed: %d", (int)r); return false; }
-  std::lock_guard<std::mutex> lk(g_tm_mu);
-  TmapSlot& s = g_tm_cache[g_tm_next];
-  g_tm_next = (g_tm_next + 1) % 64;
-  s.k = TmapKey{ptr, rows, cols, box_rows};
-  s.m = *out;
-  s.used = true;
+  tmap_store(key, *out);
+  return true;
+}
+
+// w13 [n_exp, 2I, H] viewed as 5-D (col, row-in-16, branch{w1,w3}, 16-row group, expert) so that ONE box of
+// (64 cols, 16 rows, 2 branches, 4 groups) lands in shared memory as 4 x [16 rows of w1 | same 16 rows of w3].
+bool make_tmap_w13_5d(CUtensorMap* out, const void* ptr, uint64_t n_exp, uint64_t I, uint64_t H) {
+  const TmapKey key{ptr, n_exp * 2 * I, H, 16, 5};
+  if (tmap_lookup(key, out)) return true;
+  encode_tiled_fn fn = get_encode_fn();
+  if (!fn) { snprintf(g_err, sizeof(g_err), "cuTensorMapEncodeTiled entry point not found"); return false; }
+  cuuint64_t gdim[5] = {H, 16, 2, I / 16, n_exp};
+  cuuint64_t gstride[4] = {H * 2, I * H * 2, 16 * H * 2, 2 * I * H * 2};
+  cuuint32_t box[5] = {64, 16, 2, 4, 1};
+  cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+  CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 5, const_cast<void*>(ptr), gdim, gstride, box, estr,
+                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) { snprintf(g_err, sizeof(g_err), "cuTensorMapEncodeTiled(5d) failed: %d", (int)r); return false; }
+  tmap_store(key, *out);
   return true;
 }
 
@@ -194,6 +225,14 @@ const char* eldr_status_string(int32_t st) {
 }
 
 const char* eldr_last_cuda_error(void) { return g_err; }
+
+int32_t eldr_moe_set_option(int32_t key, int32_t value) {
+  if (key == ELDR_OPT_FFN_PATH && (value == ELDR_FFN_MMA_SYNC || value == ELDR_FFN_TCGEN05)) {
+    g_ffn_path = value;
+    return ELDR_OK;
+  }
+  return ELDR_ERR_INVALID_ARG;
+}
 
 int32_t eldr_moe_profile_enable(int32_t on) {
   g_prof_on = on != 0;
@@ -335,7 +374,44 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
   const int max_work = (E < T * k ? E : T * k) + ns;
   FfnArgs f13{work, n_work, E, H, 2 * I, I, H, I / 64, hbuf, nullptr};
   FfnArgs f2{work, n_work, E, I, H, I, H, (H + 127) / 128, nullptr, ybuf};
-  if (H % 64 == 0 && I % 64 == 0) {
+  const int sms = num_sms();
+  int g13 = max_work * f13.tiles_per_expert; if (g13 > sms) g13 = sms;
+  int g2 = max_work * f2.tiles_per_expert; if (g2 > sms) g2 = sms;
+  if (H % 64 == 0 && I % 64 == 0 && g_ffn_path == ELDR_FFN_TCGEN05) {
+    // tcgen05 + TMEM path: weights are the M=128 operand, the expert's tokens the N operand
+    CUtensorMap tm_w13, tm_sw13, tm_x16, tm_x64, tm_w2, tm_sw2, tm_h16, tm_h64;
+    if (!make_tmap_w13_5d(&tm_w13, w13, E, I, H)) return ELDR_ERR_CUDA;
+    if (!make_tmap(&tm_w2, w2, (uint64_t)E * H, I, 128)) return ELDR_ERR_CUDA;
+    if (ns) {
+      if (!make_tmap_w13_5d(&tm_sw13, shared_w13, ns, I, H)) return ELDR_ERR_CUDA;
+      if (!make_tmap(&tm_sw2, shared_w2, (uint64_t)ns * H, I, 128)) return ELDR_ERR_CUDA;
+    } else {
+      tm_sw13 = tm_w13;
+      tm_sw2 = tm_w2;
+    }
+    if (!make_tmap(&tm_x16, x_perm, (uint64_t)x_rows, H, 16)) return ELDR_ERR_CUDA;
+    if (!make_tmap(&tm_x64, x_perm, (uint64_t)x_rows, H, 64)) return ELDR_ERR_CUDA;
+    if (!make_tmap(&tm_h16, hbuf, (uint64_t)out_rows, I, 16)) return ELDR_ERR_CUDA;
+    if (!make_tmap(&tm_h64, hbuf, (uint64_t)out_rows, I, 64)) return ELDR_ERR_CUDA;
+    UmmaCfg cfg;
+    cfg.np = T <= 64 ? 64 : 128;      // an expert receives at most T tokens
+    cfg.stages = T <= 64 ? 8 : 6;
+    const size_t smem = (size_t)cfg.stages * (kUmmaWBytes + cfg.np * 128) + 1024 + 256;
+    static bool umma_attr_set = false;
+    if (!umma_attr_set) {
+      const size_t mx = 8 * (kUmmaWBytes + 64 * 128) + 1024 + 256;
+      if (!set_smem(ffn_umma_kernel<0>, mx) || !set_smem(ffn_umma_kernel<1>, mx)) return ELDR_ERR_CUDA;
+      umma_attr_set = true;
+    }
+    f13.tiles_per_expert = I / 64;
+    prof_mark(3, st);
+    ffn_umma_kernel<0><<<g13, kUmmaThreads, smem, st>>>(tm_w13, tm_sw13, tm_x16, tm_x64, f13, cfg);
+    if (!launch_ok("ffn_umma_kernel<w13>")) return ELDR_ERR_CUDA;
+    prof_mark(4, st);
+    ffn_umma_kernel<1><<<g2, kUmmaThreads, smem, st>>>(tm_w2, tm_sw2, tm_h16, tm_h64, f2, cfg);
+    if (!launch_ok("ffn_umma_kernel<w2>")) return ELDR_ERR_CUDA;
+  } else if (H % 64 == 0 && I % 64 == 0) {
+    // legacy tensor-core path (mma.sync), kept selectable for comparison
     CUtensorMap tm_w13, tm_sw13, tm_x, tm_w2, tm_sw2, tm_h;
     if (!make_tmap(&tm_w13, w13, (uint64_t)E * 2 * I, H, 64)) return ELDR_ERR_CUDA;
     if (!make_tmap(&tm_w2, w2, (uint64_t)E * H, I, 128)) return ELDR_ERR_CUDA;
@@ -354,9 +430,6 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
         return ELDR_ERR_CUDA;
       attr_set = true;
     }
-    const int sms = num_sms();
-    int g13 = max_work * f13.tiles_per_expert; if (g13 > sms) g13 = sms;
-    int g2 = max_work * f2.tiles_per_expert; if (g2 > sms) g2 = sms;
     prof_mark(3, st);
     ffn_stream_kernel<0><<<g13, kFfnThreads, kFfnSmemBytes, st>>>(tm_w13, tm_sw13, tm_x, f13);
     if (!launch_ok("ffn_stream_kernel<w13>")) return ELDR_ERR_CUDA;
