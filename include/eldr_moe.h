@@ -74,6 +74,7 @@ typedef struct {
   size_t pair_pos;   /* int32   [T*k]            inverse of perm                                         */
   size_t work;       /* int32x4 [E+n_shared]     {expert, x_row0, out_row0, m} per streamed expert       */
   size_t n_work;     /* int32   [1]              n_active + n_shared                                     */
+  size_t sync;       /* uint32  [...]            epoch flags of the fused gate/top-k/route kernel (internal)  */
   size_t x_perm;     /* bf16    [T*k + T, H]     x gathered in sorted order, then a plain copy of x      */
   size_t h;          /* bf16    [T*(k+ns), I]    silu(W1 x)*(W3 x) per sorted pair, then shared experts  */
   size_t y;          /* float   [T*(k+ns), H]    W2 h per sorted pair, then shared experts               */
@@ -155,6 +156,7 @@ int32_t eldr_moe_workspace_layout(const eldr_moe_shape_t* shape, int32_t T, eldr
 /* Process-wide tuning knobs (defaults are the fast settings; used by tests and profiles to compare paths).
  *   ELDR_OPT_FFN_PATH: ELDR_FFN_TCGEN05 (default; tcgen05.mma + TMEM) or ELDR_FFN_MMA_SYNC (legacy mma.sync). */
 #define ELDR_OPT_FFN_PATH 0
+#define ELDR_OPT_PDL      1   /* 1 (default): programmatic dependent launch between the step's kernels; 0: plain */
 #define ELDR_FFN_MMA_SYNC 0
 #define ELDR_FFN_TCGEN05  1
 int32_t eldr_moe_set_option(int32_t key, int32_t value);
@@ -162,7 +164,7 @@ int32_t eldr_moe_set_option(int32_t key, int32_t value);
 /* Per-kernel device timing of eldr_moe_decode_layer (measurement aid, off by default, per host thread).
  * When enabled, the call records a CUDA event on `stream` before each of its kernels and after the last.
  * eldr_moe_profile_read waits for the last call's events and writes the ELDR_PROFILE_SLOTS durations in
- * milliseconds to HOST memory: [0] gate GEMV, [1] top-k/signature/permutation, [2] gather,
+ * milliseconds to HOST memory: [0] gate GEMV + top-k/signature + permutation (one launch), [1] permutation alone (force_routing), [2] gather,
  * [3] FFN w1/w3, [4] FFN w2, [5] combine (0 for a kernel that did not run). */
 #define ELDR_PROFILE_SLOTS 6
 int32_t eldr_moe_profile_enable(int32_t on);

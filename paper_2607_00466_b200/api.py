@@ -25,6 +25,7 @@ EXPORTS = [
     "eldr_moe_profile_enable", "eldr_moe_profile_read", "eldr_moe_set_option",
 ]
 OPT_FFN_PATH, FFN_MMA_SYNC, FFN_TCGEN05 = 0, 0, 1
+OPT_PDL = 1
 PROFILE_SLOTS = ("gate", "route", "gather", "ffn13", "ffn2", "combine")
 
 
@@ -36,7 +37,7 @@ class Shape(C.Structure):
 
 class WsLayout(C.Structure):
     """eldr_moe_ws_layout_t"""
-    _fields_ = [(n, C.c_size_t) for n in ("z", "cnt", "off", "perm", "pair_pos", "work", "n_work",
+    _fields_ = [(n, C.c_size_t) for n in ("z", "cnt", "off", "perm", "pair_pos", "work", "n_work", "sync",
                                           "x_perm", "h", "y", "total")]
 
 

@@ -95,6 +95,12 @@ __device__ __forceinline__ void mma_bf16_16816(float (&d)[4], uint32_t a0, uint3
       : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
 }
 
+// Programmatic dependent launch: no-ops unless the kernel was launched with the PDL attribute.
+// pdl_wait() returns once the preceding kernel in the stream has completed and its writes are visible;
+// every CTA calls it before touching dependent data (and before exiting, so completion stays transitive).
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 __device__ __forceinline__ float silu_f(float v) { return v / (1.0f + expf(-v)); }
 
 }  // namespace eldr

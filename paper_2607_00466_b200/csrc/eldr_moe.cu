@@ -6,6 +6,7 @@
 
 #include <cstdio>
 #include <cstring>
+#include <atomic>
 #include <mutex>
 
 #include "eldr_moe.h"
@@ -17,7 +18,8 @@ namespace {
 
 using namespace eldr;
 
-int g_ffn_path = ELDR_FFN_TCGEN05;   // process-wide tuning knob (eldr_moe_set_option)
+int g_ffn_path = ELDR_FFN_TCGEN05;   // process-wide tuning knobs (eldr_moe_set_option)
+int g_pdl = 1;
 
 thread_local char g_err[256] = "";
 thread_local int g_launches = 0;
@@ -81,6 +83,7 @@ void make_layout(const eldr_moe_shape_t* s, int T, eldr_moe_ws_layout_t* L) {
   L->pair_pos = take(Tz * k * 4);
   L->work = take((E + ns) * 16);
   L->n_work = take(4);
+  L->sync = take(((size_t)((Tz + kGateTok - 1) / kGateTok) * (((size_t)E + kGateExp - 1) / kGateExp + 2) + 1) * 4);
   L->x_perm = take((Tz * k + Tz) * H * 2);
   L->h = take(Tz * (k + ns) * I * 2);
   L->y = take(Tz * (k + ns) * H * 4);
@@ -193,6 +196,24 @@ bool make_tmap_w13_5d(CUtensorMap* out, const void* ptr, uint64_t n_exp, uint64_
   return true;
 }
 
+// Launch with the programmatic-dependent-launch attribute: the kernel may start (prologue: barrier init, TMEM
+// allocation, descriptor prefetch) while its predecessor drains; it calls griddepcontrol.wait before touching
+// the predecessor's outputs.  Profiling events between kernels disable the overlap by construction.
+template <typename... KArgs, typename... Args>
+cudaError_t launch_dep(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = (g_pdl && !g_prof_on) ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 template <typename K>
 bool set_smem(K kernel, size_t bytes) {
   return cuda_ok(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes),
@@ -213,6 +234,13 @@ int32_t launch_gate_logits(const eldr_moe_shape_t* s, int T, const eldr_bf16* x,
 
 extern "C" {
 
+#ifdef ELDR_TRACE
+void eldr_debug_read_trace(unsigned long long* h) {
+  cudaDeviceSynchronize();
+  cudaMemcpyFromSymbol(h, eldr::g_trace, sizeof(unsigned long long) * 4096 * 16);
+}
+#endif
+
 const char* eldr_status_string(int32_t st) {
   switch (st) {
     case ELDR_OK: return "ok";
@@ -229,6 +257,10 @@ const char* eldr_last_cuda_error(void) { return g_err; }
 int32_t eldr_moe_set_option(int32_t key, int32_t value) {
   if (key == ELDR_OPT_FFN_PATH && (value == ELDR_FFN_MMA_SYNC || value == ELDR_FFN_TCGEN05)) {
     g_ffn_path = value;
+    return ELDR_OK;
+  }
+  if (key == ELDR_OPT_PDL && (value == 0 || value == 1)) {
+    g_pdl = value;
     return ELDR_OK;
   }
   return ELDR_ERR_INVALID_ARG;
@@ -335,39 +367,49 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
   float* ybuf = reinterpret_cast<float*>(ws + L.y);
 
   prof_begin();
-  // a1: gate logits
+  RouteArgs ra;
+  ra.tk = TopkArgs{z, topk_ids, topk_w, token_req, token_block, sig_req, sig_block,
+                   T, E, k, s->n_layers, layer, s->renormalize};
+  ra.force_routing = force_routing ? 1 : 0;
+  ra.n_shared = ns;
+  ra.H = H;
+  ra.cnt = reinterpret_cast<int32_t*>(ws + L.cnt);
+  ra.off = reinterpret_cast<int32_t*>(ws + L.off);
+  ra.perm = perm;
+  ra.pair_pos = pair_pos;
+  ra.work = work;
+  ra.n_work = n_work;
+  ra.active = active_experts;
+  ra.n_active = n_active;
+  const int W = (T + 31) / 32;
+  const size_t route_smem = (size_t)E * W * 8 + (size_t)(2 * E + 1) * 4;
   if (!force_routing) {
+    // a1-a4 in one launch: gate GEMV tiles; last CTA of a token group runs its top-k (+signature);
+    // last group runs the permutation / union compaction
+    static std::atomic<uint32_t> g_epoch{0x5eed0000u};
+    GateRouteArgs ga;
+    ga.x = x; ga.gate_w = gate_w; ga.gate_bias = gate_bias; ga.r = ra;
+    ga.sync = reinterpret_cast<uint32_t*>(ws + L.sync);
+    ga.epoch = ++g_epoch;
+    size_t smem = (size_t)kGateTok * H * 2;
+    if (route_smem > smem) smem = route_smem;
+    if (smem > 200 * 1024) return ELDR_ERR_UNSUPPORTED;
+    if (smem > 48 * 1024 && !set_smem(gate_topk_route_kernel, smem)) return ELDR_ERR_CUDA;
+    dim3 grid((E + kGateExp - 1) / kGateExp, (T + kGateTok - 1) / kGateTok);
     prof_mark(0, st);
-    rc = launch_gate_logits(s, T, x, gate_w, gate_bias, z, st);
-    if (rc != ELDR_OK) return rc;
-  }
-  // a2-a4: top-k (+signature), permutation, union compaction -- one CTA
-  {
-    RouteArgs ra;
-    ra.tk = TopkArgs{z, topk_ids, topk_w, token_req, token_block, sig_req, sig_block,
-                     T, E, k, s->n_layers, layer, s->renormalize};
-    ra.force_routing = force_routing ? 1 : 0;
-    ra.n_shared = ns;
-    ra.cnt = reinterpret_cast<int32_t*>(ws + L.cnt);
-    ra.off = reinterpret_cast<int32_t*>(ws + L.off);
-    ra.perm = perm;
-    ra.pair_pos = pair_pos;
-    ra.work = work;
-    ra.n_work = n_work;
-    ra.active = active_experts;
-    ra.n_active = n_active;
-    const int W = (T + 31) / 32;
-    const size_t smem = (size_t)E * W * 8 + (size_t)(2 * E + 1) * 4;
-    if (smem > 48 * 1024 && !set_smem(topk_route_kernel, smem)) return ELDR_ERR_CUDA;
+    gate_topk_route_kernel<<<grid, 256, smem, st>>>(ga);
+    if (!launch_ok("gate_topk_route_kernel")) return ELDR_ERR_CUDA;
+  } else {
+    if (route_smem > 48 * 1024 && !set_smem(route_only_kernel, route_smem)) return ELDR_ERR_CUDA;
     prof_mark(1, st);
-    topk_route_kernel<<<1, 1024, smem, st>>>(ra);
-    if (!launch_ok("topk_route_kernel")) return ELDR_ERR_CUDA;
+    route_only_kernel<<<1, 1024, route_smem, st>>>(ra);
+    if (!launch_ok("route_only_kernel")) return ELDR_ERR_CUDA;
   }
   // gather token rows in expert-sorted order (+ plain copy for the shared experts)
   const int x_rows = T * k + (ns ? T : 0);
   const int out_rows = T * (k + ns);
   prof_mark(2, st);
-  gather_x_kernel<<<(x_rows + 7) / 8, 256, 0, st>>>(x, perm, x_perm, T, H, k, x_rows);
+  launch_dep(gather_x_kernel, dim3((x_rows + 7) / 8), dim3(256), 0, st, x, perm, x_perm, T, H, k, x_rows);
   if (!launch_ok("gather_x_kernel")) return ELDR_ERR_CUDA;
 
   // a5/a6: grouped SwiGLU FFN over the active experts
@@ -405,10 +447,10 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
     }
     f13.tiles_per_expert = I / 64;
     prof_mark(3, st);
-    ffn_umma_kernel<0><<<g13, kUmmaThreads, smem, st>>>(tm_w13, tm_sw13, tm_x16, tm_x64, f13, cfg);
+    launch_dep(ffn_umma_kernel<0>, dim3(g13), dim3(kUmmaThreads), smem, st, tm_w13, tm_sw13, tm_x16, tm_x64, f13, cfg);
     if (!launch_ok("ffn_umma_kernel<w13>")) return ELDR_ERR_CUDA;
     prof_mark(4, st);
-    ffn_umma_kernel<1><<<g2, kUmmaThreads, smem, st>>>(tm_w2, tm_sw2, tm_h16, tm_h64, f2, cfg);
+    launch_dep(ffn_umma_kernel<1>, dim3(g2), dim3(kUmmaThreads), smem, st, tm_w2, tm_sw2, tm_h16, tm_h64, f2, cfg);
     if (!launch_ok("ffn_umma_kernel<w2>")) return ELDR_ERR_CUDA;
   } else if (H % 64 == 0 && I % 64 == 0) {
     // legacy tensor-core path (mma.sync), kept selectable for comparison
@@ -431,23 +473,23 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
       attr_set = true;
     }
     prof_mark(3, st);
-    ffn_stream_kernel<0><<<g13, kFfnThreads, kFfnSmemBytes, st>>>(tm_w13, tm_sw13, tm_x, f13);
+    launch_dep(ffn_stream_kernel<0>, dim3(g13), dim3(kFfnThreads), kFfnSmemBytes, st, tm_w13, tm_sw13, tm_x, f13);
     if (!launch_ok("ffn_stream_kernel<w13>")) return ELDR_ERR_CUDA;
     prof_mark(4, st);
-    ffn_stream_kernel<1><<<g2, kFfnThreads, kFfnSmemBytes, st>>>(tm_w2, tm_sw2, tm_h, f2);
+    launch_dep(ffn_stream_kernel<1>, dim3(g2), dim3(kFfnThreads), kFfnSmemBytes, st, tm_w2, tm_sw2, tm_h, f2);
     if (!launch_ok("ffn_stream_kernel<w2>")) return ELDR_ERR_CUDA;
   } else {
     dim3 g13(max_work, (I + 127) / 128), g2(max_work, (H + 127) / 128);
     prof_mark(3, st);
-    ffn13_plain_kernel<<<g13, 128, 0, st>>>(w13, shared_w13, x_perm, f13);
+    launch_dep(ffn13_plain_kernel, g13, dim3(128), 0, st, w13, shared_w13, x_perm, f13);
     if (!launch_ok("ffn13_plain_kernel")) return ELDR_ERR_CUDA;
     prof_mark(4, st);
-    ffn2_plain_kernel<<<g2, 128, 0, st>>>(w2, shared_w2, hbuf, f2);
+    launch_dep(ffn2_plain_kernel, g2, dim3(128), 0, st, w2, shared_w2, hbuf, f2);
     if (!launch_ok("ffn2_plain_kernel")) return ELDR_ERR_CUDA;
   }
   // a7: weighted combine
   prof_mark(5, st);
-  combine_kernel<<<(T * (H / 4) + 255) / 256, 256, 0, st>>>(ybuf, topk_w, pair_pos, out, T, H, k, ns);
+  launch_dep(combine_kernel, dim3((T * (H / 4) + 255) / 256), dim3(256), 0, st, ybuf, topk_w, pair_pos, out, T, H, k, ns);
   if (!launch_ok("combine_kernel")) return ELDR_ERR_CUDA;
   prof_mark(ELDR_PROFILE_SLOTS, st);
   return ELDR_OK;

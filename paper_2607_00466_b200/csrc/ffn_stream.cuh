@@ -62,6 +62,8 @@ ffn_stream_kernel(const __grid_constant__ CUtensorMap tm_w, const __grid_constan
     mbar_fence_init();
   }
   __syncthreads();
+  pdl_launch_dependents();
+  pdl_wait();
 
   const int n_work = *a.n_work;
   const int total_tiles = n_work * a.tiles_per_expert;
@@ -186,6 +188,8 @@ ffn_stream_kernel(const __grid_constant__ CUtensorMap tm_w, const __grid_constan
 __global__ void __launch_bounds__(128) ffn13_plain_kernel(const uint16_t* __restrict__ w13,
                                                           const uint16_t* __restrict__ shared_w13,
                                                           const uint16_t* __restrict__ x_perm, FfnArgs a) {
+  pdl_launch_dependents();
+  pdl_wait();
   if ((int)blockIdx.x >= *a.n_work) return;
   const int4 wk = a.work[blockIdx.x];
   const bool shared = wk.x >= a.E;
@@ -209,6 +213,8 @@ __global__ void __launch_bounds__(128) ffn13_plain_kernel(const uint16_t* __rest
 __global__ void __launch_bounds__(128) ffn2_plain_kernel(const uint16_t* __restrict__ w2,
                                                          const uint16_t* __restrict__ shared_w2,
                                                          const uint16_t* __restrict__ h, FfnArgs a) {
+  pdl_launch_dependents();
+  pdl_wait();
   if ((int)blockIdx.x >= *a.n_work) return;
   const int4 wk = a.work[blockIdx.x];
   const bool shared = wk.x >= a.E;

@@ -104,6 +104,9 @@ ffn_umma_kernel(const __grid_constant__ CUtensorMap tm_w, const __grid_constant_
   tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+  // everything above overlapped the previous kernel's tail; the work list / activations are its outputs
+  pdl_launch_dependents();
+  pdl_wait();
 
   const int n_work = *a.n_work;
   const int total_tiles = n_work * a.tiles_per_expert;

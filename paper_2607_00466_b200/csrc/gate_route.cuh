@@ -5,6 +5,21 @@
 
 namespace eldr {
 
+// Optional intra-kernel timeline (debug builds only: -DELDR_TRACE): thread 0 of every CTA stamps %globaltimer.
+#ifdef ELDR_TRACE
+__device__ unsigned long long g_trace[4096 * 16];
+#define ELDR_STAMP(id)                                                                        \
+  do {                                                                                        \
+    if (threadIdx.x == 0) {                                                                   \
+      unsigned long long t_;                                                                  \
+      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_));                                  \
+      g_trace[((blockIdx.y * gridDim.x + blockIdx.x) & 4095) * 16 + (id)] = t_;               \
+    }                                                                                         \
+  } while (0)
+#else
+#define ELDR_STAMP(id) do {} while (0)
+#endif
+
 constexpr int kMaxExperts = 256;   // 8 logits per lane in the warp top-k
 constexpr int kMaxTopK = 16;
 constexpr int kGateTok = 8;        // tokens per CTA in the gate GEMV
@@ -13,11 +28,9 @@ constexpr int kGateExp = 8;        // experts per CTA (= warps)
 // ------------------------------------------------------------------------------------ a1: gate GEMV
 // z[t,e] = sum_h x[t,h]*Wg[e,h] + bias[e], fp32 FMA on CUDA cores (no TF32/bf16 MMA: near-ties must not
 // flip).  CTA = 8 warps: warp w owns expert blockIdx.x*8+w against an 8-token x tile held in smem as bf16.
-__global__ void __launch_bounds__(256) gate_logits_kernel(const uint16_t* __restrict__ x,
-                                                          const float* __restrict__ gate_w,
-                                                          const float* __restrict__ gate_bias,
-                                                          float* __restrict__ z, int T, int H, int E) {
-  extern __shared__ __align__(16) uint8_t smem_raw[];
+__device__ __forceinline__ void gate_tile(const uint16_t* __restrict__ x, const float* __restrict__ gate_w,
+                                          const float* __restrict__ gate_bias, float* __restrict__ z, int T, int H,
+                                          int E, uint8_t* smem_raw) {
   uint4* xs4 = reinterpret_cast<uint4*>(smem_raw);
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int t0 = blockIdx.y * kGateTok;
@@ -29,6 +42,7 @@ __global__ void __launch_bounds__(256) gate_logits_kernel(const uint16_t* __rest
     xs4[v] = val;
   }
   __syncthreads();
+  ELDR_STAMP(1);
   const int e = blockIdx.x * kGateExp + warp;
   if (e >= E) return;
   float acc[kGateTok];
@@ -79,6 +93,14 @@ __global__ void __launch_bounds__(256) gate_logits_kernel(const uint16_t* __rest
   }
 }
 
+__global__ void __launch_bounds__(256) gate_logits_kernel(const uint16_t* __restrict__ x,
+                                                          const float* __restrict__ gate_w,
+                                                          const float* __restrict__ gate_bias,
+                                                          float* __restrict__ z, int T, int H, int E) {
+  extern __shared__ __align__(16) uint8_t smem_raw[];
+  gate_tile(x, gate_w, gate_bias, z, T, H, E, smem_raw);
+}
+
 // ----------------------------------------------------------------------- a2: warp softmax top-k
 // One warp, one token.  Lane l holds logits of experts l, l+32, ...  k rounds of warp arg-max with the
 // order (z descending, id ascending); lane j ends up holding the j-th pick and its weight.
@@ -89,7 +111,7 @@ __device__ __forceinline__ void warp_topk(const float* __restrict__ zrow, int E,
 #pragma unroll
   for (int i = 0; i < NV; ++i) {
     const int e = lane + 32 * i;
-    v[i] = (e < E) ? zrow[e] : -INFINITY;
+    v[i] = (e < E) ? __ldcg(zrow + e) : -INFINITY;
   }
   float zmax = v[0];
 #pragma unroll
@@ -178,7 +200,7 @@ __global__ void __launch_bounds__(256) topk_kernel(TopkArgs a) {
 // ------------------------------------------------- a2+a3+a4: top-k, signature, permutation, union
 struct RouteArgs {
   TopkArgs tk;
-  int force_routing, n_shared;
+  int force_routing, n_shared, H;
   int32_t* cnt;        // [E]
   int32_t* off;        // [E+1]
   int32_t* perm;       // [T*k]
@@ -189,10 +211,11 @@ struct RouteArgs {
   int32_t* n_active;   // [1]
 };
 
-// Single CTA (decode batches: T <= 1024).  Membership bitmask mask[e][t/32] makes the counting sort
-// deterministic and atomic-free in global memory: rank of pair (t,e) = popcount of expert e's bits below t.
-__global__ void __launch_bounds__(1024) topk_route_kernel(RouteArgs a) {
-  extern __shared__ __align__(16) uint8_t smem_raw[];
+// Permutation / union compaction by ONE CTA of `nthr` threads (decode batches: T <= 1024).  A membership
+// bitmask mask[e][t/32] in shared memory makes the counting sort deterministic and free of global atomics:
+// rank of pair (t,e) = popcount of expert e's bits below t.  With do_sig the pairs are also recorded in the
+// signature tables (force_routing: the ids were given, no top-k ran).
+__device__ __forceinline__ void route_phases(const RouteArgs& a, uint8_t* smem_raw, int nthr, bool do_sig) {
   const int T = a.tk.T, E = a.tk.E, k = a.tk.k;
   const int W = (T + 31) >> 5;
   uint32_t* mask = reinterpret_cast<uint32_t*>(smem_raw);   // [E][W]
@@ -201,29 +224,21 @@ __global__ void __launch_bounds__(1024) topk_route_kernel(RouteArgs a) {
   int32_t* s_off = s_cnt + E;                                 // [E+1]
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
 
-  for (int i = tid; i < E * W; i += 1024) mask[i] = 0u;
+  for (int i = tid; i < E * W; i += nthr) mask[i] = 0u;
   __syncthreads();
 
-  for (int t = warp; t < T; t += 32) {
-    int id = 0; float w = 0.f;
-    if (!a.force_routing) {
-      warp_topk(a.tk.z + (size_t)t * E, E, k, a.tk.renorm, lane, id, w);
-      if (lane < k) {
-        a.tk.ids[(size_t)t * k + lane] = id;
-        a.tk.w[(size_t)t * k + lane] = w;
-      }
-    } else if (lane < k) {
-      id = min(max(a.tk.ids[(size_t)t * k + lane], 0), E - 1);
-    }
-    if (lane < k) {
-      atomicOr(&mask[id * W + (t >> 5)], 1u << (t & 31));
+  for (int p = tid; p < T * k; p += nthr) {
+    const int t = p / k;
+    const int id = min(max(__ldcg(a.tk.ids + p), 0), E - 1);
+    atomicOr(&mask[id * W + (t >> 5)], 1u << (t & 31));
+    if (do_sig)
       sig_add(a.tk.sig_req, a.tk.sig_block, a.tk.token_req ? a.tk.token_req[t] : -1,
               a.tk.token_block ? a.tk.token_block[t] : -1, a.tk.L, a.tk.layer, E, id);
-    }
   }
   __syncthreads();
+  ELDR_STAMP(6);
 
-  for (int e = tid; e < E; e += 1024) {
+  for (int e = tid; e < E; e += nthr) {
     int run = 0;
     for (int w = 0; w < W; ++w) {
       pref[e * W + w] = run;
@@ -232,6 +247,7 @@ __global__ void __launch_bounds__(1024) topk_route_kernel(RouteArgs a) {
     s_cnt[e] = run;
   }
   __syncthreads();
+  ELDR_STAMP(7);
 
   if (warp == 0) {     // exclusive scan of cnt and ascending compaction of the active experts
     constexpr int PER = kMaxExperts / 32;
@@ -278,15 +294,112 @@ __global__ void __launch_bounds__(1024) topk_route_kernel(RouteArgs a) {
     if (lane < a.n_shared) a.work[n_act + lane] = make_int4(E + lane, T * k, T * k + lane * T, T);
   }
   __syncthreads();
+  ELDR_STAMP(8);
 
-  for (int p = tid; p < T * k; p += 1024) {
+  for (int p = tid; p < T * k; p += nthr) {
     const int t = p / k;
-    const int e = min(max(a.tk.ids[p], 0), E - 1);
+    const int e = min(max(__ldcg(a.tk.ids + p), 0), E - 1);
     const int rank = pref[e * W + (t >> 5)] + __popc(mask[e * W + (t >> 5)] & ((1u << (t & 31)) - 1u));
     const int pos = s_off[e] + rank;
     a.perm[pos] = p;
     a.pair_pos[p] = pos;
   }
+}
+
+// force_routing: ids / weights are inputs; one CTA records the signatures and builds the permutation.
+__global__ void __launch_bounds__(1024) route_only_kernel(RouteArgs a) {
+  extern __shared__ __align__(16) uint8_t smem_raw[];
+  pdl_launch_dependents();
+  route_phases(a, smem_raw, 1024, true);
+}
+
+// ------------------------------------------------------------------ a1..a4 in ONE launch
+// Grid (E/8, T/8).  Every CTA computes its 8-token x 8-expert logit tile.  The LAST CTA of a token group to
+// publish its tile (epoch flags + one atomicExch election; no counters to zero, so no memset in the stream)
+// runs the warp top-k + signature accumulation for that group's 8 tokens, one token per warp; the last GROUP to
+// finish runs the permutation / union compaction.  Latency ~ one GEMV tile + one top-k + one routing pass.
+struct GateRouteArgs {
+  const uint16_t* x;
+  const float* gate_w;
+  const float* gate_bias;
+  RouteArgs r;
+  uint32_t* sync;      // [n_groups*n_etiles] tile flags | [n_groups] elected | [n_groups] group flags | [1] elected
+  uint32_t epoch;      // unique per call
+};
+
+__device__ __forceinline__ uint32_t ld_volatile_u32(const uint32_t* p) {
+  uint32_t v;
+  asm volatile("ld.volatile.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_volatile_u32(uint32_t* p, uint32_t v) {
+  asm volatile("st.volatile.global.u32 [%0], %1;" :: "l"(p), "r"(v) : "memory");
+}
+
+// Publish `mine = epoch`, then return true in exactly one of the CTAs that observe all `n` flags set.
+__device__ __forceinline__ bool publish_and_elect(uint32_t* flags, int n, int mine, uint32_t* elected,
+                                                  uint32_t epoch, int* s_flag) {
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    const int lane = threadIdx.x;
+    if (lane == 0) {
+      st_volatile_u32(flags + mine, epoch);
+      __threadfence();
+    }
+    __syncwarp();
+    bool all = true;
+    for (int i = lane; i < n; i += 32) all = all && (ld_volatile_u32(flags + i) == epoch);
+    all = __all_sync(0xffffffffu, all);
+    if (lane == 0) {
+      int win = 0;
+      if (all) win = (atomicExch(elected, epoch) != epoch);
+      *s_flag = win;
+    }
+  }
+  __syncthreads();
+  const bool win = *s_flag != 0;
+  if (win) __threadfence();
+  return win;
+}
+
+__global__ void __launch_bounds__(256) gate_topk_route_kernel(GateRouteArgs a) {
+  extern __shared__ __align__(16) uint8_t smem_raw[];
+  __shared__ int s_flag;
+  const TopkArgs& tk = a.r.tk;
+  const int T = tk.T, E = tk.E, k = tk.k;
+  const int n_etiles = gridDim.x, n_groups = gridDim.y;
+  ELDR_STAMP(0);
+  pdl_launch_dependents();
+  gate_tile(a.x, a.gate_w, a.gate_bias, const_cast<float*>(tk.z), T, a.r.H, E, smem_raw);
+  ELDR_STAMP(2);
+
+  uint32_t* tile_flags = a.sync;
+  uint32_t* elected = tile_flags + n_groups * n_etiles;
+  uint32_t* group_flags = elected + n_groups;
+  uint32_t* elected2 = group_flags + n_groups;
+  const int g = blockIdx.y;
+  if (!publish_and_elect(tile_flags + g * n_etiles, n_etiles, blockIdx.x, elected + g, a.epoch, &s_flag)) return;
+  ELDR_STAMP(3);
+
+  // top-k + signature for this group's tokens: one token per warp
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int t = g * kGateTok + warp;
+  if (t < T) {
+    int id; float w;
+    warp_topk(tk.z + (size_t)t * E, E, k, tk.renorm, lane, id, w);
+    if (lane < k) {
+      tk.ids[(size_t)t * k + lane] = id;
+      tk.w[(size_t)t * k + lane] = w;
+      sig_add(tk.sig_req, tk.sig_block, tk.token_req ? tk.token_req[t] : -1,
+              tk.token_block ? tk.token_block[t] : -1, tk.L, tk.layer, E, id);
+    }
+  }
+  ELDR_STAMP(4);
+  if (!publish_and_elect(group_flags, n_groups, g, elected2, a.epoch, &s_flag)) return;
+  ELDR_STAMP(5);
+  route_phases(a.r, smem_raw, 256, false);
+  ELDR_STAMP(10);
 }
 
 // x_perm[row] = x[token of sorted pair row]  (rows >= T*k: plain copy of x for the shared experts)
@@ -296,6 +409,8 @@ __global__ void __launch_bounds__(256) gather_x_kernel(const uint16_t* __restric
                                                        int n_rows) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int row = blockIdx.x * 8 + warp;
+  pdl_launch_dependents();
+  pdl_wait();
   if (row >= n_rows) return;
   const int t = (row < T * k) ? perm[row] / k : row - T * k;
   const uint4* src = reinterpret_cast<const uint4*>(x + (size_t)t * H);
@@ -313,16 +428,26 @@ __global__ void __launch_bounds__(256) combine_kernel(const float* __restrict__ 
                                                       int n_shared) {
   const int q_per_row = H >> 2;
   const int idx = blockIdx.x * 256 + threadIdx.x;
+  pdl_wait();
   if (idx >= T * q_per_row) return;
   const int t = idx / q_per_row, c4 = idx - t * q_per_row;
   float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-  for (int j = 0; j < k; ++j) {
-    const int pos = pair_pos[t * k + j];
-    const float wt = w[t * k + j];
-    const float4 v = *reinterpret_cast<const float4*>(y + (size_t)pos * H + (size_t)c4 * 4);
-    acc.x = fmaf(wt, v.x, acc.x); acc.y = fmaf(wt, v.y, acc.y);
-    acc.z = fmaf(wt, v.z, acc.z); acc.w = fmaf(wt, v.w, acc.w);
-  }
+  // two dependent loads per slot (position, then the staged row): issue all of them before the first FMA
+  int pos[kMaxTopK];
+  float wt[kMaxTopK];
+  float4 v[kMaxTopK];
+#pragma unroll
+  for (int j = 0; j < kMaxTopK; ++j)
+    if (j < k) { pos[j] = __ldg(pair_pos + t * k + j); wt[j] = __ldg(w + t * k + j); }
+#pragma unroll
+  for (int j = 0; j < kMaxTopK; ++j)
+    if (j < k) v[j] = __ldcs(reinterpret_cast<const float4*>(y + (size_t)pos[j] * H + (size_t)c4 * 4));
+#pragma unroll
+  for (int j = 0; j < kMaxTopK; ++j)
+    if (j < k) {
+      acc.x = fmaf(wt[j], v[j].x, acc.x); acc.y = fmaf(wt[j], v[j].y, acc.y);
+      acc.z = fmaf(wt[j], v[j].z, acc.z); acc.w = fmaf(wt[j], v[j].w, acc.w);
+    }
   for (int s = 0; s < n_shared; ++s) {
     const float4 v = *reinterpret_cast<const float4*>(y + ((size_t)T * k + (size_t)s * T + t) * H + (size_t)c4 * 4);
     acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;

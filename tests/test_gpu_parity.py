@@ -351,3 +351,20 @@ def test_host_buffer_entry_point_matches_device_entry_point(gpu):
                                    h_na, None, None, None, None, dl.workspace)
     assert torch.equal(h_out.view(torch.int16), ref.cpu().view(torch.int16))
     assert int(h_na.item()) == int(dl.n_active.item())
+
+
+@pytest.mark.parametrize("ffn_path,pdl", [(0, 1), (1, 0), (0, 0)])
+def test_alternate_paths_match_oracle(gpu, oracle, ffn_path, pdl):
+    """The selectable paths (legacy mma.sync FFN, launches without programmatic dependent launch) must pass the
+    same parity gates as the default (tcgen05 + PDL), including multi-pass experts (m > 64) and shared experts."""
+    gpu.eldr_moe_set_option(gpu.OPT_FFN_PATH, ffn_path)
+    gpu.eldr_moe_set_option(gpu.OPT_PDL, pdl)
+    try:
+        shape = synth.MoEShape(hidden=512, inter=256, n_experts=8, top_k=2, n_shared=1, n_layers=2)
+        lw = synth.make_layer_weights(shape, 31, w_std=0.05, gate_std=0.2)
+        x = synth.make_hidden(150, shape.hidden, 31)
+        token_req, token_block = synth.decode_maps(150)
+        run_case(gpu, oracle, shape, lw, x, None, token_req, token_block, n_req=150, n_blk=150, layer=1)
+    finally:
+        gpu.eldr_moe_set_option(gpu.OPT_FFN_PATH, gpu.FFN_TCGEN05)
+        gpu.eldr_moe_set_option(gpu.OPT_PDL, 1)
