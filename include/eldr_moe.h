@@ -157,6 +157,11 @@ int32_t eldr_moe_workspace_layout(const eldr_moe_shape_t* shape, int32_t T, eldr
  *   ELDR_OPT_FFN_PATH: ELDR_FFN_TCGEN05 (default; tcgen05.mma + TMEM) or ELDR_FFN_MMA_SYNC (legacy mma.sync). */
 #define ELDR_OPT_FFN_PATH 0
 #define ELDR_OPT_PDL      1   /* 1 (default): programmatic dependent launch between the step's kernels; 0: plain */
+#define ELDR_OPT_STEP_PATH 2  /* ELDR_STEP_FUSED (default): the whole step in ONE persistent launch (T <= 256,
+                                 H,I % 64 == 0); ELDR_STEP_STAGED: one launch per stage (gate+route, gather, w1/w3, w2,
+                                 combine), also the path for shapes the fused kernel does not take */
+#define ELDR_STEP_STAGED  0
+#define ELDR_STEP_FUSED   1
 #define ELDR_FFN_MMA_SYNC 0
 #define ELDR_FFN_TCGEN05  1
 int32_t eldr_moe_set_option(int32_t key, int32_t value);

@@ -13,6 +13,7 @@
 #include "ffn_stream.cuh"
 #include "ffn_umma.cuh"
 #include "gate_route.cuh"
+#include "moe_fused.cuh"
 
 namespace {
 
@@ -20,6 +21,7 @@ using namespace eldr;
 
 int g_ffn_path = ELDR_FFN_TCGEN05;   // process-wide tuning knobs (eldr_moe_set_option)
 int g_pdl = 1;
+int g_step_path = ELDR_STEP_FUSED;
 
 thread_local char g_err[256] = "";
 thread_local int g_launches = 0;
@@ -76,6 +78,10 @@ void make_layout(const eldr_moe_shape_t* s, int T, eldr_moe_ws_layout_t* L) {
   const size_t Tz = T > 0 ? T : 1;
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + bytes, 256); return r; };
+  // epoch flags first, at a T-independent offset and size: the fused kernel keeps its generation word there
+  const size_t sync_staged = ((size_t)((kFusedMaxT > (int)Tz ? kFusedMaxT : Tz) + kGateTok - 1) / kGateTok * ((E + kGateExp - 1) / kGateExp + 2) + 1) * 4;
+  const size_t sync_fused = ((size_t)kSyncHReady + (E + ns) * ((I + 63) / 64)) * 4;
+  L->sync = take(align_up(sync_fused, 256) + sync_staged);   // [fused | staged]: never aliased (both derive epochs)
   L->z = take(Tz * E * 4);
   L->cnt = take(E * 4);
   L->off = take((E + 1) * 4);
@@ -83,7 +89,6 @@ void make_layout(const eldr_moe_shape_t* s, int T, eldr_moe_ws_layout_t* L) {
   L->pair_pos = take(Tz * k * 4);
   L->work = take((E + ns) * 16);
   L->n_work = take(4);
-  L->sync = take(((size_t)((Tz + kGateTok - 1) / kGateTok) * (((size_t)E + kGateExp - 1) / kGateExp + 2) + 1) * 4);
   L->x_perm = take((Tz * k + Tz) * H * 2);
   L->h = take(Tz * (k + ns) * I * 2);
   L->y = take(Tz * (k + ns) * H * 4);
@@ -263,6 +268,10 @@ int32_t eldr_moe_set_option(int32_t key, int32_t value) {
     g_pdl = value;
     return ELDR_OK;
   }
+  if (key == ELDR_OPT_STEP_PATH && (value == ELDR_STEP_STAGED || value == ELDR_STEP_FUSED)) {
+    g_step_path = value;
+    return ELDR_OK;
+  }
   return ELDR_ERR_INVALID_ARG;
 }
 
@@ -366,6 +375,49 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
   uint16_t* hbuf = reinterpret_cast<uint16_t*>(ws + L.h);
   float* ybuf = reinterpret_cast<float*>(ws + L.y);
 
+  // ------------------------------------------------------------------ whole step in one persistent launch
+  if (g_step_path == ELDR_STEP_FUSED && g_ffn_path == ELDR_FFN_TCGEN05 && H % 64 == 0 && I % 64 == 0 &&
+      T <= kFusedMaxT && num_sms() <= 256) {
+    FusedArgs fa;
+    fa.x = x; fa.gate_w = gate_w; fa.gate_bias = gate_bias;
+    fa.tk = TopkArgs{z, topk_ids, topk_w, token_req, token_block, sig_req, sig_block,
+                     T, E, k, s->n_layers, layer, s->renormalize};
+    fa.force_routing = force_routing ? 1 : 0;
+    fa.n_shared = ns; fa.H = H; fa.I = I;
+    fa.cnt = reinterpret_cast<int32_t*>(ws + L.cnt);
+    fa.off = reinterpret_cast<int32_t*>(ws + L.off);
+    fa.perm = perm; fa.pair_pos = pair_pos; fa.work = work; fa.n_work = n_work;
+    fa.active = active_experts; fa.n_active = n_active;
+    fa.sync = reinterpret_cast<uint32_t*>(ws + L.sync);
+    fa.hbuf = hbuf; fa.ybuf = ybuf; fa.out = out;
+    fa.np = T <= 64 ? 64 : 128;
+    fa.stages = T <= 64 ? 8 : 6;
+    const size_t smem = fused_smem_bytes(fa.stages, fa.np, E, ns, T, k);
+    if (smem <= 227 * 1024) {
+      CUtensorMap tm_w13, tm_sw13, tm_w2, tm_sw2;
+      if (!make_tmap_w13_5d(&tm_w13, w13, E, I, H)) return ELDR_ERR_CUDA;
+      if (!make_tmap(&tm_w2, w2, (uint64_t)E * H, I, 128)) return ELDR_ERR_CUDA;
+      if (ns) {
+        if (!make_tmap_w13_5d(&tm_sw13, shared_w13, ns, I, H)) return ELDR_ERR_CUDA;
+        if (!make_tmap(&tm_sw2, shared_w2, (uint64_t)ns * H, I, 128)) return ELDR_ERR_CUDA;
+      } else {
+        tm_sw13 = tm_w13;
+        tm_sw2 = tm_w2;
+      }
+      static bool fused_attr_set = false;
+      if (!fused_attr_set) {
+        if (!set_smem(moe_fused_kernel, 227 * 1024)) return ELDR_ERR_CUDA;
+        fused_attr_set = true;
+      }
+      prof_begin();
+      prof_mark(0, st);
+      launch_dep(moe_fused_kernel, dim3(num_sms()), dim3(kFusedThreads), smem, st, tm_w13, tm_sw13, tm_w2, tm_sw2, fa);
+      if (!launch_ok("moe_fused_kernel")) return ELDR_ERR_CUDA;
+      prof_mark(ELDR_PROFILE_SLOTS, st);
+      return ELDR_OK;
+    }
+  }
+
   prof_begin();
   RouteArgs ra;
   ra.tk = TopkArgs{z, topk_ids, topk_w, token_req, token_block, sig_req, sig_block,
@@ -389,7 +441,7 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
     static std::atomic<uint32_t> g_epoch{0x5eed0000u};
     GateRouteArgs ga;
     ga.x = x; ga.gate_w = gate_w; ga.gate_bias = gate_bias; ga.r = ra;
-    ga.sync = reinterpret_cast<uint32_t*>(ws + L.sync);
+    ga.sync = reinterpret_cast<uint32_t*>(ws + L.sync + align_up(((size_t)kSyncHReady + (size_t)(E + ns) * ((I + 63) / 64)) * 4, 256));
     ga.epoch = ++g_epoch;
     size_t smem = (size_t)kGateTok * H * 2;
     if (route_smem > smem) smem = route_smem;

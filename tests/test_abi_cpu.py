@@ -43,8 +43,11 @@ def test_workspace_sizes_and_layout(lib):
     assert 0 < b64 < b256
     assert api.eldr_moe_workspace_bytes_host(s, 64) > b64
     L = api.eldr_moe_workspace_layout(s, 64)
-    offs = [L.z, L.cnt, L.off, L.perm, L.pair_pos, L.work, L.n_work, L.sync, L.x_perm, L.h, L.y, L.total]
+    offs = [L.sync, L.z, L.cnt, L.off, L.perm, L.pair_pos, L.work, L.n_work, L.x_perm, L.h, L.y, L.total]
     assert offs == sorted(offs) and L.total == b64 and all(o % 256 == 0 for o in offs)
+    # the epoch-flag region sits first, at an offset and size that do not depend on T (the generation word lives there)
+    L2 = api.eldr_moe_workspace_layout(s, 256)
+    assert L.sync == 0 and L2.sync == 0 and L.z == L2.z
     # y staging [T*k, H] fp32 is the largest intermediate
     assert L.total - L.y >= 64 * 8 * 2048 * 4
 

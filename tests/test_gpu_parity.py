@@ -353,10 +353,13 @@ def test_host_buffer_entry_point_matches_device_entry_point(gpu):
     assert int(h_na.item()) == int(dl.n_active.item())
 
 
-@pytest.mark.parametrize("ffn_path,pdl", [(0, 1), (1, 0), (0, 0)])
-def test_alternate_paths_match_oracle(gpu, oracle, ffn_path, pdl):
-    """The selectable paths (legacy mma.sync FFN, launches without programmatic dependent launch) must pass the
-    same parity gates as the default (tcgen05 + PDL), including multi-pass experts (m > 64) and shared experts."""
+@pytest.mark.parametrize("step_path,ffn_path,pdl", [(1, 1, 0), (0, 1, 1), (0, 0, 1), (0, 1, 0), (0, 0, 0), (1, 1, 1)])
+def test_alternate_paths_match_oracle(gpu, oracle, step_path, ffn_path, pdl):
+    """The selectable paths (one persistent launch vs one launch per stage, legacy mma.sync FFN, launches without
+    programmatic dependent launch) must pass the same parity gates, including multi-pass experts (m > 64) and
+    shared experts.  Consecutive cases reuse the same workspace memory, so this also checks that the epoch flags
+    of one path never confuse the other."""
+    gpu.eldr_moe_set_option(gpu.OPT_STEP_PATH, step_path)
     gpu.eldr_moe_set_option(gpu.OPT_FFN_PATH, ffn_path)
     gpu.eldr_moe_set_option(gpu.OPT_PDL, pdl)
     try:
@@ -364,7 +367,74 @@ def test_alternate_paths_match_oracle(gpu, oracle, ffn_path, pdl):
         lw = synth.make_layer_weights(shape, 31, w_std=0.05, gate_std=0.2)
         x = synth.make_hidden(150, shape.hidden, 31)
         token_req, token_block = synth.decode_maps(150)
-        run_case(gpu, oracle, shape, lw, x, None, token_req, token_block, n_req=150, n_blk=150, layer=1)
+        r = run_case(gpu, oracle, shape, lw, x, None, token_req, token_block, n_req=150, n_blk=150, layer=1)
+        assert gpu.eldr_moe_last_launch_count() == (1 if (step_path == 1 and ffn_path == 1) else 5)
     finally:
+        gpu.eldr_moe_set_option(gpu.OPT_STEP_PATH, gpu.STEP_FUSED)
         gpu.eldr_moe_set_option(gpu.OPT_FFN_PATH, gpu.FFN_TCGEN05)
         gpu.eldr_moe_set_option(gpu.OPT_PDL, 1)
+
+
+@pytest.mark.parametrize("u", [16, 96])
+def test_staged_path_qwen_union(gpu, oracle, qwen_layer, u):
+    """The one-launch-per-stage path (taken for T > 256 and for shapes outside the fused kernel) on the
+    Qwen3-shaped layer, and the same workspace then handed back to the fused path."""
+    shape, lw, dl = qwen_layer
+    T = 64
+    x, bias = synth.union_case(shape, T, u, synth.accepted_union_seed(T, u))
+    token_req, token_block = synth.decode_maps(T)
+    gpu.eldr_moe_set_option(gpu.OPT_STEP_PATH, gpu.STEP_STAGED)
+    try:
+        r = run_case(gpu, oracle, shape, lw, x, bias, token_req, token_block, n_req=T, n_blk=T, layer_obj=dl)
+        assert gpu.eldr_moe_last_launch_count() == 5 and r["n_active"] == u
+    finally:
+        gpu.eldr_moe_set_option(gpu.OPT_STEP_PATH, gpu.STEP_FUSED)
+    r2 = run_case(gpu, oracle, shape, lw, x, bias, token_req, token_block, n_req=T, n_blk=T, layer_obj=dl)
+    assert gpu.eldr_moe_last_launch_count() == 1 and r2["n_active"] == u
+
+
+def test_large_batch_takes_staged_path(gpu, oracle):
+    """T > 256 is outside the fused kernel: the library falls back to the staged kernels by itself."""
+    shape = synth.MoEShape(hidden=256, inter=128, n_experts=16, top_k=4, n_layers=1)
+    lw = synth.make_layer_weights(shape, 5, w_std=0.05, gate_std=0.2)
+    x = synth.make_hidden(300, shape.hidden, 5)
+    run_case(gpu, oracle, shape, lw, x)
+    assert gpu.eldr_moe_last_launch_count() == 5
+
+
+def test_fused_kernel_back_to_back_steps_and_graph_capture(gpu, oracle, qwen_layer):
+    """Many steps enqueued back to back on one workspace (generation word + epoch flags), alternating union
+    sizes, then the same step replayed from a CUDA graph: every replay must reproduce the eager result bit for
+    bit (the launch carries no host-side epoch)."""
+    import torch
+    shape, lw, dl = qwen_layer
+    T = 64
+    cases = []
+    for u in (16, 128, 32):
+        xb, bias = synth.union_case(shape, T, u, synth.accepted_union_seed(T, u))
+        cases.append((u, gpu.bf16_from_bits(xb), torch.from_numpy(bias).cuda()))
+    ref = {}
+    for u, x, b in cases:
+        ref[u] = dl.run(x, b).clone()
+    outs = []
+    for i in range(30):
+        u, x, b = cases[i % 3]
+        outs.append((u, dl.run(x, b).clone()))
+    torch.cuda.synchronize()
+    for u, o in outs:
+        assert torch.equal(o.view(torch.int16), ref[u].view(torch.int16))
+    u, x, b = cases[0]
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        dl.run(x, b)
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            dl.run(x, b)
+    torch.cuda.current_stream().wait_stream(side)
+    for _ in range(5):
+        dl.out.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(dl.out[:T].view(torch.int16), ref[u].view(torch.int16))
+        assert int(dl.n_active.item()) == 16
