@@ -74,10 +74,11 @@ typedef struct {
   size_t pair_pos;   /* int32   [T*k]            inverse of perm                                         */
   size_t work;       /* int32x4 [E+n_shared]     {expert, x_row0, out_row0, m} per streamed expert       */
   size_t n_work;     /* int32   [1]              n_active + n_shared                                     */
-  size_t sync;       /* uint32  [...]            epoch flags of the fused gate/top-k/route kernel (internal)  */
+  size_t sync;       /* uint32  [...]            epoch flags + generation word (internal); offset 0, size independent of T */
   size_t x_perm;     /* bf16    [T*k + T, H]     x gathered in sorted order, then a plain copy of x      */
   size_t h;          /* bf16    [T*(k+ns), I]    silu(W1 x)*(W3 x) per sorted pair, then shared experts  */
   size_t y;          /* float   [T*(k+ns), H]    W2 h per sorted pair, then shared experts               */
+  size_t partial;    /* float   [2][256][128][128] parked fp32 accumulators of tiles split between two SMs (internal) */
   size_t total;      /* bytes needed                                                                    */
 } eldr_moe_ws_layout_t;
 

@@ -39,7 +39,7 @@ class Shape(C.Structure):
 class WsLayout(C.Structure):
     """eldr_moe_ws_layout_t"""
     _fields_ = [(n, C.c_size_t) for n in ("z", "cnt", "off", "perm", "pair_pos", "work", "n_work", "sync",
-                                          "x_perm", "h", "y", "total")]
+                                          "x_perm", "h", "y", "partial", "total")]
 
 
 def lib_path() -> str:

@@ -80,7 +80,7 @@ void make_layout(const eldr_moe_shape_t* s, int T, eldr_moe_ws_layout_t* L) {
   auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + bytes, 256); return r; };
   // epoch flags first, at a T-independent offset and size: the fused kernel keeps its generation word there
   const size_t sync_staged = ((size_t)((kFusedMaxT > (int)Tz ? kFusedMaxT : Tz) + kGateTok - 1) / kGateTok * ((E + kGateExp - 1) / kGateExp + 2) + 1) * 4;
-  const size_t sync_fused = ((size_t)kSyncHReady + (E + ns) * ((I + 63) / 64)) * 4;
+  const size_t sync_fused = fused_sync_words((int)E, (int)ns, (int)I) * 4;
   L->sync = take(align_up(sync_fused, 256) + sync_staged);   // [fused | staged]: never aliased (both derive epochs)
   L->z = take(Tz * E * 4);
   L->cnt = take(E * 4);
@@ -92,6 +92,7 @@ void make_layout(const eldr_moe_shape_t* s, int T, eldr_moe_ws_layout_t* L) {
   L->x_perm = take((Tz * k + Tz) * H * 2);
   L->h = take(Tz * (k + ns) * I * 2);
   L->y = take(Tz * (k + ns) * H * 4);
+  L->partial = take(fused_partial_bytes(256));   // stream-K fix-up slots of the fused kernel (grid <= 256 CTAs)
   L->total = o;
 }
 
@@ -390,10 +391,14 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
     fa.active = active_experts; fa.n_active = n_active;
     fa.sync = reinterpret_cast<uint32_t*>(ws + L.sync);
     fa.hbuf = hbuf; fa.ybuf = ybuf; fa.out = out;
-    fa.np = T <= 64 ? 64 : 128;
-    fa.stages = T <= 64 ? 8 : 6;
-    const size_t smem = fused_smem_bytes(fa.stages, fa.np, E, ns, T, k);
-    if (smem <= 227 * 1024) {
+    fa.partial = reinterpret_cast<float*>(ws + L.partial);
+    const size_t smem_max = 227 * 1024;
+    const size_t fixed = fused_smem_fixed_bytes(E, ns, T, k);
+    const size_t min_area = (size_t)3 * (kUmmaWBytes + kNPCap * 128) > (size_t)kGateTok * H * 2
+                                ? (size_t)3 * (kUmmaWBytes + kNPCap * 128) : (size_t)kGateTok * H * 2;
+    fa.stage_area = fixed < smem_max ? (int)((smem_max - fixed) / 1024 * 1024) : 0;
+    const size_t smem = fixed + fa.stage_area;
+    if ((size_t)fa.stage_area >= min_area) {
       CUtensorMap tm_w13, tm_sw13, tm_w2, tm_sw2;
       if (!make_tmap_w13_5d(&tm_w13, w13, E, I, H)) return ELDR_ERR_CUDA;
       if (!make_tmap(&tm_w2, w2, (uint64_t)E * H, I, 128)) return ELDR_ERR_CUDA;
@@ -441,7 +446,7 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
     static std::atomic<uint32_t> g_epoch{0x5eed0000u};
     GateRouteArgs ga;
     ga.x = x; ga.gate_w = gate_w; ga.gate_bias = gate_bias; ga.r = ra;
-    ga.sync = reinterpret_cast<uint32_t*>(ws + L.sync + align_up(((size_t)kSyncHReady + (size_t)(E + ns) * ((I + 63) / 64)) * 4, 256));
+    ga.sync = reinterpret_cast<uint32_t*>(ws + L.sync + align_up(fused_sync_words(E, ns, I) * 4, 256));
     ga.epoch = ++g_epoch;
     size_t smem = (size_t)kGateTok * H * 2;
     if (route_smem > smem) smem = route_smem;

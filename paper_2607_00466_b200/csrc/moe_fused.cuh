@@ -2,28 +2,34 @@
 // "the gate partitions the batch among experts ... each step fetches the weights of every expert the batch
 // activates"; PAPER.md:198/:253 signature counts).  One CTA per SM, 8 warps.
 //
-//   G  gate GEMV: 8-token x 8-expert logit tiles spread over the grid (fp32 FMA, gate rows prefetched 16 deep
-//      while the x tile lands in shared memory); each tile publishes an epoch flag.
+//   G  gate GEMV: 8-token x 8-expert logit tiles spread over the grid.  fp32 FMA on CUDA cores; a warp owns
+//      2 experts x 4 tokens (halves the shared-memory traffic of 1 x 8), gate rows are requested 8 float4 deep
+//      per row BEFORE the x tile is staged so both latencies overlap.  Each tile publishes an epoch flag.
 //   K  top-k: the CTA that owns token group g polls the group's tile flags, runs a redux-based warp top-k
 //      (+ fused signature increments), publishes the group flag.
 //   R  routing, redundantly in EVERY CTA from the 4*T*k bytes of ids: membership bitmasks -> counts ->
-//      offsets -> union-compacted work list -> token<->position maps, all in shared memory (no second
-//      election, no route/gather kernels, no work-list round trip through HBM).  CTA 0 also writes the
-//      routing outputs of the C ABI (active list, n_active, cnt/off/perm/pair_pos).
-//   F  expert FFN on tcgen05 + TMEM, swap-AB (weights = M operand, the expert's tokens = N operand).  Work
-//      units = [w1/w3 tiles of all active experts, expert-major] ++ [w2 tiles, expert-major], claimed from a
-//      global counter (first unit static) by the weights-producer lane and broadcast to the other roles through
-//      a 4-slot shared-memory ring.  Weights: TMA (SWIZZLE_128B, evict_first), 16 KiB per stage.  Activations:
-//      a producer warp gathers the expert's token rows with cp.async straight from x (w1/w3) or h (w2) into the
-//      swizzled K-major B tile -- the permutation is never materialised in HBM.  A w2 unit of expert e waits on
-//      the epoch flags of e's w1/w3 tiles (release/acquire through L2); the queue order makes this
-//      deadlock-free: a unit only ever waits on units claimed before it.
-//   C  ordered combine: after a flag barrier over the grid, out[t] = sum_j w[t,j]*y[pos(t,j)] (+ shared) in
-//      slot order, one RNE rounding to bf16: run-to-run bit-identical.
+//      offsets -> union-compacted work list (the weights producer starts streaming here) -> token<->position
+//      maps, all in shared memory.  No second election, no route/gather kernels, no work list in HBM.
+//      CTA 0 also writes the routing outputs of the C ABI (active list, n_active, cnt/off/perm/pair_pos).
+//   F  expert FFN on tcgen05 + TMEM, swap-AB (weights = M=128 operand, the expert's tokens = N operand), as a
+//      STATIC stream-K schedule: per phase (A: w1/w3 tiles, B: w2 tiles) the flattened sequence of 16 KiB
+//      weight stages (tile-major, k-chunk minor) is cut into gridDim.x equal contiguous ranges, so every SM
+//      streams the same number of bytes (+-1 stage) whatever the union size.  A tile cut by a range boundary
+//      is finished by the CTA that owns its k=0 end: the other owner(s) -- which reach the tile FIRST, at the
+//      start of their range -- park raw fp32 accumulators in a scratch slot and raise a flag; the head owner adds
+//      them in ascending CTA order (a fixed order: results are run-to-run bit-identical).  Weights: TMA
+//      (SWIZZLE_128B, evict_first).  Activations: a producer warp gathers the expert's token rows with cp.async
+//      straight from x (A) or h (B) into the swizzled K-major B tile -- the permutation never exists in HBM.
+//      Phase B waits on per-tile epoch flags of the expert's h tiles (release/acquire through L2).  Phase A
+//      never waits on phase B and first pieces never wait on anything, so there is no cycle.
+//      The B-tile rows per stage adapt to the batch's largest tokens-per-expert count, so small-m steps get a
+//      deeper weight ring (more bytes in flight).
+//   C  ordered combine after a flag barrier over the grid: out[t] = sum_j w[t,j]*y[pos(t,j)] (+ shared) in
+//      slot order, one RNE rounding to bf16.
 //
-// No counter needs zeroing by the host: flags compare against epoch = gen+1, gen lives in the workspace and is
-// bumped by CTA 0 after the last barrier (so the launch is CUDA-graph capturable and robust to a workspace of
-// arbitrary initial contents up to a 2^-32 flag collision).
+// Nothing needs zeroing by the host: flags compare against epoch = gen+1; gen lives in the workspace and is
+// bumped by CTA 0 after the last barrier (the launch is CUDA-graph capturable; a workspace of arbitrary initial
+// contents works up to a 2^-32 flag collision).
 #pragma once
 #include "device_utils.cuh"
 #include "ffn_umma.cuh"
@@ -33,17 +39,24 @@ namespace eldr {
 
 constexpr int kFusedThreads = 256;
 constexpr int kFusedMaxT = 256;
-constexpr int kSchedSlots = 4;
-constexpr int kXLag = 4;                  // cp.async groups kept in flight by the activations producer
+constexpr int kNPCap = 128;               // token columns per accumulator pass (TMEM: 2 x 128 columns)
+constexpr int kMaxStages = 12;
+constexpr int kXLag = 2;                  // cp.async groups kept in flight by EACH of the two activations producers
 
 // sync region (uint32 words) at the START of the layer workspace
 constexpr int kSyncGen = 0;
-constexpr int kSyncCounter = 1;
-constexpr int kSyncSchedReady = 2;
-constexpr int kSyncDone = 32;             // [256]  per-CTA "all my units are finished"
-constexpr int kSyncGroup = kSyncDone + 256;     // [32]   per token group "ids/weights written"
-constexpr int kSyncTile = kSyncGroup + 32;      // [32 groups][32 expert tiles] gate logits written
-constexpr int kSyncHReady = kSyncTile + 1024;   // [(E+ns) work slots][tilesA] h tile written
+constexpr int kSyncDone = 32;                   // [256]     per CTA "all my pieces are finished"
+constexpr int kSyncGroup = kSyncDone + 256;     // [32]      per token group "ids/weights written"
+constexpr int kSyncTile = kSyncGroup + 32;      // [32][32]  gate logit tile written
+constexpr int kSyncPartial = kSyncTile + 1024;  // [2][256]  per (phase, CTA) "partial accumulators parked"
+constexpr int kSyncHReady = kSyncPartial + 512; // [(E+ns)*2*tilesA] per phase-A tile "h tile written"
+
+__host__ __device__ inline size_t fused_sync_words(int E, int ns, int I) {
+  return (size_t)kSyncHReady + (size_t)(E + ns) * 2 * ((I + 63) / 64);
+}
+__host__ __device__ inline size_t fused_partial_bytes(int n_cta) {
+  return (size_t)2 * n_cta * 128 * kNPCap * 4;
+}
 
 struct FusedArgs {
   const uint16_t* x;
@@ -60,11 +73,25 @@ struct FusedArgs {
   int32_t* active;
   int32_t* n_active;
   uint32_t* sync;
+  float* partial;              // [2][gridDim.x][128][kNPCap] fp32 scratch of the stream-K fix-up
   uint16_t* hbuf;              // [T*(k+ns), I] bf16
   float* ybuf;                 // [T*(k+ns), H] fp32
   uint16_t* out;               // [T,H] bf16
-  int np, stages;              // token rows per pass (64|128), smem ring depth
+  int stage_area;              // bytes of shared memory cut into ring stages (multiple of 1024; set by the host)
 };
+
+#ifdef ELDR_TRACE
+__device__ __forceinline__ unsigned long long gtime() {
+  unsigned long long t_;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_));
+  return t_;
+}
+#define FSTAMP(id) do { g_trace[(blockIdx.x & 4095) * 16 + (id)] = gtime(); } while (0)
+#define FVALUE(id, v) do { g_trace[(blockIdx.x & 4095) * 16 + (id)] = (unsigned long long)(v); } while (0)
+#else
+#define FSTAMP(id) do {} while (0)
+#define FVALUE(id, v) do {} while (0)
+#endif
 
 __device__ __forceinline__ void flag_release(uint32_t* p, uint32_t v) {
   asm volatile("st.release.gpu.global.u32 [%0], %1;" :: "l"(p), "r"(v) : "memory");
@@ -74,15 +101,22 @@ __device__ __forceinline__ uint32_t flag_acquire(const uint32_t* p) {
   asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
 }
-// One warp waits until flags[0..n) all equal epoch (lanes stride over the flags).  Traps instead of hanging.
+// One warp waits until flags[0..n) all equal epoch (lanes stride over the flags; a short sleep between polls
+// keeps 148 pollers from saturating the flag's L2 slice).  Traps instead of hanging.
 __device__ __forceinline__ void warp_wait_flags(const uint32_t* flags, int n, uint32_t epoch, int lane) {
   for (int i = lane; i < n; i += 32) {
     uint32_t spins = 0;
     while (flag_acquire(flags + i) != epoch) {
+      __nanosleep(40);
       if (++spins > (1u << 24)) __trap();
     }
   }
   __syncwarp();
+}
+__device__ __forceinline__ bool warp_test_flags(const uint32_t* flags, int n, uint32_t epoch, int lane) {
+  bool ok = true;
+  for (int i = lane; i < n; i += 32) ok = ok && (flag_acquire(flags + i) == epoch);
+  return __all_sync(0xffffffffu, ok);
 }
 
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
@@ -94,42 +128,57 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 // ------------------------------------------------------------------------------------ G: one logit tile
-// 8 tokens (group g) x 8 experts (tile et), warp w owns expert et*8+w.  The first 16 float4 of the gate row
-// are requested BEFORE the x tile is staged, so the two DRAM/L2 latencies overlap.
+// 8 tokens (group g) x 8 experts (tile et).  Warp w: experts 2*(w&3), 2*(w&3)+1 of the tile, tokens 4*(w>>2)..+3.
 __device__ __forceinline__ void fused_gate_tile(const FusedArgs& a, int et, int g, uint8_t* smem_raw) {
   const int T = a.tk.T, H = a.H, E = a.tk.E;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int t0 = g * kGateTok;
-  const int e = et * kGateExp + warp;
+  const int ep = warp & 3, th = warp >> 2;
+  const int e0 = et * kGateExp + 2 * ep, e1 = e0 + 1;
   const int q_per_row = H >> 2;
-  constexpr int kDepth = 16;
-  const float4* wrow = reinterpret_cast<const float4*>(a.gate_w + (size_t)(e < E ? e : 0) * H);
-  float4 wv[kDepth];
+  constexpr int kDepth = 8;
+  const float4* wrow0 = reinterpret_cast<const float4*>(a.gate_w + (size_t)(e0 < E ? e0 : 0) * H);
+  const float4* wrow1 = reinterpret_cast<const float4*>(a.gate_w + (size_t)(e1 < E ? e1 : 0) * H);
+  const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
+  float4 wa[kDepth], wb[kDepth];
 #pragma unroll
   for (int u = 0; u < kDepth; ++u) {
     const int c4 = lane + 32 * u;
-    wv[u] = (e < E && c4 < q_per_row) ? __ldg(wrow + c4) : make_float4(0.f, 0.f, 0.f, 0.f);
+    wa[u] = (c4 < q_per_row) ? __ldg(wrow0 + c4) : zero4;
+    wb[u] = (c4 < q_per_row) ? __ldg(wrow1 + c4) : zero4;
   }
   uint4* xs4 = reinterpret_cast<uint4*>(smem_raw);
   const int vec_per_row = H >> 3;
+  const int n_vec = kGateTok * vec_per_row;
   __syncthreads();                       // the previous tile's readers are done with the x tile
-  for (int v = tid; v < kGateTok * vec_per_row; v += kFusedThreads) {
-    const int t = v / vec_per_row, c = v - t * vec_per_row;
-    uint4 val = make_uint4(0u, 0u, 0u, 0u);
-    if (t0 + t < T) val = __ldcg(reinterpret_cast<const uint4*>(a.x + (size_t)(t0 + t) * H + (size_t)c * 8));
-    xs4[v] = val;
+  for (int v0 = 0; v0 < n_vec; v0 += 8 * kFusedThreads) {
+    uint4 val[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      const int v = v0 + tid + j * kFusedThreads;
+      const int t = v / vec_per_row, c = v - t * vec_per_row;
+      val[j] = make_uint4(0u, 0u, 0u, 0u);
+      if (v < n_vec && t0 + t < T) val[j] = __ldcg(reinterpret_cast<const uint4*>(a.x + (size_t)(t0 + t) * H + (size_t)c * 8));
+    }
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      const int v = v0 + tid + j * kFusedThreads;
+      if (v < n_vec) xs4[v] = val[j];
+    }
   }
   __syncthreads();
-  float acc[kGateTok];
+  if (tid == 0) FSTAMP(14);
+  float acc0[4], acc1[4];
 #pragma unroll
-  for (int t = 0; t < kGateTok; ++t) acc[t] = 0.f;
-  const uint2* xs2 = reinterpret_cast<const uint2*>(smem_raw);
+  for (int t = 0; t < 4; ++t) { acc0[t] = 0.f; acc1[t] = 0.f; }
+  const uint2* xs2 = reinterpret_cast<const uint2*>(smem_raw) + (size_t)(4 * th) * q_per_row;
   for (int base = 0; base < q_per_row; base += 32 * kDepth) {
     if (base > 0) {
 #pragma unroll
       for (int u = 0; u < kDepth; ++u) {
         const int c4 = base + lane + 32 * u;
-        wv[u] = (e < E && c4 < q_per_row) ? __ldg(wrow + c4) : make_float4(0.f, 0.f, 0.f, 0.f);
+        wa[u] = (c4 < q_per_row) ? __ldg(wrow0 + c4) : zero4;
+        wb[u] = (c4 < q_per_row) ? __ldg(wrow1 + c4) : zero4;
       }
     }
 #pragma unroll
@@ -137,31 +186,42 @@ __device__ __forceinline__ void fused_gate_tile(const FusedArgs& a, int et, int 
       const int c4 = base + lane + 32 * u;
       if (c4 < q_per_row) {
 #pragma unroll
-        for (int t = 0; t < kGateTok; ++t) {
+        for (int t = 0; t < 4; ++t) {
           const uint2 xv = xs2[t * q_per_row + c4];
-          float s = acc[t];
-          s = fmaf(wv[u].x, bf16_lo(xv.x), s);
-          s = fmaf(wv[u].y, bf16_hi(xv.x), s);
-          s = fmaf(wv[u].z, bf16_lo(xv.y), s);
-          s = fmaf(wv[u].w, bf16_hi(xv.y), s);
-          acc[t] = s;
+          const float x0 = bf16_lo(xv.x), x1 = bf16_hi(xv.x), x2 = bf16_lo(xv.y), x3 = bf16_hi(xv.y);
+          float s0 = acc0[t], s1 = acc1[t];
+          s0 = fmaf(wa[u].x, x0, s0); s1 = fmaf(wb[u].x, x0, s1);
+          s0 = fmaf(wa[u].y, x1, s0); s1 = fmaf(wb[u].y, x1, s1);
+          s0 = fmaf(wa[u].z, x2, s0); s1 = fmaf(wb[u].z, x2, s1);
+          s0 = fmaf(wa[u].w, x3, s0); s1 = fmaf(wb[u].w, x3, s1);
+          acc0[t] = s0; acc1[t] = s1;
         }
       }
     }
   }
 #pragma unroll
-  for (int t = 0; t < kGateTok; ++t) {
-    float s = acc[t];
+  for (int t = 0; t < 4; ++t) {
+    float s0 = acc0[t], s1 = acc1[t];
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-    acc[t] = s;
+    for (int o = 16; o > 0; o >>= 1) {
+      s0 += __shfl_xor_sync(0xffffffffu, s0, o);
+      s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+    }
+    acc0[t] = s0; acc1[t] = s1;
   }
-  if (lane == 0 && e < E) {
-    const float b = a.gate_bias ? a.gate_bias[e] : 0.f;
+  if (tid == 0) FSTAMP(15);
+  if (lane == 0) {
     float* z = const_cast<float*>(a.tk.z);
+    const float b0 = (a.gate_bias && e0 < E) ? a.gate_bias[e0] : 0.f;
+    const float b1 = (a.gate_bias && e1 < E) ? a.gate_bias[e1] : 0.f;
 #pragma unroll
-    for (int t = 0; t < kGateTok; ++t)
-      if (t0 + t < T) z[(size_t)(t0 + t) * E + e] = acc[t] + b;
+    for (int t = 0; t < 4; ++t) {
+      const int tt = t0 + 4 * th + t;
+      if (tt < T) {
+        if (e0 < E) z[(size_t)tt * E + e0] = acc0[t] + b0;
+        if (e1 < E) z[(size_t)tt * E + e1] = acc1[t] + b1;
+      }
+    }
   }
 }
 
@@ -185,13 +245,11 @@ __device__ __forceinline__ void warp_topk_redux(const float* __restrict__ zrow, 
     key[i] = (e < E) ? f32_order_key(__ldcg(zrow + e)) : 0u;      // 0 = "absent": below every finite key
   }
   float denom_all = 0.f;
-  uint32_t kmax_all = 0u;
   if (!renorm) {
     uint32_t m = key[0];
 #pragma unroll
     for (int i = 1; i < NV; ++i) m = max(m, key[i]);
-    kmax_all = __reduce_max_sync(0xffffffffu, m);
-    const float zmax = f32_from_order_key(kmax_all);
+    const float zmax = f32_from_order_key(__reduce_max_sync(0xffffffffu, m));
 #pragma unroll
     for (int i = 0; i < NV; ++i)
       if (lane + 32 * i < E) denom_all += expf(f32_from_order_key(key[i]) - zmax);
@@ -230,29 +288,36 @@ __device__ __forceinline__ void warp_topk_redux(const float* __restrict__ zrow, 
 
 // ------------------------------------------------------------------------------------ shared-memory plan
 struct FusedSmem {
-  uint32_t stage_base;     // S stages of [16 KiB weights | np*128 B activations], 1024-aligned
-  uint32_t bar_base;       // full[S], empty[S], tfull[2], tempty[2], sfull[4], sempty[4]
+  uint32_t stage_base;     // stage_area bytes cut into S stages of [16 KiB weights | np*128 B activations]
+  uint32_t bar_base;       // full[kMaxStages], empty[kMaxStages], tfull[2], tempty[2]
   uint32_t tmem_slot;
-  int4* ring;              // [kSchedSlots] {unit or -1,..}
   int4* work;              // [E+ns] {expert, x_row0, out_row0, m}
-  int32_t* n_work;         // [1]
+  int32_t* cumpass;        // [E+ns+1] exclusive scan of accumulator passes per work entry
+  int32_t* meta;           // [8] {n_work, np, S, total passes}
   uint16_t* tok_of_pos;    // [T*k (+T)]
   uint16_t* pos_of_pair;   // [T*k]
+  uint8_t* ids8;           // [T*k] expert id of each pair (E <= 256)
+  uint8_t* route_scratch;  // mask [E][W], pref [E][W], cnt [E], off [E+1] (part a -> part b)
 };
 
-__host__ __device__ inline size_t fused_smem_bytes(int S, int np, int E, int ns, int T, int k) {
-  size_t o = (size_t)S * (kUmmaWBytes + (size_t)np * 128);
-  o += (2 * (size_t)S + 12) * 8 + 16;                    // barriers + tmem slot
-  o += kSchedSlots * 16;
-  o += (size_t)(E + ns) * 16 + 16;
+// Bytes of everything except the stage ring (barriers, routing tables); the host gives the ring what is left.
+__host__ __device__ inline size_t fused_smem_fixed_bytes(int E, int ns, int T, int k) {
+  const size_t W = (T + 31) / 32;
+  size_t o = 256;                                        // barriers + tmem slot
+  o += (size_t)(E + ns) * 16;
+  o += ((size_t)(E + ns + 1) * 4 + 15) / 16 * 16;
+  o += 32;
   o += (((size_t)T * k + T) * 2 + 15) / 16 * 16;
   o += ((size_t)T * k * 2 + 15) / 16 * 16;
+  o += ((size_t)T * k + 15) / 16 * 16;
+  o += ((size_t)E * W * 8 + (size_t)(2 * E + 1) * 4 + 15) / 16 * 16;   // route scratch: mask, pref, cnt, off
   return o + 1024;                                       // alignment slack
 }
 
-// ---------------------------------------------------------------------------------------- R: local routing
-// Scratch (mask, pref, s_cnt, s_off) lives in the (not yet used) stage area.
-__device__ __forceinline__ void fused_route(const FusedArgs& a, const FusedSmem& sm, uint8_t* scratch, bool is_cta0) {
+// ------------------------------------------------------------------------------ R (part a): union + work list
+// Scratch (mask, pref, s_cnt, s_off) has its own shared-memory region: part b still reads it while the weights
+// producer is already filling the stage ring.
+__device__ __forceinline__ void fused_route_a(const FusedArgs& a, const FusedSmem& sm, uint8_t* scratch, bool is_cta0) {
   const int T = a.tk.T, E = a.tk.E, k = a.tk.k, ns = a.n_shared;
   const int W = (T + 31) >> 5;
   uint32_t* mask = reinterpret_cast<uint32_t*>(scratch);     // [E][W]
@@ -262,15 +327,37 @@ __device__ __forceinline__ void fused_route(const FusedArgs& a, const FusedSmem&
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const bool do_sig = is_cta0 && a.force_routing;
 
+  // ids: all loads in flight before the first use
+  constexpr int kIdsPer = 4;
+  int idr[kIdsPer];
+#pragma unroll
+  for (int j = 0; j < kIdsPer; ++j) {
+    const int p = tid + j * kFusedThreads;
+    idr[j] = (p < T * k) ? __ldcg(a.tk.ids + p) : 0;
+  }
   for (int i = tid; i < E * W; i += kFusedThreads) mask[i] = 0u;
   __syncthreads();
-  for (int p = tid; p < T * k; p += kFusedThreads) {
-    const int t = p / k;
-    const int id = min(max(__ldcg(a.tk.ids + p), 0), E - 1);
-    atomicOr(&mask[id * W + (t >> 5)], 1u << (t & 31));
-    if (do_sig)
-      sig_add(a.tk.sig_req, a.tk.sig_block, a.tk.token_req ? a.tk.token_req[t] : -1,
-              a.tk.token_block ? a.tk.token_block[t] : -1, a.tk.L, a.tk.layer, E, id);
+  for (int p0 = 0; p0 < T * k; p0 += kIdsPer * kFusedThreads) {
+    if (p0 > 0) {
+#pragma unroll
+      for (int j = 0; j < kIdsPer; ++j) {
+        const int p = p0 + tid + j * kFusedThreads;
+        idr[j] = (p < T * k) ? __ldcg(a.tk.ids + p) : 0;
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < kIdsPer; ++j) {
+      const int p = p0 + tid + j * kFusedThreads;
+      if (p < T * k) {
+        const int t = p / k;
+        const int id = min(max(idr[j], 0), E - 1);
+        sm.ids8[p] = (uint8_t)id;
+        atomicOr(&mask[id * W + (t >> 5)], 1u << (t & 31));
+        if (do_sig)
+          sig_add(a.tk.sig_req, a.tk.sig_block, a.tk.token_req ? a.tk.token_req[t] : -1,
+                  a.tk.token_block ? a.tk.token_block[t] : -1, a.tk.L, a.tk.layer, E, id);
+      }
+    }
   }
   __syncthreads();
   for (int e = tid; e < E; e += kFusedThreads) {
@@ -284,13 +371,14 @@ __device__ __forceinline__ void fused_route(const FusedArgs& a, const FusedSmem&
   __syncthreads();
   if (warp == 0) {
     constexpr int PER = kMaxExperts / 32;
-    int c[PER], csum = 0, asum = 0;
+    int c[PER], csum = 0, asum = 0, cmax = 0;
 #pragma unroll
     for (int i = 0; i < PER; ++i) {
       const int e = lane * PER + i;
       c[i] = (e < E) ? s_cnt[e] : 0;
       csum += c[i];
       asum += (c[i] > 0);
+      cmax = max(cmax, c[i]);
     }
     int cinc = csum, ainc = asum;
 #pragma unroll
@@ -299,6 +387,8 @@ __device__ __forceinline__ void fused_route(const FusedArgs& a, const FusedSmem&
       const int av = __shfl_up_sync(0xffffffffu, ainc, o);
       if (lane >= o) { cinc += cv; ainc += av; }
     }
+    cmax = (int)__reduce_max_sync(0xffffffffu, (unsigned)cmax);
+    if (ns) cmax = T;
     int coff = cinc - csum, aoff = ainc - asum;
     const int n_act = __shfl_sync(0xffffffffu, ainc, 31);
     const int total = __shfl_sync(0xffffffffu, cinc, 31);
@@ -319,21 +409,61 @@ __device__ __forceinline__ void fused_route(const FusedArgs& a, const FusedSmem&
     }
     if (is_cta0)
       for (int i = n_act + lane; i < E; i += 32) a.active[i] = -1;
-    if (lane == 0) {
-      s_off[E] = total;
-      *sm.n_work = n_act + ns;
-      if (is_cta0) { a.off[E] = total; *a.n_active = n_act; *a.n_work = n_act + ns; }
-    }
     if (lane < ns) {
       const int4 wk = make_int4(E + lane, T * k, T * k + lane * T, T);
       sm.work[n_act + lane] = wk;
       if (is_cta0) a.work[n_act + lane] = wk;
     }
+    __syncwarp();
+    // accumulator passes per entry (1 unless an expert got more than kNPCap tokens) and their exclusive scan
+    const int n_work = n_act + ns;
+    constexpr int PER2 = (kMaxExperts + 8 + 31) / 32;
+    int ps = 0;
+#pragma unroll
+    for (int i = 0; i < PER2; ++i) {
+      const int ent = lane * PER2 + i;
+      if (ent < n_work) ps += (sm.work[ent].w + kNPCap - 1) / kNPCap;
+    }
+    int pinc = ps;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int pv = __shfl_up_sync(0xffffffffu, pinc, o);
+      if (lane >= o) pinc += pv;
+    }
+    int poff = pinc - ps;
+#pragma unroll
+    for (int i = 0; i < PER2; ++i) {
+      const int ent = lane * PER2 + i;
+      if (ent < n_work) {
+        sm.cumpass[ent] = poff;
+        poff += (sm.work[ent].w + kNPCap - 1) / kNPCap;
+      }
+    }
+    if (lane == 31) sm.cumpass[n_work] = pinc;
+    if (lane == 0) {
+      const int np = (min(cmax, kNPCap) + 15) & ~15;
+      s_off[E] = total;
+      sm.meta[0] = n_work;
+      sm.meta[1] = np;
+      sm.meta[2] = min(kMaxStages, a.stage_area / (kUmmaWBytes + np * 128));
+      if (is_cta0) { a.off[E] = total; *a.n_active = n_act; *a.n_work = n_work; }
+    }
+    if (lane == 31) sm.meta[3] = pinc;
   }
   __syncthreads();
-  for (int p = tid; p < T * k; p += kFusedThreads) {
+}
+
+// ---------------------------------------------------------------------- R (part b): token <-> position maps
+__device__ __forceinline__ void fused_route_b(const FusedArgs& a, const FusedSmem& sm, uint8_t* scratch, bool is_cta0,
+                                              int tid, int nthr) {
+  const int T = a.tk.T, E = a.tk.E, k = a.tk.k, ns = a.n_shared;
+  const int W = (T + 31) >> 5;
+  const uint32_t* mask = reinterpret_cast<const uint32_t*>(scratch);
+  const uint32_t* pref = mask + (size_t)E * W;
+  const int32_t* s_off = reinterpret_cast<const int32_t*>(pref + (size_t)E * W) + E;
+  for (int p = tid; p < T * k; p += nthr) {
     const int t = p / k;
-    const int e = min(max(__ldcg(a.tk.ids + p), 0), E - 1);
+    const int e = sm.ids8[p];
     const int rank = pref[e * W + (t >> 5)] + __popc(mask[e * W + (t >> 5)] & ((1u << (t & 31)) - 1u));
     const int pos = s_off[e] + rank;
     sm.tok_of_pos[pos] = (uint16_t)t;
@@ -341,13 +471,46 @@ __device__ __forceinline__ void fused_route(const FusedArgs& a, const FusedSmem&
     if (is_cta0) { a.perm[pos] = p; a.pair_pos[p] = pos; }
   }
   if (ns)
-    for (int t = tid; t < T; t += kFusedThreads) sm.tok_of_pos[T * k + t] = (uint16_t)t;
-  __syncthreads();
+    for (int t = tid; t < T; t += nthr) sm.tok_of_pos[T * k + t] = (uint16_t)t;
 }
 
-// ------------------------------------------------------------------------------------------- the kernel
-struct UnitInfo { int mode, ent, rt; };
+// -------------------------------------------------------------------------------- F: stream-K piece walker
+// Phase ph (0: w1/w3, 1: w2): tiles = (work entry, pass, row tile), flattened entry-major; each tile has `kit`
+// k-chunks (stages).  CTA c owns stages [c*P/G, (c+1)*P/G).  A piece = the part of one tile inside that range.
+struct Piece {
+  int tile, k0, k1, ent, pass, rt;
+};
+struct PieceWalker {
+  int tpe, kit;          // row tiles per (entry, pass); k-chunks per tile
+  long long g, hi;       // current / end stage
+  int ent;               // cursor into cumpass
+  const int32_t* cumpass;
+  __device__ __forceinline__ void init(int ph, int tilesA, int tilesB, int kitA, int kitB, int total_pass,
+                                       const int32_t* cp, int cta, int G) {
+    tpe = ph == 0 ? tilesA : tilesB;
+    kit = ph == 0 ? kitA : kitB;
+    const long long P = (long long)total_pass * tpe * kit;
+    g = P * cta / G;
+    hi = P * (cta + 1) / G;
+    ent = 0;
+    cumpass = cp;
+  }
+  __device__ __forceinline__ bool next(Piece& p) {
+    if (g >= hi) return false;
+    p.tile = (int)(g / kit);
+    p.k0 = (int)(g - (long long)p.tile * kit);
+    p.k1 = (int)min((long long)kit, p.k0 + (hi - g));
+    const int cpi = p.tile / tpe;
+    p.rt = p.tile - cpi * tpe;
+    while (cumpass[ent + 1] <= cpi) ++ent;
+    p.ent = ent;
+    p.pass = cpi - cumpass[ent];
+    g += p.k1 - p.k0;
+    return true;
+  }
+};
 
+// ------------------------------------------------------------------------------------------- the kernel
 __global__ void __launch_bounds__(kFusedThreads, 1)
 moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_constant__ CUtensorMap tm_sw13,
                  const __grid_constant__ CUtensorMap tm_w2, const __grid_constant__ CUtensorMap tm_sw2,
@@ -356,47 +519,45 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int G = gridDim.x, cta = blockIdx.x;
   const int T = a.tk.T, E = a.tk.E, k = a.tk.k, H = a.H, I = a.I, ns = a.n_shared;
-  const int NP = a.np, S = a.stages;
-  const uint32_t stage_bytes = kUmmaWBytes + NP * 128;
 
   FusedSmem sm;
   {
     const uint32_t base = (smem_u32(smem_dyn) + 1023u) & ~1023u;
     uint8_t* gen = smem_dyn + (base - smem_u32(smem_dyn));
     sm.stage_base = base;
-    size_t o = (size_t)S * stage_bytes;
+    size_t o = (size_t)a.stage_area;
     sm.bar_base = base + (uint32_t)o;
-    o += (2 * (size_t)S + 12) * 8;
-    sm.tmem_slot = base + (uint32_t)o;
-    o += 16;
-    sm.ring = reinterpret_cast<int4*>(gen + o);
-    o += kSchedSlots * 16;
+    sm.tmem_slot = base + (uint32_t)o + 240;
+    o += 256;
     sm.work = reinterpret_cast<int4*>(gen + o);
     o += (size_t)(E + ns) * 16;
-    sm.n_work = reinterpret_cast<int32_t*>(gen + o);
-    o += 16;
+    sm.cumpass = reinterpret_cast<int32_t*>(gen + o);
+    o += ((size_t)(E + ns + 1) * 4 + 15) / 16 * 16;
+    sm.meta = reinterpret_cast<int32_t*>(gen + o);
+    o += 32;
     sm.tok_of_pos = reinterpret_cast<uint16_t*>(gen + o);
     o += (((size_t)T * k + T) * 2 + 15) / 16 * 16;
     sm.pos_of_pair = reinterpret_cast<uint16_t*>(gen + o);
+    o += ((size_t)T * k * 2 + 15) / 16 * 16;
+    sm.ids8 = gen + o;
+    o += ((size_t)T * k + 15) / 16 * 16;
+    sm.route_scratch = gen + o;
   }
   uint8_t* scratch = smem_dyn + (sm.stage_base - smem_u32(smem_dyn));     // stage area, generic pointer
   auto full_bar = [&](int s) { return sm.bar_base + 8u * s; };
-  auto empty_bar = [&](int s) { return sm.bar_base + 8u * (S + s); };
-  auto tfull_bar = [&](int b) { return sm.bar_base + 8u * (2 * S + b); };
-  auto tempty_bar = [&](int b) { return sm.bar_base + 8u * (2 * S + 2 + b); };
-  auto sfull_bar = [&](int b) { return sm.bar_base + 8u * (2 * S + 4 + b); };
-  auto sempty_bar = [&](int b) { return sm.bar_base + 8u * (2 * S + 8 + b); };
+  auto empty_bar = [&](int s) { return sm.bar_base + 8u * (kMaxStages + s); };
+  auto tfull_bar = [&](int b) { return sm.bar_base + 8u * (2 * kMaxStages + b); };
+  auto tempty_bar = [&](int b) { return sm.bar_base + 8u * (2 * kMaxStages + 2 + b); };
 
   // ------------------------------------------------------------- prologue (overlaps the previous kernel's tail)
   if (tid == 0) {
-    for (int s = 0; s < S; ++s) { mbar_init(full_bar(s), 2); mbar_init(empty_bar(s), 1); }
+    for (int s = 0; s < kMaxStages; ++s) { mbar_init(full_bar(s), 2); mbar_init(empty_bar(s), 1); }
     for (int b = 0; b < 2; ++b) { mbar_init(tfull_bar(b), 1); mbar_init(tempty_bar(b), 4); }
-    for (int b = 0; b < kSchedSlots; ++b) { mbar_init(sfull_bar(b), 1); mbar_init(sempty_bar(b), 6); }
     mbar_fence_init();
     tma_prefetch_desc(&tm_w13);
     tma_prefetch_desc(&tm_w2);
   }
-  const uint32_t tmem_cols = 2 * NP;
+  constexpr uint32_t tmem_cols = 2 * kNPCap;
   if (warp == 6) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(sm.tmem_slot), "r"(tmem_cols) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
@@ -406,16 +567,12 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
   tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(sm.tmem_slot));
+  if (tid == 0) FSTAMP(0);
   pdl_launch_dependents();
   pdl_wait();
+  if (tid == 0) FSTAMP(1);
 
   const uint32_t epoch = __ldcg(a.sync + kSyncGen) + 1u;
-  if (cta == 0 && tid == 0) {
-    // dynamic unit counter: unit `cta` is everyone's first (static), the counter hands out the rest
-    a.sync[kSyncCounter] = (uint32_t)G;
-    __threadfence();
-    flag_release(a.sync + kSyncSchedReady, epoch);
-  }
 
   // ------------------------------------------------------------------------------ G + K: gate and top-k
   if (!a.force_routing) {
@@ -424,9 +581,8 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     for (int tile = cta; tile < n_tiles; tile += G) {
       const int g = tile / n_et, et = tile - g * n_et;
       fused_gate_tile(a, et, g, scratch);
-      __threadfence();
       __syncthreads();
-      if (tid == 0) flag_release(a.sync + kSyncTile + g * 32 + et, epoch);
+      if (tid == 0) flag_release(a.sync + kSyncTile + g * 32 + et, epoch);    // cumulative over the barrier
     }
     for (int g = ((cta - n_tiles % G) + G) % G; g < n_gr; g += G) {       // owner(g) = (n_tiles + g) % G
       if (warp == 0) warp_wait_flags(a.sync + kSyncTile + g * 32, n_et, epoch, lane);
@@ -442,108 +598,109 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
                   a.tk.token_block ? a.tk.token_block[t] : -1, a.tk.L, a.tk.layer, E, id);
         }
       }
-      __threadfence();
       __syncthreads();
       if (tid == 0) flag_release(a.sync + kSyncGroup + g, epoch);
     }
+    if (tid == 0) FSTAMP(2);
     if (warp == 0) warp_wait_flags(a.sync + kSyncGroup, n_gr, epoch, lane);
     __syncthreads();
+    if (tid == 0) FSTAMP(3);
   }
 
   // ------------------------------------------------------------------------------------------ R: routing
-  fused_route(a, sm, scratch, cta == 0);
+  fused_route_a(a, sm, sm.route_scratch, cta == 0);
+  if (tid == 0) FSTAMP(4);
+  if (warp != 4) {
+    // the weights producer (warp 4) is already streaming; everyone else finishes the position maps
+    fused_route_b(a, sm, sm.route_scratch, cta == 0, warp < 4 ? tid : tid - 32, kFusedThreads - 32);
+    asm volatile("bar.sync 2, 224;" ::: "memory");
+  }
 
   // ------------------------------------------------------------------------------------------ F: expert FFN
-  const int n_work = *sm.n_work;
+  const int n_work = sm.meta[0];
+  const int NP = sm.meta[1], S = sm.meta[2], total_pass = sm.meta[3];
+  const uint32_t stage_bytes = kUmmaWBytes + NP * 128;
   const int tilesA = I / 64, tilesB = (H + 127) / 128;
-  const int nA = n_work * tilesA, total_units = nA + n_work * tilesB;
   const int kitA = H / 64, kitB = I / 64;
   uint32_t* hready = a.sync + kSyncHReady;
-  auto decode = [&](int u) {
-    UnitInfo r;
-    if (u < nA) { r.mode = 0; r.ent = u / tilesA; r.rt = u - r.ent * tilesA; }
-    else { const int v = u - nA; r.mode = 1; r.ent = v / tilesB; r.rt = v - r.ent * tilesB; }
-    return r;
-  };
-  // consumer side of the unit ring: lane 0 reads, frees the slot, broadcasts
-  auto next_unit = [&](uint32_t n) {
-    int u = 0;
-    if (lane == 0) {
-      const int slot = n & (kSchedSlots - 1);
-      mbar_wait(sfull_bar(slot), (n / kSchedSlots) & 1);
-      u = sm.ring[slot].x;
-      mbar_arrive(sempty_bar(slot));
-    }
-    return __shfl_sync(0xffffffffu, u, 0);
-  };
+  uint32_t* pready = a.sync + kSyncPartial;
+  (void)n_work;
 
   if (warp == 4) {
-    // ================================================================ scheduler + weights producer (one lane)
+    // ================================================================ weights producer (one lane)
     if (lane == 0) {
       const uint64_t pol = l2_policy_evict_first();
-      { uint32_t spins = 0; while (flag_acquire(a.sync + kSyncSchedReady) != epoch) if (++spins > (1u << 24)) __trap(); }
-      uint32_t it = 0, n = 0;
-      int u = cta;
-      while (true) {
-        const int slot = n & (kSchedSlots - 1);
-        mbar_wait(sempty_bar(slot), ((n / kSchedSlots) & 1) ^ 1);
-        sm.ring[slot] = make_int4(u < total_units ? u : -1, 0, 0, 0);
-        mbar_arrive(sfull_bar(slot));
-        ++n;
-        if (u >= total_units) break;
-        const UnitInfo ui = decode(u);
-        const int4 wk = sm.work[ui.ent];
-        const bool shared = wk.x >= E;
-        const int we = shared ? wk.x - E : wk.x;
-        const int k_iters = ui.mode == 0 ? kitA : kitB;
-        const CUtensorMap* tmw = ui.mode == 0 ? (shared ? &tm_sw13 : &tm_w13) : (shared ? &tm_sw2 : &tm_w2);
-        const int claim_at = k_iters > 6 ? k_iters - 6 : 0;
-        int next = -1;
-        for (int n0 = 0; n0 < wk.w; n0 += NP) {
-          const bool last_pass = n0 + NP >= wk.w;
-          for (int kc = 0; kc < k_iters; ++kc, ++it) {
-            if (last_pass && kc == claim_at) next = (int)atomicAdd(a.sync + kSyncCounter, 1u);
+      FSTAMP(5);
+      uint32_t it = 0;
+      for (int ph = 0; ph < 2; ++ph) {
+        PieceWalker pw;
+        pw.init(ph, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G);
+        Piece p;
+        while (pw.next(p)) {
+          const int4 wk = sm.work[p.ent];
+          const bool shared = wk.x >= E;
+          const int we = shared ? wk.x - E : wk.x;
+          const CUtensorMap* tmw = ph == 0 ? (shared ? &tm_sw13 : &tm_w13) : (shared ? &tm_sw2 : &tm_w2);
+          for (int kc = p.k0; kc < p.k1; ++kc, ++it) {
             const int s = it % S;
             mbar_wait(empty_bar(s), ((it / S) & 1) ^ 1);
             mbar_arrive_expect_tx(full_bar(s), kUmmaWBytes);
             const uint32_t dst = sm.stage_base + s * stage_bytes;
-            if (ui.mode == 0) tma_load_5d(dst, tmw, kc * 64, 0, 0, ui.rt * 4, we, full_bar(s), pol);
-            else tma_load_2d(dst, tmw, kc * 64, we * H + ui.rt * 128, full_bar(s), pol);
+            if (ph == 0) tma_load_5d(dst, tmw, kc * 64, 0, 0, p.rt * 4, we, full_bar(s), pol);
+            else tma_load_2d(dst, tmw, kc * 64, we * H + p.rt * 128, full_bar(s), pol);
           }
         }
-        u = next;
       }
+      FSTAMP(7);
     }
     __syncwarp();
-  } else if (warp == 5) {
-    // ================================================================ activations producer (cp.async gather)
-    uint32_t it = 0, pend = 0;
+  } else if (warp == 5 || warp == 7) {
+    // ================================================================ activations producers (cp.async gather)
+    // two warps, alternating ring stages: the per-stage barrier wait / proxy fence / arrive is what bounds one warp
+    const uint32_t xw = warp == 7 ? 1u : 0u;
+    uint32_t it = 0, pend = 0, last = 0;
+#ifdef ELDR_TRACE
+    unsigned long long stall = 0, nb = 0;
+#endif
     auto drain = [&]() {
       cp_async_wait<0>();
       fence_proxy_async_smem();
       __syncwarp();
       if (lane == 0)
-        for (uint32_t j = 0; j < pend; ++j) mbar_arrive(full_bar((it - pend + j) % S));
+        for (uint32_t j = 0; j < pend; ++j) mbar_arrive(full_bar((last - 2 * (pend - 1 - j)) % S));
       pend = 0;
     };
-    for (uint32_t n = 0;; ++n) {
-      const int u = next_unit(n);
-      if (u < 0) break;
-      const UnitInfo ui = decode(u);
-      const int4 wk = sm.work[ui.ent];
-      const int k_iters = ui.mode == 0 ? kitA : kitB;
-      if (ui.mode == 1) {
-        // every h tile of this expert must have landed; first hand over everything already in flight, or a
-        // unit of THIS CTA that the flags depend on could starve
-        drain();
-        warp_wait_flags(hready + (size_t)ui.ent * tilesA, tilesA, epoch, lane);
-      }
-      const size_t row_bytes = (size_t)(ui.mode == 0 ? H : I) * 2;
-      const uint8_t* src_base = reinterpret_cast<const uint8_t*>(ui.mode == 0 ? a.x : a.hbuf);
-      for (int n0 = 0; n0 < wk.w; n0 += NP) {
-        const int n_here = min(NP, wk.w - n0);
+    for (int ph = 0; ph < 2; ++ph) {
+      PieceWalker pw;
+      pw.init(ph, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G);
+      Piece p;
+      int ready_ent = -1;
+      const size_t row_bytes = (size_t)(ph == 0 ? H : I) * 2;
+      const uint8_t* src_base = reinterpret_cast<const uint8_t*>(ph == 0 ? a.x : a.hbuf);
+      while (pw.next(p)) {
+        const int4 wk = sm.work[p.ent];
+        if (ph == 1 && p.ent != ready_ent) {
+          // every h tile of this expert must have landed.  If not yet: first hand over everything already in
+          // flight (a piece of THIS CTA that the flags depend on could otherwise starve), then wait.
+          const uint32_t* fl = hready + (size_t)sm.cumpass[p.ent] * tilesA;
+          const int nfl = (sm.cumpass[p.ent + 1] - sm.cumpass[p.ent]) * tilesA;
+          if (!warp_test_flags(fl, nfl, epoch, lane)) {
+#ifdef ELDR_TRACE
+            const unsigned long long t0_ = gtime();
+#endif
+            drain();
+            warp_wait_flags(fl, nfl, epoch, lane);
+#ifdef ELDR_TRACE
+            stall += gtime() - t0_; ++nb;
+#endif
+          }
+          ready_ent = p.ent;
+        }
+        const int n0 = p.pass * kNPCap;
+        const int n_here = min(kNPCap, wk.w - n0);
         const int n_pad = (n_here + 15) & ~15;
-        for (int kc = 0; kc < k_iters; ++kc) {
+        for (int kc = p.k0; kc < p.k1; ++kc, ++it) {
+          if ((it & 1u) != xw) continue;
           const int s = it % S;
           if (lane == 0) mbar_wait(empty_bar(s), ((it / S) & 1) ^ 1);
           __syncwarp();
@@ -551,117 +708,174 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
           for (int q = lane; q < n_pad * 8; q += 32) {
             const int r = q >> 3, c = q & 7;
             const int rr = min(r, n_here - 1);                     // padding rows: any valid row (result ignored)
-            const size_t grow = ui.mode == 0 ? (size_t)sm.tok_of_pos[wk.y + n0 + rr] : (size_t)(wk.z + n0 + rr);
+            const size_t grow = ph == 0 ? (size_t)sm.tok_of_pos[wk.y + n0 + rr] : (size_t)(wk.z + n0 + rr);
             cp_async16(dst + r * 128 + ((c ^ (r & 7)) << 4), src_base + grow * row_bytes + (size_t)kc * 128 + c * 16);
           }
           cp_async_commit();
-          ++it;
+          last = it;
           ++pend;
           if (pend > kXLag) {
             cp_async_wait<kXLag>();
             fence_proxy_async_smem();
             __syncwarp();
-            if (lane == 0) mbar_arrive(full_bar((it - pend) % S));
+            if (lane == 0) mbar_arrive(full_bar((last - 2 * (pend - 1)) % S));
             --pend;
           }
         }
       }
     }
     drain();
+#ifdef ELDR_TRACE
+    if (lane == 0 && xw == 0) { FVALUE(12, stall); FVALUE(13, nb); }
+#endif
   } else if (warp == 6) {
     // ================================================================ MMA issuer
-    uint32_t it = 0, pass = 0;
-    for (uint32_t n = 0;; ++n) {
-      const int u = next_unit(n);
-      if (u < 0) break;
-      const UnitInfo ui = decode(u);
-      const int4 wk = sm.work[ui.ent];
-      const int k_iters = ui.mode == 0 ? kitA : kitB;
-      for (int n0 = 0; n0 < wk.w; n0 += NP, ++pass) {
-        const int n_pad = (min(NP, wk.w - n0) + 15) & ~15;
+    uint32_t it = 0, piece_no = 0;
+    for (int ph = 0; ph < 2; ++ph) {
+      PieceWalker pw;
+      pw.init(ph, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G);
+      Piece p;
+      while (pw.next(p)) {
+        const int4 wk = sm.work[p.ent];
+        const int n_pad = (min(kNPCap, wk.w - p.pass * kNPCap) + 15) & ~15;
         const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n_pad >> 3) << 17) | (8u << 24);
-        const int buf = pass & 1;
-        mbar_wait(tempty_bar(buf), ((pass >> 1) & 1) ^ 1);
+        const int buf = piece_no & 1;
+        mbar_wait(tempty_bar(buf), ((piece_no >> 1) & 1) ^ 1);
         tc_fence_after();
-        const uint32_t d_tmem = tmem_base + buf * NP;
-        for (int kc = 0; kc < k_iters; ++kc, ++it) {
+        const uint32_t d_tmem = tmem_base + buf * kNPCap;
+        for (int kc = p.k0; kc < p.k1; ++kc, ++it) {
           const int s = it % S;
           mbar_wait(full_bar(s), (it / S) & 1);
           tc_fence_after();
           if (lane == 0) {
+            if (it == 0) FSTAMP(6);
             const uint32_t sa = sm.stage_base + s * stage_bytes;
             const uint64_t da = umma_desc_sw128(sa), db = umma_desc_sw128(sa + kUmmaWBytes);
 #pragma unroll
             for (int kk = 0; kk < 4; ++kk)
-              umma_bf16(d_tmem, da + 2 * kk, db + 2 * kk, idesc, (kc | kk) ? 1u : 0u);
+              umma_bf16(d_tmem, da + 2 * kk, db + 2 * kk, idesc, (kc > p.k0 || kk > 0) ? 1u : 0u);
             umma_commit(empty_bar(s));
-            if (kc == k_iters - 1) umma_commit(tfull_bar(buf));
+            if (kc == p.k1 - 1) umma_commit(tfull_bar(buf));
           }
           __syncwarp();
         }
+        ++piece_no;
       }
     }
   } else if (warp < 4) {
     // ================================================================ epilogue (TMEM lane quarter = warp)
     const int qtr = warp;
-    uint32_t pass = 0;
-    for (uint32_t n = 0;; ++n) {
-      const int u = next_unit(n);
-      if (u < 0) break;
-      const UnitInfo ui = decode(u);
-      const int4 wk = sm.work[ui.ent];
-      for (int n0 = 0; n0 < wk.w; n0 += NP, ++pass) {
-        const int n_here = min(NP, wk.w - n0);
-        const int buf = pass & 1;
-        mbar_wait(tfull_bar(buf), (pass >> 1) & 1);
+    uint32_t piece_no = 0;
+    for (int ph = 0; ph < 2; ++ph) {
+      PieceWalker pw;
+      pw.init(ph, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G);
+      const long long P = (long long)total_pass * pw.tpe * pw.kit;
+      Piece p;
+      while (pw.next(p)) {
+        const int4 wk = sm.work[p.ent];
+        const int n0 = p.pass * kNPCap;
+        const int n_here = min(kNPCap, wk.w - n0);
+        const int buf = piece_no & 1;
+        mbar_wait(tfull_bar(buf), (piece_no >> 1) & 1);
         tc_fence_after();
-        const uint32_t t_addr = tmem_base + buf * NP + ((uint32_t)(qtr * 32) << 16);
-        for (int c0 = 0; c0 < n_here; c0 += 16) {
-          float v[16];
-          tmem_ld16(t_addr + c0, v);
-          if (ui.mode == 0) {
-            // lanes 0-15: g for i = rt*64 + 16*qtr + lane; lanes 16-31: u for the same i
-            const bool lo = lane < 16;
-            const int i = ui.rt * 64 + 16 * qtr + (lane & 15);
+        const uint32_t t_addr = tmem_base + buf * kNPCap + ((uint32_t)(qtr * 32) << 16);
+        const int row = 32 * qtr + lane;                        // TMEM lane = row of the 128-row tile
+        if (p.k0 > 0) {
+          // ---- not the head of this tile: park the raw accumulators for the head owner
+          float* dstp = a.partial + ((size_t)(ph * G + cta) * 128 + row) * kNPCap;
+          for (int c0 = 0; c0 < n_here; c0 += 16) {
+            float v[16];
+            tmem_ld16(t_addr + c0, v);
 #pragma unroll
-            for (int kk = 0; kk < 8; ++kk) {
-              const float send = lo ? v[8 + kk] : v[kk];
-              const float recv = __shfl_xor_sync(0xffffffffu, send, 16);
-              const float gv = lo ? v[kk] : recv;
-              const float uv = lo ? recv : v[8 + kk];
-              const int tok = n0 + c0 + (lo ? kk : 8 + kk);
-              if (tok < wk.w) a.hbuf[(size_t)(wk.z + tok) * I + i] = f32_to_bf16_rn(silu_f(gv) * uv);
+            for (int q = 0; q < 4; ++q)
+              *reinterpret_cast<float4*>(dstp + c0 + 4 * q) = make_float4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
+          }
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(tempty_bar(buf));
+          __threadfence();
+          asm volatile("bar.sync 1, 128;" ::: "memory");
+          if (tid == 0) flag_release(pready + ph * 256 + cta, epoch);
+        } else {
+          // ---- head (or only) owner: add the parked partials of the following CTAs in ascending order
+          int n_partner = 0;
+          if (p.k1 < pw.kit) {
+            const long long tile_end = ((long long)p.tile + 1) * pw.kit;
+            long long covered = (long long)p.tile * pw.kit + p.k1;
+            int j = cta + 1;
+            while (covered < tile_end && j < G) {
+              const long long hj = P * (j + 1) / G;
+              if (hj > covered) {                              // CTA j owns a non-empty piece of this tile
+                if (lane == 0) {
+                  uint32_t spins = 0;
+                  while (flag_acquire(pready + ph * 256 + j) != epoch) { __nanosleep(40); if (++spins > (1u << 24)) __trap(); }
+                }
+                covered = min(hj, tile_end);
+                n_partner = j - cta;
+              }
+              ++j;
             }
-          } else {
-            const int r = ui.rt * 128 + 32 * qtr + lane;
-            if (r < H) {
+            __syncwarp();
+          }
+          for (int c0 = 0; c0 < n_here; c0 += 16) {
+            float v[16];
+            tmem_ld16(t_addr + c0, v);
+            for (int j = 1; j <= n_partner; ++j) {
+              // CTAs with an empty range parked nothing; their slot is skipped by the same test as above
+              const long long lj = P * (cta + j) / G, hj = P * (cta + j + 1) / G;
+              if (hj <= lj) continue;
+              const float* srcp = a.partial + ((size_t)(ph * G + cta + j) * 128 + row) * kNPCap + c0;
 #pragma unroll
-              for (int kk = 0; kk < 16; ++kk) {
-                const int tok = n0 + c0 + kk;
-                if (tok < wk.w) a.ybuf[(size_t)(wk.z + tok) * H + r] = v[kk];
+              for (int q = 0; q < 4; ++q) {
+                const float4 pv = __ldcg(reinterpret_cast<const float4*>(srcp + 4 * q));
+                v[4 * q] += pv.x; v[4 * q + 1] += pv.y; v[4 * q + 2] += pv.z; v[4 * q + 3] += pv.w;
+              }
+            }
+            if (ph == 0) {
+              // lanes 0-15: g for i = rt*64 + 16*qtr + lane; lanes 16-31: u for the same i
+              const bool lo = lane < 16;
+              const int i = p.rt * 64 + 16 * qtr + (lane & 15);
+#pragma unroll
+              for (int kk = 0; kk < 8; ++kk) {
+                const float send = lo ? v[8 + kk] : v[kk];
+                const float recv = __shfl_xor_sync(0xffffffffu, send, 16);
+                const float gv = lo ? v[kk] : recv;
+                const float uv = lo ? recv : v[8 + kk];
+                const int tok = n0 + c0 + (lo ? kk : 8 + kk);
+                if (tok < wk.w) a.hbuf[(size_t)(wk.z + tok) * I + i] = f32_to_bf16_rn(silu_f(gv) * uv);
+              }
+            } else {
+              const int r = p.rt * 128 + row;
+              if (r < H) {
+#pragma unroll
+                for (int kk = 0; kk < 16; ++kk) {
+                  const int tok = n0 + c0 + kk;
+                  if (tok < wk.w) a.ybuf[(size_t)(wk.z + tok) * H + r] = v[kk];
+                }
               }
             }
           }
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(tempty_bar(buf));
+          if (ph == 0) {
+            // publish "h tile written": the four epilogue warps meet, one thread releases (cumulative)
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+            if (tid == 0) flag_release(hready + p.tile, epoch);
+          }
         }
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(tempty_bar(buf));
-      }
-      if (ui.mode == 0) {
-        // publish "h tile (ent, rt) written": every writer fences, the four epilogue warps meet, one releases
-        __threadfence();
-        asm volatile("bar.sync 1, 128;" ::: "memory");
-        if (tid == 0) flag_release(hready + (size_t)ui.ent * tilesA + ui.rt, epoch);
+        ++piece_no;
       }
     }
   }
 
   // ------------------------------------------------------------------------------ grid barrier, then C: combine
-  __threadfence();
+  if (tid == 0) FSTAMP(8);
   __syncthreads();
   if (tid == 0) flag_release(a.sync + kSyncDone + cta, epoch);
   if (warp == 0) warp_wait_flags(a.sync + kSyncDone, G, epoch, lane);
   __syncthreads();
+  if (tid == 0) FSTAMP(9);
   {
     const int q_per_row = H >> 2;
     for (int idx = cta * kFusedThreads + tid; idx < T * q_per_row; idx += G * kFusedThreads) {
@@ -692,6 +906,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
       *reinterpret_cast<uint2*>(a.out + (size_t)t * H + (size_t)c4 * 4) = o;
     }
   }
+  if (tid == 0) FSTAMP(10);
   if (cta == 0 && tid == 0) a.sync[kSyncGen] = epoch;      // every CTA read gen before its done flag
 
   tc_fence_before();
