@@ -650,6 +650,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
             else tma_load_2d(dst, tmw, kc * 64, we * H + p.rt * 128, full_bar(s), pol);
           }
         }
+        if (ph == 0) FSTAMP(11);
       }
       FSTAMP(7);
     }
@@ -726,7 +727,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     }
     drain();
 #ifdef ELDR_TRACE
-    if (lane == 0 && xw == 0) { FVALUE(12, stall); FVALUE(13, nb); }
+    if (lane == 0 && xw == 0) { FVALUE(12, stall); }
 #endif
   } else if (warp == 6) {
     // ================================================================ MMA issuer
@@ -761,6 +762,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
         }
         ++piece_no;
       }
+      if (ph == 0 && lane == 0) FSTAMP(13);
     }
   } else if (warp < 4) {
     // ================================================================ epilogue (TMEM lane quarter = warp)
