@@ -245,6 +245,12 @@ void eldr_debug_read_trace(unsigned long long* h) {
   cudaDeviceSynchronize();
   cudaMemcpyFromSymbol(h, eldr::g_trace, sizeof(unsigned long long) * 4096 * 16);
 }
+void eldr_debug_clear_trace(void) {
+  cudaDeviceSynchronize();
+  void* p = nullptr;
+  cudaGetSymbolAddress(&p, eldr::g_trace);
+  cudaMemset(p, 0, sizeof(unsigned long long) * 4096 * 16);
+}
 #endif
 
 const char* eldr_status_string(int32_t st) {

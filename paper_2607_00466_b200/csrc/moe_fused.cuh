@@ -48,14 +48,14 @@ constexpr int kSyncGen = 0;
 constexpr int kSyncDone = 32;                   // [256]     per CTA "all my pieces are finished"
 constexpr int kSyncGroup = kSyncDone + 256;     // [32]      per token group "ids/weights written"
 constexpr int kSyncTile = kSyncGroup + 32;      // [32][32]  gate logit tile written
-constexpr int kSyncPartial = kSyncTile + 1024;  // [2][256]  per (phase, CTA) "partial accumulators parked"
-constexpr int kSyncHReady = kSyncPartial + 512; // [(E+ns)*2*tilesA] per phase-A tile "h tile written"
+constexpr int kSyncPartial = kSyncTile + 1024;  // [4][256]  per (sub-phase, CTA) "partial accumulators parked"
+constexpr int kSyncHReady = kSyncPartial + 1024; // [(E+ns)*2*tilesA] per phase-A tile "h tile written"
 
 __host__ __device__ inline size_t fused_sync_words(int E, int ns, int I) {
   return (size_t)kSyncHReady + (size_t)(E + ns) * 2 * ((I + 63) / 64);
 }
 __host__ __device__ inline size_t fused_partial_bytes(int n_cta) {
-  return (size_t)2 * n_cta * 128 * kNPCap * 4;
+  return (size_t)4 * n_cta * 128 * kNPCap * 4;
 }
 
 struct FusedArgs {
@@ -73,7 +73,7 @@ struct FusedArgs {
   int32_t* active;
   int32_t* n_active;
   uint32_t* sync;
-  float* partial;              // [2][gridDim.x][128][kNPCap] fp32 scratch of the stream-K fix-up
+  float* partial;              // [4][gridDim.x][128][kNPCap] fp32 scratch of the stream-K fix-up
   uint16_t* hbuf;              // [T*(k+ns), I] bf16
   float* ybuf;                 // [T*(k+ns), H] fp32
   uint16_t* out;               // [T,H] bf16
@@ -167,7 +167,6 @@ __device__ __forceinline__ void fused_gate_tile(const FusedArgs& a, int et, int 
     }
   }
   __syncthreads();
-  if (tid == 0) FSTAMP(14);
   float acc0[4], acc1[4];
 #pragma unroll
   for (int t = 0; t < 4; ++t) { acc0[t] = 0.f; acc1[t] = 0.f; }
@@ -209,7 +208,6 @@ __device__ __forceinline__ void fused_gate_tile(const FusedArgs& a, int et, int 
     }
     acc0[t] = s0; acc1[t] = s1;
   }
-  if (tid == 0) FSTAMP(15);
   if (lane == 0) {
     float* z = const_cast<float*>(a.tk.z);
     const float b0 = (a.gate_bias && e0 < E) ? a.gate_bias[e0] : 0.f;
@@ -480,16 +478,34 @@ __device__ __forceinline__ void fused_route_b(const FusedArgs& a, const FusedSme
 struct Piece {
   int tile, k0, k1, ent, pass, rt;
 };
+// Where the (entry, pass) list is cut in two.  Halving only pays when each SM's stage range still spans several
+// tiles per sub-phase (otherwise every tile is split over 2-3 SMs and the fix-up chain costs more than the
+// hand-over it hides); measured on B200 it gave nothing at |U| = 64..128 and lost 8 us at |U| = 16, so the cut is
+// at the end: sub-phases 1 and 3 are empty.
+__device__ __forceinline__ int split_mid(int total_pass, int tilesA, int kitA, int G) {
+  (void)tilesA; (void)kitA; (void)G;
+  return total_pass;
+}
 struct PieceWalker {
   int tpe, kit;          // row tiles per (entry, pass); k-chunks per tile
   long long g, hi;       // current / end stage
   int ent;               // cursor into cumpass
   const int32_t* cumpass;
-  __device__ __forceinline__ void init(int ph, int tilesA, int tilesB, int kitA, int kitB, int total_pass,
+  int tile0;             // first tile of this sub-phase
+  // Sub-phase sp: 0 = w1/w3 of the first half of the (entry, pass) list, 1 = w1/w3 of the second half,
+  // 2 = w2 of the first half, 3 = w2 of the second half.  Each sub-phase is cut into gridDim.x equal stage ranges.
+  // Running them in this order puts one whole sub-phase of streaming between the production of an expert's h
+  // and its consumption, which hides the release -> poll -> load chain of the hand-over.
+  __device__ __forceinline__ void init(int sp, int tilesA, int tilesB, int kitA, int kitB, int total_pass,
                                        const int32_t* cp, int cta, int G) {
+    const int ph = sp >> 1;
     tpe = ph == 0 ? tilesA : tilesB;
     kit = ph == 0 ? kitA : kitB;
-    const long long P = (long long)total_pass * tpe * kit;
+    const int mid = split_mid(total_pass, tilesA, kitA, G);
+    const int cp_lo = (sp & 1) ? mid : 0;
+    const int cp_hi = (sp & 1) ? total_pass : mid;
+    tile0 = cp_lo * tpe;
+    const long long P = (long long)(cp_hi - cp_lo) * tpe * kit;
     g = P * cta / G;
     hi = P * (cta + 1) / G;
     ent = 0;
@@ -497,8 +513,9 @@ struct PieceWalker {
   }
   __device__ __forceinline__ bool next(Piece& p) {
     if (g >= hi) return false;
-    p.tile = (int)(g / kit);
-    p.k0 = (int)(g - (long long)p.tile * kit);
+    const int lt = (int)(g / kit);                 // tile index inside the sub-phase
+    p.tile = tile0 + lt;
+    p.k0 = (int)(g - (long long)lt * kit);
     p.k1 = (int)min((long long)kit, p.k0 + (hi - g));
     const int cpi = p.tile / tpe;
     p.rt = p.tile - cpi * tpe;
@@ -632,9 +649,10 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
       const uint64_t pol = l2_policy_evict_first();
       FSTAMP(5);
       uint32_t it = 0;
-      for (int ph = 0; ph < 2; ++ph) {
+      for (int sp = 0; sp < 4; ++sp) {
+      const int ph = sp >> 1;
         PieceWalker pw;
-        pw.init(ph, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G);
+        pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G);
         Piece p;
         while (pw.next(p)) {
           const int4 wk = sm.work[p.ent];
@@ -650,7 +668,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
             else tma_load_2d(dst, tmw, kc * 64, we * H + p.rt * 128, full_bar(s), pol);
           }
         }
-        if (ph == 0) FSTAMP(11);
+        if (sp == 1) FSTAMP(11);
       }
       FSTAMP(7);
     }
@@ -671,9 +689,10 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
         for (uint32_t j = 0; j < pend; ++j) mbar_arrive(full_bar((last - 2 * (pend - 1 - j)) % S));
       pend = 0;
     };
-    for (int ph = 0; ph < 2; ++ph) {
+    for (int sp = 0; sp < 4; ++sp) {
+      const int ph = sp >> 1;
       PieceWalker pw;
-      pw.init(ph, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G);
+      pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G);
       Piece p;
       int ready_ent = -1;
       const size_t row_bytes = (size_t)(ph == 0 ? H : I) * 2;
@@ -696,6 +715,9 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
 #endif
           }
           ready_ent = p.ent;
+#ifdef ELDR_TRACE
+          if (lane == 0 && xw == 0 && g_trace[(blockIdx.x & 4095) * 16 + 14] == 0) FSTAMP(14);
+#endif
         }
         const int n0 = p.pass * kNPCap;
         const int n_here = min(kNPCap, wk.w - n0);
@@ -732,9 +754,10 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
   } else if (warp == 6) {
     // ================================================================ MMA issuer
     uint32_t it = 0, piece_no = 0;
-    for (int ph = 0; ph < 2; ++ph) {
+    for (int sp = 0; sp < 4; ++sp) {
+      const int ph = sp >> 1;
       PieceWalker pw;
-      pw.init(ph, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G);
+      pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G);
       Piece p;
       while (pw.next(p)) {
         const int4 wk = sm.work[p.ent];
@@ -762,29 +785,66 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
         }
         ++piece_no;
       }
-      if (ph == 0 && lane == 0) FSTAMP(13);
+      if (sp == 1 && lane == 0) FSTAMP(13);
     }
   } else if (warp < 4) {
     // ================================================================ epilogue (TMEM lane quarter = warp)
     const int qtr = warp;
     uint32_t piece_no = 0;
-    for (int ph = 0; ph < 2; ++ph) {
+    for (int sp = 0; sp < 4; ++sp) {
+      const int ph = sp >> 1;
       PieceWalker pw;
-      pw.init(ph, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G);
-      const long long P = (long long)total_pass * pw.tpe * pw.kit;
+      pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G);
+      const int mid_ = split_mid(total_pass, tilesA, kitA, G);
+      const long long P = (long long)((sp & 1) ? total_pass - mid_ : mid_) * pw.tpe * pw.kit;
       Piece p;
       while (pw.next(p)) {
         const int4 wk = sm.work[p.ent];
         const int n0 = p.pass * kNPCap;
         const int n_here = min(kNPCap, wk.w - n0);
         const int buf = piece_no & 1;
+        const int row = 32 * qtr + lane;                        // TMEM lane = row of the 128-row tile
+        // Head piece of a split tile: the other pieces were parked long ago (their owners reach the tile first).
+        // Find them, wait for their flags and request the first chunk of the first partner BEFORE waiting for our
+        // own accumulator: under a saturated memory system every dependent L2 round trip costs more than a microsecond.
+        int n_partner = 0;
+        float4 pf0[4], pf1[4];                                  // two chunks of the first partner in flight
+        bool pf_valid = false;
+        if (p.k0 == 0 && p.k1 < pw.kit) {
+          const long long tile_end = ((long long)(p.tile - pw.tile0) + 1) * pw.kit;
+          long long covered = (long long)(p.tile - pw.tile0) * pw.kit + p.k1;
+          int j = cta + 1;
+          while (covered < tile_end && j < G) {
+            const long long hj = P * (j + 1) / G;
+            if (hj > covered) {                              // CTA j owns a non-empty piece of this tile
+              if (lane == 0) {
+                uint32_t spins = 0;
+                while (flag_acquire(pready + sp * 256 + j) != epoch) { __nanosleep(40); if (++spins > (1u << 24)) __trap(); }
+              }
+              covered = min(hj, tile_end);
+              n_partner = j - cta;
+            }
+            ++j;
+          }
+          __syncwarp();
+          pf_valid = n_partner >= 1 && (P * (cta + 2) / G > P * (cta + 1) / G);
+        }
+        const float* pf_src = a.partial + ((size_t)(sp * G + cta + 1) * 128 + row) * kNPCap;
+        auto pf_load = [&](float4 (&dst)[4], int c0) {
+          if (pf_valid && c0 < n_here) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) dst[q] = __ldcg(reinterpret_cast<const float4*>(pf_src + c0 + 4 * q));
+          }
+        };
+        pf_load(pf0, 0);
+        pf_load(pf1, 16);
         mbar_wait(tfull_bar(buf), (piece_no >> 1) & 1);
         tc_fence_after();
+        if (tid == 0 && ph == 0) FSTAMP(2);
         const uint32_t t_addr = tmem_base + buf * kNPCap + ((uint32_t)(qtr * 32) << 16);
-        const int row = 32 * qtr + lane;                        // TMEM lane = row of the 128-row tile
         if (p.k0 > 0) {
           // ---- not the head of this tile: park the raw accumulators for the head owner
-          float* dstp = a.partial + ((size_t)(ph * G + cta) * 128 + row) * kNPCap;
+          float* dstp = a.partial + ((size_t)(sp * G + cta) * 128 + row) * kNPCap;
           for (int c0 = 0; c0 < n_here; c0 += 16) {
             float v[16];
             tmem_ld16(t_addr + c0, v);
@@ -797,36 +857,24 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
           if (lane == 0) mbar_arrive(tempty_bar(buf));
           __threadfence();
           asm volatile("bar.sync 1, 128;" ::: "memory");
-          if (tid == 0) flag_release(pready + ph * 256 + cta, epoch);
+          if (tid == 0) flag_release(pready + sp * 256 + cta, epoch);
         } else {
           // ---- head (or only) owner: add the parked partials of the following CTAs in ascending order
-          int n_partner = 0;
-          if (p.k1 < pw.kit) {
-            const long long tile_end = ((long long)p.tile + 1) * pw.kit;
-            long long covered = (long long)p.tile * pw.kit + p.k1;
-            int j = cta + 1;
-            while (covered < tile_end && j < G) {
-              const long long hj = P * (j + 1) / G;
-              if (hj > covered) {                              // CTA j owns a non-empty piece of this tile
-                if (lane == 0) {
-                  uint32_t spins = 0;
-                  while (flag_acquire(pready + ph * 256 + j) != epoch) { __nanosleep(40); if (++spins > (1u << 24)) __trap(); }
-                }
-                covered = min(hj, tile_end);
-                n_partner = j - cta;
-              }
-              ++j;
-            }
-            __syncwarp();
-          }
-          for (int c0 = 0; c0 < n_here; c0 += 16) {
+          auto chunk = [&](int c0, float4 (&pfx)[4]) {
             float v[16];
             tmem_ld16(t_addr + c0, v);
-            for (int j = 1; j <= n_partner; ++j) {
+            if (pf_valid) {
+#pragma unroll
+              for (int q = 0; q < 4; ++q) {
+                v[4 * q] += pfx[q].x; v[4 * q + 1] += pfx[q].y; v[4 * q + 2] += pfx[q].z; v[4 * q + 3] += pfx[q].w;
+              }
+              pf_load(pfx, c0 + 32);                           // refill this buffer two chunks ahead
+            }
+            for (int j = pf_valid ? 2 : 1; j <= n_partner; ++j) {
               // CTAs with an empty range parked nothing; their slot is skipped by the same test as above
               const long long lj = P * (cta + j) / G, hj = P * (cta + j + 1) / G;
               if (hj <= lj) continue;
-              const float* srcp = a.partial + ((size_t)(ph * G + cta + j) * 128 + row) * kNPCap + c0;
+              const float* srcp = a.partial + ((size_t)(sp * G + cta + j) * 128 + row) * kNPCap + c0;
 #pragma unroll
               for (int q = 0; q < 4; ++q) {
                 const float4 pv = __ldcg(reinterpret_cast<const float4*>(srcp + 4 * q));
@@ -844,7 +892,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
                 const float gv = lo ? v[kk] : recv;
                 const float uv = lo ? recv : v[8 + kk];
                 const int tok = n0 + c0 + (lo ? kk : 8 + kk);
-                if (tok < wk.w) a.hbuf[(size_t)(wk.z + tok) * I + i] = f32_to_bf16_rn(silu_f(gv) * uv);
+                if (tok < wk.w) a.hbuf[(size_t)(wk.z + tok) * I + i] = f32_to_bf16_rn(__fdividef(gv, 1.0f + __expf(-gv)) * uv);
               }
             } else {
               const int r = p.rt * 128 + row;
@@ -856,14 +904,20 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
                 }
               }
             }
+          };
+          for (int c0 = 0; c0 < n_here; c0 += 32) {
+            chunk(c0, pf0);
+            if (tid == 0 && ph == 0 && c0 == 0) FSTAMP(3);
+            if (c0 + 16 < n_here) chunk(c0 + 16, pf1);
           }
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive(tempty_bar(buf));
+          if (tid == 0 && ph == 0) FSTAMP(4);
           if (ph == 0) {
             // publish "h tile written": the four epilogue warps meet, one thread releases (cumulative)
             asm volatile("bar.sync 1, 128;" ::: "memory");
-            if (tid == 0) flag_release(hready + p.tile, epoch);
+            if (tid == 0) { flag_release(hready + p.tile, epoch); FSTAMP(15); }
           }
         }
         ++piece_no;
