@@ -161,6 +161,8 @@ int32_t eldr_moe_workspace_layout(const eldr_moe_shape_t* shape, int32_t T, eldr
 #define ELDR_OPT_STEP_PATH 2  /* ELDR_STEP_FUSED (default): the whole step in ONE persistent launch (T <= 256,
                                  H,I % 64 == 0); ELDR_STEP_STAGED: one launch per stage (gate+route, gather, w1/w3, w2,
                                  combine), also the path for shapes the fused kernel does not take */
+#define ELDR_OPT_RING_KB  3   /* fused step: cap on the shared-memory stage ring in KiB per SM (bytes in flight);
+                                 32..208; default 208 (all of it) */
 #define ELDR_STEP_STAGED  0
 #define ELDR_STEP_FUSED   1
 #define ELDR_FFN_MMA_SYNC 0

@@ -22,6 +22,7 @@ using namespace eldr;
 int g_ffn_path = ELDR_FFN_TCGEN05;   // process-wide tuning knobs (eldr_moe_set_option)
 int g_pdl = 1;
 int g_step_path = ELDR_STEP_FUSED;
+int g_ring_kb = 208;
 
 thread_local char g_err[256] = "";
 thread_local int g_launches = 0;
@@ -279,6 +280,10 @@ int32_t eldr_moe_set_option(int32_t key, int32_t value) {
     g_step_path = value;
     return ELDR_OK;
   }
+  if (key == ELDR_OPT_RING_KB && value >= 32 && value <= 208) {
+    g_ring_kb = value;
+    return ELDR_OK;
+  }
   return ELDR_ERR_INVALID_ARG;
 }
 
@@ -403,6 +408,7 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
     const size_t min_area = (size_t)3 * (kUmmaWBytes + kNPCap * 128) > (size_t)kGateTok * H * 2
                                 ? (size_t)3 * (kUmmaWBytes + kNPCap * 128) : (size_t)kGateTok * H * 2;
     fa.stage_area = fixed < smem_max ? (int)((smem_max - fixed) / 1024 * 1024) : 0;
+    fa.ring_bytes = g_ring_kb * 1024;
     const size_t smem = fixed + fa.stage_area;
     if ((size_t)fa.stage_area >= min_area) {
       CUtensorMap tm_w13, tm_sw13, tm_w2, tm_sw2;
@@ -414,6 +420,9 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
       } else {
         tm_sw13 = tm_w13;
         tm_sw2 = tm_w2;
+#ifdef ELDR_EXP_W13_2D
+        if (!make_tmap(&tm_sw13, w13, (uint64_t)E * 2 * I, H, 128)) return ELDR_ERR_CUDA;
+#endif
       }
       static bool fused_attr_set = false;
       if (!fused_attr_set) {

@@ -78,6 +78,7 @@ struct FusedArgs {
   float* ybuf;                 // [T*(k+ns), H] fp32
   uint16_t* out;               // [T,H] bf16
   int stage_area;              // bytes of shared memory cut into ring stages (multiple of 1024; set by the host)
+  int ring_bytes;              // cap on the bytes the ring keeps in flight (<= stage_area)
 };
 
 #ifdef ELDR_TRACE
@@ -88,7 +89,11 @@ __device__ __forceinline__ unsigned long long gtime() {
 }
 #define FSTAMP(id) do { g_trace[(blockIdx.x & 4095) * 16 + (id)] = gtime(); } while (0)
 #define FVALUE(id, v) do { g_trace[(blockIdx.x & 4095) * 16 + (id)] = (unsigned long long)(v); } while (0)
+#define FVALUE2(id, v) do { g_trace[((blockIdx.x + 2048) & 4095) * 16 + (id)] = (unsigned long long)(v); } while (0)
+#define FTIMED(acc, stmt) do { const long long c0_ = clock64(); stmt; acc += clock64() - c0_; } while (0)
 #else
+#define FVALUE2(id, v) do {} while (0)
+#define FTIMED(acc, stmt) do { stmt; } while (0)
 #define FSTAMP(id) do {} while (0)
 #define FVALUE(id, v) do {} while (0)
 #endif
@@ -443,7 +448,7 @@ __device__ __forceinline__ void fused_route_a(const FusedArgs& a, const FusedSme
       s_off[E] = total;
       sm.meta[0] = n_work;
       sm.meta[1] = np;
-      sm.meta[2] = min(kMaxStages, a.stage_area / (kUmmaWBytes + np * 128));
+      sm.meta[2] = min(kMaxStages, max(min(a.stage_area, a.ring_bytes), 2 * (kXLag + 1) * (kUmmaWBytes + np * 128)) / (kUmmaWBytes + np * 128));  // >= 2*(kXLag+1): the two activation producers hold that many stages before arriving
       if (is_cta0) { a.off[E] = total; *a.n_active = n_act; *a.n_work = n_work; }
     }
     if (lane == 31) sm.meta[3] = pinc;
@@ -649,6 +654,8 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
       const uint64_t pol = l2_policy_evict_first();
       FSTAMP(5);
       uint32_t it = 0;
+      long long w_wait[2] = {0, 0}, w_iss[2] = {0, 0};
+      (void)w_wait; (void)w_iss;
       for (int sp = 0; sp < 4; ++sp) {
       const int ph = sp >> 1;
         PieceWalker pw;
@@ -661,16 +668,28 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
           const CUtensorMap* tmw = ph == 0 ? (shared ? &tm_sw13 : &tm_w13) : (shared ? &tm_sw2 : &tm_w2);
           for (int kc = p.k0; kc < p.k1; ++kc, ++it) {
             const int s = it % S;
-            mbar_wait(empty_bar(s), ((it / S) & 1) ^ 1);
+            FTIMED(w_wait[ph], mbar_wait(empty_bar(s), ((it / S) & 1) ^ 1));
+#ifdef ELDR_TRACE
+            const long long cw_ = clock64();
+#endif
             mbar_arrive_expect_tx(full_bar(s), kUmmaWBytes);
             const uint32_t dst = sm.stage_base + s * stage_bytes;
-            if (ph == 0) tma_load_5d(dst, tmw, kc * 64, 0, 0, p.rt * 4, we, full_bar(s), pol);
+            if (ph == 0)
+#ifdef ELDR_EXP_W13_2D
+              tma_load_2d(dst, &tm_sw13, kc * 64, we * 2 * I + p.rt * 128, full_bar(s), pol);
+            else if (false)
+#endif
+              tma_load_5d(dst, tmw, kc * 64, 0, 0, p.rt * 4, we, full_bar(s), pol);
             else tma_load_2d(dst, tmw, kc * 64, we * H + p.rt * 128, full_bar(s), pol);
+#ifdef ELDR_TRACE
+            w_iss[ph] += clock64() - cw_;
+#endif
           }
         }
         if (sp == 1) FSTAMP(11);
       }
       FSTAMP(7);
+      FVALUE2(0, w_wait[0]); FVALUE2(1, w_wait[1]); FVALUE2(10, w_iss[0]); FVALUE2(11, w_iss[1]);
     }
     __syncwarp();
   } else if (warp == 5 || warp == 7) {
@@ -728,6 +747,9 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
           if (lane == 0) mbar_wait(empty_bar(s), ((it / S) & 1) ^ 1);
           __syncwarp();
           const uint32_t dst = sm.stage_base + s * stage_bytes + kUmmaWBytes;
+#ifdef ELDR_EXP_NOX
+          if (false)
+#endif
           for (int q = lane; q < n_pad * 8; q += 32) {
             const int r = q >> 3, c = q & 7;
             const int rr = min(r, n_here - 1);                     // padding rows: any valid row (result ignored)
@@ -753,35 +775,40 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
 #endif
   } else if (warp == 6) {
     // ================================================================ MMA issuer
-    uint32_t it = 0, piece_no = 0;
+    // The warp stays converged; every operand of the issue path is warp-uniform (redux / kernel parameters) and
+    // the tcgen05 instructions are predicated on the elected lane inside the asm, so one stage costs four
+    // back-to-back UTCHMMA + one UTCBAR instead of five ELECT/R2UR waterfalls.  Ring slot and parity are carried
+    // incrementally (no division by the run-time ring depth).
+    const uint32_t leader = elect_one();
+    const uint32_t uS = warp_uniform((uint32_t)S), ustage = warp_uniform(stage_bytes);
+    const uint32_t ubase = warp_uniform(sm.stage_base), ubar = warp_uniform(sm.bar_base);
+    const uint32_t utmem = warp_uniform(tmem_base);
+    uint32_t s = 0, par = 0, piece_no = 0;
+    bool first = true;
     for (int sp = 0; sp < 4; ++sp) {
-      const int ph = sp >> 1;
       PieceWalker pw;
       pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G);
       Piece p;
       while (pw.next(p)) {
         const int4 wk = sm.work[p.ent];
-        const int n_pad = (min(kNPCap, wk.w - p.pass * kNPCap) + 15) & ~15;
-        const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n_pad >> 3) << 17) | (8u << 24);
-        const int buf = piece_no & 1;
-        mbar_wait(tempty_bar(buf), ((piece_no >> 1) & 1) ^ 1);
+        const uint32_t n_pad = warp_uniform((uint32_t)((min(kNPCap, wk.w - p.pass * kNPCap) + 15) & ~15));
+        const uint32_t nk = warp_uniform((uint32_t)(p.k1 - p.k0));
+        const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((n_pad >> 3) << 17) | (8u << 24);
+        const uint32_t buf = piece_no & 1u;
+        mbar_wait(ubar + 8u * (2 * kMaxStages + 2 + buf), ((piece_no >> 1) & 1u) ^ 1u);      // tempty
         tc_fence_after();
-        const uint32_t d_tmem = tmem_base + buf * kNPCap;
-        for (int kc = p.k0; kc < p.k1; ++kc, ++it) {
-          const int s = it % S;
-          mbar_wait(full_bar(s), (it / S) & 1);
+        const uint32_t d_tmem = utmem + buf * kNPCap;
+        for (uint32_t j = 0; j < nk; ++j) {
+          mbar_wait(ubar + 8u * s, par);                                                      // full
           tc_fence_after();
-          if (lane == 0) {
-            if (it == 0) FSTAMP(6);
-            const uint32_t sa = sm.stage_base + s * stage_bytes;
-            const uint64_t da = umma_desc_sw128(sa), db = umma_desc_sw128(sa + kUmmaWBytes);
+          if (first) { first = false; if (lane == 0) FSTAMP(6); }
+          const uint32_t sa = ubase + s * ustage;
+          const uint64_t da = umma_desc_sw128(sa), db = umma_desc_sw128(sa + kUmmaWBytes);
 #pragma unroll
-            for (int kk = 0; kk < 4; ++kk)
-              umma_bf16(d_tmem, da + 2 * kk, db + 2 * kk, idesc, (kc > p.k0 || kk > 0) ? 1u : 0u);
-            umma_commit(empty_bar(s));
-            if (kc == p.k1 - 1) umma_commit(tfull_bar(buf));
-          }
-          __syncwarp();
+          for (int kk = 0; kk < 4; ++kk) umma_bf16_if(leader, d_tmem, da + 2 * kk, db + 2 * kk, idesc, (j | kk) ? 1u : 0u);
+          umma_commit_if(leader, ubar + 8u * (kMaxStages + s));                                // empty
+          if (j == nk - 1) umma_commit_if(leader, ubar + 8u * (2 * kMaxStages + buf));         // tfull
+          if (++s == uS) { s = 0; par ^= 1u; }
         }
         ++piece_no;
       }
@@ -892,7 +919,12 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
                 const float gv = lo ? v[kk] : recv;
                 const float uv = lo ? recv : v[8 + kk];
                 const int tok = n0 + c0 + (lo ? kk : 8 + kk);
-                if (tok < wk.w) a.hbuf[(size_t)(wk.z + tok) * I + i] = f32_to_bf16_rn(__fdividef(gv, 1.0f + __expf(-gv)) * uv);
+#ifdef ELDR_EXP_NOEPI
+                if (tok < 0)
+#else
+                if (tok < wk.w)
+#endif
+                  a.hbuf[(size_t)(wk.z + tok) * I + i] = f32_to_bf16_rn(__fdividef(gv, 1.0f + __expf(-gv)) * uv);
               }
             } else {
               const int r = p.rt * 128 + row;
@@ -900,7 +932,12 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
 #pragma unroll
                 for (int kk = 0; kk < 16; ++kk) {
                   const int tok = n0 + c0 + kk;
-                  if (tok < wk.w) a.ybuf[(size_t)(wk.z + tok) * H + r] = v[kk];
+#ifdef ELDR_EXP_NOEPI
+                  if (tok < 0)
+#else
+                  if (tok < wk.w)
+#endif
+                    a.ybuf[(size_t)(wk.z + tok) * H + r] = v[kk];
                 }
               }
             }
