@@ -150,7 +150,7 @@ def main():
 
     import torch
     import torch.distributed as dist
-    from paper_2607_00466_b200 import api, synth
+    from paper_2607_00466_b200 import api, replicas, synth
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
@@ -228,12 +228,9 @@ def main():
                       "us_p90": round(float(np.percentile(per, 90)), 2),
                       "algorithmic_MB": round(c["bytes"] / 1e6, 1), "GBps": round(c["bytes"] / c["us"] / 1e3, 1),
                       "tokens_per_s": round(T / c["us"] * 1e6, 0)})
-    if world > 1:
-        tmax = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        total_ms = float(tmax.item())
+    total_ms = replicas.max_over_ranks(total_ms, dist if world > 1 else None, "cuda")
     total_bytes = sum(c["bytes"] for c in cases) * K
-    value = total_bytes * world / (total_ms * 1e-3) / 1e9
+    value = replicas.job_throughput_gbs(total_bytes, world, total_ms)
     peak, peak_kind = measured_peaks()
     for s in sweep:
         s["frac_of_%s_%.0f" % (peak_kind, peak)] = round(s["GBps"] / peak, 3)
@@ -297,11 +294,8 @@ def main():
     e1.record()
     barrier()
     e2e_ms = e0.elapsed_time(e1)
-    if world > 1:
-        tmax = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        e2e_ms = float(tmax.item())
-    e2e = {"value": round(total_bytes * world / (e2e_ms * 1e-3) / 1e9, 1), "unit": "GB/s",
+    e2e_ms = replicas.max_over_ranks(e2e_ms, dist if world > 1 else None, "cuda")
+    e2e = {"value": round(replicas.job_throughput_gbs(total_bytes, world, e2e_ms), 1), "unit": "GB/s",
            "h2d_bytes_per_step": T * shape.hidden * 2 + 2 * T * 4,
            "d2h_bytes_per_step": T * shape.hidden * 2 + T * shape.top_k * 8 + 4,
            "ms_per_step": round(e2e_ms / n_steps, 4)}
