@@ -411,7 +411,9 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
     fa.ring_bytes = g_ring_kb * 1024;
     const size_t smem = fixed + fa.stage_area;
     if ((size_t)fa.stage_area >= min_area) {
-      CUtensorMap tm_w13, tm_sw13, tm_w2, tm_sw2;
+      CUtensorMap tm_w13, tm_sw13, tm_w2, tm_sw2, tm_x, tm_h;
+      if (!make_tmap(&tm_x, x, (uint64_t)T, H, 1)) return ELDR_ERR_CUDA;                       // gather4: 1-row box
+      if (!make_tmap(&tm_h, hbuf, (uint64_t)T * (k + ns), I, 16)) return ELDR_ERR_CUDA;
       if (!make_tmap_w13_5d(&tm_w13, w13, E, I, H)) return ELDR_ERR_CUDA;
       if (!make_tmap(&tm_w2, w2, (uint64_t)E * H, I, 128)) return ELDR_ERR_CUDA;
       if (ns) {
@@ -431,7 +433,7 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
       }
       prof_begin();
       prof_mark(0, st);
-      launch_dep(moe_fused_kernel, dim3(num_sms()), dim3(kFusedThreads), smem, st, tm_w13, tm_sw13, tm_w2, tm_sw2, fa);
+      launch_dep(moe_fused_kernel, dim3(num_sms()), dim3(kFusedThreads), smem, st, tm_w13, tm_sw13, tm_w2, tm_sw2, tm_x, tm_h, fa);
       if (!launch_ok("moe_fused_kernel")) return ELDR_ERR_CUDA;
       prof_mark(ELDR_PROFILE_SLOTS, st);
       return ELDR_OK;

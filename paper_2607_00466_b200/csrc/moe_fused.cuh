@@ -41,7 +41,6 @@ constexpr int kFusedThreads = 256;
 constexpr int kFusedMaxT = 256;
 constexpr int kNPCap = 128;               // token columns per accumulator pass (TMEM: 2 x 128 columns)
 constexpr int kMaxStages = 12;
-constexpr int kXLag = 2;                  // cp.async groups kept in flight by EACH of the two activations producers
 
 // sync region (uint32 words) at the START of the layer workspace
 constexpr int kSyncGen = 0;
@@ -448,7 +447,7 @@ __device__ __forceinline__ void fused_route_a(const FusedArgs& a, const FusedSme
       s_off[E] = total;
       sm.meta[0] = n_work;
       sm.meta[1] = np;
-      sm.meta[2] = min(kMaxStages, max(min(a.stage_area, a.ring_bytes), 2 * (kXLag + 1) * (kUmmaWBytes + np * 128)) / (kUmmaWBytes + np * 128));  // >= 2*(kXLag+1): the two activation producers hold that many stages before arriving
+      sm.meta[2] = min(kMaxStages, max(min(a.stage_area, a.ring_bytes), 3 * (kUmmaWBytes + np * 128)) / (kUmmaWBytes + np * 128));
       if (is_cta0) { a.off[E] = total; *a.n_active = n_act; *a.n_work = n_work; }
     }
     if (lane == 31) sm.meta[3] = pinc;
@@ -536,6 +535,7 @@ struct PieceWalker {
 __global__ void __launch_bounds__(kFusedThreads, 1)
 moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_constant__ CUtensorMap tm_sw13,
                  const __grid_constant__ CUtensorMap tm_w2, const __grid_constant__ CUtensorMap tm_sw2,
+                 const __grid_constant__ CUtensorMap tm_x, const __grid_constant__ CUtensorMap tm_h,
                  const FusedArgs a) {
   extern __shared__ uint8_t smem_dyn[];
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -578,6 +578,8 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     mbar_fence_init();
     tma_prefetch_desc(&tm_w13);
     tma_prefetch_desc(&tm_w2);
+    tma_prefetch_desc(&tm_x);
+    tma_prefetch_desc(&tm_h);
   }
   constexpr uint32_t tmem_cols = 2 * kNPCap;
   if (warp == 6) {
@@ -693,46 +695,42 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     }
     __syncwarp();
   } else if (warp == 5 || warp == 7) {
-    // ================================================================ activations producers (cp.async gather)
-    // two warps, alternating ring stages: the per-stage barrier wait / proxy fence / arrive is what bounds one warp
+    // ================================================================ activations producers (TMA)
+    // Phase A: the expert's token rows of x are gathered four rows per instruction (tile::gather4) straight into
+    // the swizzled K-major B tile -- the permutation never exists in HBM.  Phase B: the expert's h rows are
+    // contiguous, plain 16-row boxes.  Nothing here waits for data: a stage's bytes are in flight as soon as its
+    // slot is free, as deep as the ring (cp.async groups tracked by a warp capped that at six stages).
+    // Two warps alternate ring stages.
     const uint32_t xw = warp == 7 ? 1u : 0u;
-    uint32_t it = 0, pend = 0, last = 0;
+    const uint64_t xpol = l2_policy_evict_last();
+    uint32_t it = 0;
 #ifdef ELDR_TRACE
     unsigned long long stall = 0, nb = 0;
 #endif
-    auto drain = [&]() {
-      cp_async_wait<0>();
-      fence_proxy_async_smem();
-      __syncwarp();
-      if (lane == 0)
-        for (uint32_t j = 0; j < pend; ++j) mbar_arrive(full_bar((last - 2 * (pend - 1 - j)) % S));
-      pend = 0;
-    };
     for (int sp = 0; sp < 4; ++sp) {
       const int ph = sp >> 1;
       PieceWalker pw;
       pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G);
       Piece p;
       int ready_ent = -1;
-      const size_t row_bytes = (size_t)(ph == 0 ? H : I) * 2;
-      const uint8_t* src_base = reinterpret_cast<const uint8_t*>(ph == 0 ? a.x : a.hbuf);
       while (pw.next(p)) {
         const int4 wk = sm.work[p.ent];
         if (ph == 1 && p.ent != ready_ent) {
-          // every h tile of this expert must have landed.  If not yet: first hand over everything already in
-          // flight (a piece of THIS CTA that the flags depend on could otherwise starve), then wait.
+          // every h tile of this expert must have landed (written by generic stores of other CTAs, read here by
+          // the async proxy: acquire, then a proxy fence)
           const uint32_t* fl = hready + (size_t)sm.cumpass[p.ent] * tilesA;
           const int nfl = (sm.cumpass[p.ent + 1] - sm.cumpass[p.ent]) * tilesA;
           if (!warp_test_flags(fl, nfl, epoch, lane)) {
 #ifdef ELDR_TRACE
             const unsigned long long t0_ = gtime();
 #endif
-            drain();
             warp_wait_flags(fl, nfl, epoch, lane);
 #ifdef ELDR_TRACE
             stall += gtime() - t0_; ++nb;
 #endif
           }
+          fence_proxy_async_all();
+          __syncwarp();
           ready_ent = p.ent;
 #ifdef ELDR_TRACE
           if (lane == 0 && xw == 0 && g_trace[(blockIdx.x & 4095) * 16 + 14] == 0) FSTAMP(14);
@@ -741,35 +739,32 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
         const int n0 = p.pass * kNPCap;
         const int n_here = min(kNPCap, wk.w - n0);
         const int n_pad = (n_here + 15) & ~15;
+        // phase A: this lane's four gather rows (padding rows repeat the last valid row; their columns are ignored)
+        int r0 = 0, r1 = 0, r2 = 0, r3 = 0;
+        if (ph == 0 && 4 * lane < n_pad) {
+          const uint16_t* tp = sm.tok_of_pos + wk.y + n0;
+          r0 = tp[min(4 * lane, n_here - 1)];
+          r1 = tp[min(4 * lane + 1, n_here - 1)];
+          r2 = tp[min(4 * lane + 2, n_here - 1)];
+          r3 = tp[min(4 * lane + 3, n_here - 1)];
+        }
         for (int kc = p.k0; kc < p.k1; ++kc, ++it) {
           if ((it & 1u) != xw) continue;
           const int s = it % S;
-          if (lane == 0) mbar_wait(empty_bar(s), ((it / S) & 1) ^ 1);
+          if (lane == 0) {
+            mbar_wait(empty_bar(s), ((it / S) & 1) ^ 1);
+            mbar_arrive_expect_tx(full_bar(s), (uint32_t)n_pad * 128u);
+          }
           __syncwarp();
           const uint32_t dst = sm.stage_base + s * stage_bytes + kUmmaWBytes;
-#ifdef ELDR_EXP_NOX
-          if (false)
-#endif
-          for (int q = lane; q < n_pad * 8; q += 32) {
-            const int r = q >> 3, c = q & 7;
-            const int rr = min(r, n_here - 1);                     // padding rows: any valid row (result ignored)
-            const size_t grow = ph == 0 ? (size_t)sm.tok_of_pos[wk.y + n0 + rr] : (size_t)(wk.z + n0 + rr);
-            cp_async16(dst + r * 128 + ((c ^ (r & 7)) << 4), src_base + grow * row_bytes + (size_t)kc * 128 + c * 16);
-          }
-          cp_async_commit();
-          last = it;
-          ++pend;
-          if (pend > kXLag) {
-            cp_async_wait<kXLag>();
-            fence_proxy_async_smem();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(full_bar((last - 2 * (pend - 1)) % S));
-            --pend;
+          if (ph == 0) {
+            if (4 * lane < n_pad) tma_gather4(dst + lane * 512, &tm_x, kc * 64, r0, r1, r2, r3, full_bar(s), xpol);
+          } else {
+            if (16 * lane < n_pad) tma_load_2d(dst + lane * 2048, &tm_h, kc * 64, wk.z + n0 + 16 * lane, full_bar(s), xpol);
           }
         }
       }
     }
-    drain();
 #ifdef ELDR_TRACE
     if (lane == 0 && xw == 0) { FVALUE(12, stall); }
 #endif
@@ -952,7 +947,9 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
           if (lane == 0) mbar_arrive(tempty_bar(buf));
           if (tid == 0 && ph == 0) FSTAMP(4);
           if (ph == 0) {
-            // publish "h tile written": the four epilogue warps meet, one thread releases (cumulative)
+            // publish "h tile written": each writer orders its stores before later async-proxy (TMA) reads, the
+            // four epilogue warps meet, one thread releases (cumulative)
+            fence_proxy_async_all();
             asm volatile("bar.sync 1, 128;" ::: "memory");
             if (tid == 0) { flag_release(hready + p.tile, epoch); FSTAMP(15); }
           }
