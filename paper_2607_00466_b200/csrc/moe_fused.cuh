@@ -89,8 +89,10 @@ __device__ __forceinline__ unsigned long long gtime() {
 #define FSTAMP(id) do { g_trace[(blockIdx.x & 4095) * 16 + (id)] = gtime(); } while (0)
 #define FVALUE(id, v) do { g_trace[(blockIdx.x & 4095) * 16 + (id)] = (unsigned long long)(v); } while (0)
 #define FVALUE2(id, v) do { g_trace[((blockIdx.x + 2048) & 4095) * 16 + (id)] = (unsigned long long)(v); } while (0)
+#define FSTAMP2(id) do { g_trace[((blockIdx.x + 2048) & 4095) * 16 + (id)] = gtime(); } while (0)
 #define FTIMED(acc, stmt) do { const long long c0_ = clock64(); stmt; acc += clock64() - c0_; } while (0)
 #else
+#define FSTAMP2(id) do {} while (0)
 #define FVALUE2(id, v) do {} while (0)
 #define FTIMED(acc, stmt) do { stmt; } while (0)
 #define FSTAMP(id) do {} while (0)
@@ -105,16 +107,35 @@ __device__ __forceinline__ uint32_t flag_acquire(const uint32_t* p) {
   asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
 }
-// One warp waits until flags[0..n) all equal epoch (lanes stride over the flags; a short sleep between polls
-// keeps 148 pollers from saturating the flag's L2 slice).  Traps instead of hanging.
+__device__ __forceinline__ uint32_t flag_relaxed(const uint32_t* p) {
+  uint32_t v;
+  asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void fence_acq_rel_gpu() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
+// One warp waits until flags[0..n) all equal epoch.  Every lane keeps all of its flags' (relaxed) loads in flight
+// together -- a chain of acquire loads costs one L2 round trip per flag -- and one fence after the last successful
+// poll gives the acquire.  A short sleep between polls keeps 148 pollers from saturating the flags' L2 slice.
+// Traps instead of hanging.
 __device__ __forceinline__ void warp_wait_flags(const uint32_t* flags, int n, uint32_t epoch, int lane) {
-  for (int i = lane; i < n; i += 32) {
-    uint32_t spins = 0;
-    while (flag_acquire(flags + i) != epoch) {
-      __nanosleep(40);
-      if (++spins > (1u << 24)) __trap();
+  uint32_t spins = 0;
+  for (;;) {
+    bool ok = true;
+    for (int i0 = 0; i0 < n; i0 += 256) {
+      uint32_t v[8];
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        const int i = i0 + lane + 32 * j;
+        v[j] = (i < n) ? flag_relaxed(flags + i) : epoch;
+      }
+#pragma unroll
+      for (int j = 0; j < 8; ++j) ok = ok && (v[j] == epoch);
     }
+    if (__all_sync(0xffffffffu, ok)) break;
+    __nanosleep(40);
+    if (++spins > (1u << 24)) __trap();
   }
+  fence_acq_rel_gpu();
   __syncwarp();
 }
 __device__ __forceinline__ bool warp_test_flags(const uint32_t* flags, int n, uint32_t epoch, int lane) {
@@ -608,6 +629,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
       __syncthreads();
       if (tid == 0) flag_release(a.sync + kSyncTile + g * 32 + et, epoch);    // cumulative over the barrier
     }
+    if (tid == 0) FSTAMP2(12);
     for (int g = ((cta - n_tiles % G) + G) % G; g < n_gr; g += G) {       // owner(g) = (n_tiles + g) % G
       if (warp == 0) warp_wait_flags(a.sync + kSyncTile + g * 32, n_et, epoch, lane);
       __syncthreads();
@@ -625,15 +647,15 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
       __syncthreads();
       if (tid == 0) flag_release(a.sync + kSyncGroup + g, epoch);
     }
-    if (tid == 0) FSTAMP(2);
+    if (tid == 0) FSTAMP2(13);
     if (warp == 0) warp_wait_flags(a.sync + kSyncGroup, n_gr, epoch, lane);
     __syncthreads();
-    if (tid == 0) FSTAMP(3);
+    if (tid == 0) FSTAMP2(14);
   }
 
   // ------------------------------------------------------------------------------------------ R: routing
   fused_route_a(a, sm, sm.route_scratch, cta == 0);
-  if (tid == 0) FSTAMP(4);
+  if (tid == 0) FSTAMP2(15);
   if (warp != 4) {
     // the weights producer (warp 4) is already streaming; everyone else finishes the position maps
     fused_route_b(a, sm, sm.route_scratch, cta == 0, warp < 4 ? tid : tid - 32, kFusedThreads - 32);
@@ -829,6 +851,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
         // Head piece of a split tile: the other pieces were parked long ago (their owners reach the tile first).
         // Find them, wait for their flags and request the first chunk of the first partner BEFORE waiting for our
         // own accumulator: under a saturated memory system every dependent L2 round trip costs more than a microsecond.
+        if (tid == 0 && ph == 0) FSTAMP2(3);
         int n_partner = 0;
         float4 pf0[4], pf1[4];                                  // two chunks of the first partner in flight
         bool pf_valid = false;
@@ -858,6 +881,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
             for (int q = 0; q < 4; ++q) dst[q] = __ldcg(reinterpret_cast<const float4*>(pf_src + c0 + 4 * q));
           }
         };
+        if (tid == 0 && ph == 0) FSTAMP2(2);
         pf_load(pf0, 0);
         pf_load(pf1, 16);
         mbar_wait(tfull_bar(buf), (piece_no >> 1) & 1);
