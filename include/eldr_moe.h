@@ -163,6 +163,9 @@ int32_t eldr_moe_workspace_layout(const eldr_moe_shape_t* shape, int32_t T, eldr
                                  combine), also the path for shapes the fused kernel does not take */
 #define ELDR_OPT_RING_KB  3   /* fused step: cap on the shared-memory stage ring in KiB per SM (bytes in flight);
                                  32..208; default 208 (all of it) */
+#define ELDR_OPT_DP_MIN_ROUNDS 4 /* fused step: a phase whose tile count is at least this many rounds of the grid runs its
+                                 whole rounds round-robin (no split tiles) and only the remainder as stream-K; below it the
+                                 whole phase is stream-K.  1..2^20; default 6 */
 #define ELDR_STEP_STAGED  0
 #define ELDR_STEP_FUSED   1
 #define ELDR_FFN_MMA_SYNC 0

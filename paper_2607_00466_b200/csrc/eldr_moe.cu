@@ -23,6 +23,7 @@ int g_ffn_path = ELDR_FFN_TCGEN05;   // process-wide tuning knobs (eldr_moe_set_
 int g_pdl = 1;
 int g_step_path = ELDR_STEP_FUSED;
 int g_ring_kb = 208;
+int g_dp_min_rounds = 6;
 
 thread_local char g_err[256] = "";
 thread_local int g_launches = 0;
@@ -284,6 +285,10 @@ int32_t eldr_moe_set_option(int32_t key, int32_t value) {
     g_ring_kb = value;
     return ELDR_OK;
   }
+  if (key == ELDR_OPT_DP_MIN_ROUNDS && value >= 1 && value <= (1 << 20)) {
+    g_dp_min_rounds = value;
+    return ELDR_OK;
+  }
   return ELDR_ERR_INVALID_ARG;
 }
 
@@ -409,6 +414,7 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
                                 ? (size_t)3 * (kUmmaWBytes + kNPCap * 128) : (size_t)kGateTok * H * 2;
     fa.stage_area = fixed < smem_max ? (int)((smem_max - fixed) / 1024 * 1024) : 0;
     fa.ring_bytes = g_ring_kb * 1024;
+    fa.dp_min_rounds = g_dp_min_rounds;
     const size_t smem = fixed + fa.stage_area;
     if ((size_t)fa.stage_area >= min_area) {
       CUtensorMap tm_w13, tm_sw13, tm_w2, tm_sw2, tm_x, tm_h;

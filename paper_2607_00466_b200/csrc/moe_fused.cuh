@@ -78,6 +78,7 @@ struct FusedArgs {
   uint16_t* out;               // [T,H] bf16
   int stage_area;              // bytes of shared memory cut into ring stages (multiple of 1024; set by the host)
   int ring_bytes;              // cap on the bytes the ring keeps in flight (<= stage_area)
+  int dp_min_rounds;           // hybrid schedule: data-parallel part only if a phase has at least this many tile rounds
 };
 
 #ifdef ELDR_TRACE
@@ -503,51 +504,61 @@ __device__ __forceinline__ void fused_route_b(const FusedArgs& a, const FusedSme
 struct Piece {
   int tile, k0, k1, ent, pass, rt;
 };
-// Where the (entry, pass) list is cut in two.  Halving only pays when each SM's stage range still spans several
-// tiles per sub-phase (otherwise every tile is split over 2-3 SMs and the fix-up chain costs more than the
-// hand-over it hides); measured on B200 it gave nothing at |U| = 64..128 and lost 8 us at |U| = 16, so the cut is
-// at the end: sub-phases 1 and 3 are empty.
-__device__ __forceinline__ int split_mid(int total_pass, int tilesA, int kitA, int G) {
-  (void)tilesA; (void)kitA; (void)G;
-  return total_pass;
-}
+// Hybrid schedule.  Per phase the tile list (entry-major, so experts come in order) is cut at R0 = the largest
+// multiple of gridDim.x:
+//   part 0 ("data-parallel"): tiles [0, R0) go round-robin, whole, tile r*G + c to CTA c in round r -- no split,
+//           no fix-up, and experts FINISH IN ORDER over the phase;
+//   part 1 ("stream-K remainder"): the stages of tiles [R0, end) are cut into gridDim.x equal contiguous ranges.
+// Sub-phase order A0 A1 B0 B1: B0 starts on the first experts, whose h tiles were all produced in A0 (several
+// microseconds earlier), so the w1/w3 -> w2 hand-over costs no pipeline drain; B1 needs the last experts, finished
+// a whole B0 earlier.  (With equal contiguous ranges over the WHOLE phase every expert had a tile finished in the
+// last microsecond of A, and every CTA stalled ~9 us at the hand-over.)
 struct PieceWalker {
   int tpe, kit;          // row tiles per (entry, pass); k-chunks per tile
-  long long g, hi;       // current / end stage
+  long long g, hi, P;    // remainder part: current / end stage of this CTA, total stages
   int ent;               // cursor into cumpass
   const int32_t* cumpass;
-  int tile0;             // first tile of this sub-phase
-  // Sub-phase sp: 0 = w1/w3 of the first half of the (entry, pass) list, 1 = w1/w3 of the second half,
-  // 2 = w2 of the first half, 3 = w2 of the second half.  Each sub-phase is cut into gridDim.x equal stage ranges.
-  // Running them in this order puts one whole sub-phase of streaming between the production of an expert's h
-  // and its consumption, which hides the release -> poll -> load chain of the hand-over.
+  int tile0;             // remainder part: first tile (R0)
+  int dp_tile, dp_end, G;
+  bool dp;
   __device__ __forceinline__ void init(int sp, int tilesA, int tilesB, int kitA, int kitB, int total_pass,
-                                       const int32_t* cp, int cta, int G) {
+                                       const int32_t* cp, int cta, int G_, int min_rounds) {
     const int ph = sp >> 1;
     tpe = ph == 0 ? tilesA : tilesB;
     kit = ph == 0 ? kitA : kitB;
-    const int mid = split_mid(total_pass, tilesA, kitA, G);
-    const int cp_lo = (sp & 1) ? mid : 0;
-    const int cp_hi = (sp & 1) ? total_pass : mid;
-    tile0 = cp_lo * tpe;
-    const long long P = (long long)(cp_hi - cp_lo) * tpe * kit;
+    G = G_;
+    const int n_tiles = total_pass * tpe;
+    const int R0 = (n_tiles / G >= min_rounds) ? (n_tiles / G) * G : 0;   // few rounds: all stream-K
+    dp = (sp & 1) == 0;
+    dp_tile = cta;
+    dp_end = R0;
+    tile0 = R0;
+    P = (long long)(n_tiles - R0) * kit;
     g = P * cta / G;
     hi = P * (cta + 1) / G;
     ent = 0;
     cumpass = cp;
   }
   __device__ __forceinline__ bool next(Piece& p) {
-    if (g >= hi) return false;
-    const int lt = (int)(g / kit);                 // tile index inside the sub-phase
-    p.tile = tile0 + lt;
-    p.k0 = (int)(g - (long long)lt * kit);
-    p.k1 = (int)min((long long)kit, p.k0 + (hi - g));
+    if (dp) {
+      if (dp_tile >= dp_end) return false;
+      p.tile = dp_tile;
+      p.k0 = 0;
+      p.k1 = kit;
+      dp_tile += G;
+    } else {
+      if (g >= hi) return false;
+      const int lt = (int)(g / kit);                 // tile index inside the remainder
+      p.tile = tile0 + lt;
+      p.k0 = (int)(g - (long long)lt * kit);
+      p.k1 = (int)min((long long)kit, p.k0 + (hi - g));
+      g += p.k1 - p.k0;
+    }
     const int cpi = p.tile / tpe;
     p.rt = p.tile - cpi * tpe;
     while (cumpass[ent + 1] <= cpi) ++ent;
     p.ent = ent;
     p.pass = cpi - cumpass[ent];
-    g += p.k1 - p.k0;
     return true;
   }
 };
@@ -683,7 +694,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
       for (int sp = 0; sp < 4; ++sp) {
       const int ph = sp >> 1;
         PieceWalker pw;
-        pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G);
+        pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds);
         Piece p;
         while (pw.next(p)) {
           const int4 wk = sm.work[p.ent];
@@ -732,7 +743,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     for (int sp = 0; sp < 4; ++sp) {
       const int ph = sp >> 1;
       PieceWalker pw;
-      pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G);
+      pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds);
       Piece p;
       int ready_ent = -1;
       while (pw.next(p)) {
@@ -804,7 +815,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     bool first = true;
     for (int sp = 0; sp < 4; ++sp) {
       PieceWalker pw;
-      pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G);
+      pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds);
       Piece p;
       while (pw.next(p)) {
         const int4 wk = sm.work[p.ent];
@@ -838,9 +849,8 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     for (int sp = 0; sp < 4; ++sp) {
       const int ph = sp >> 1;
       PieceWalker pw;
-      pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G);
-      const int mid_ = split_mid(total_pass, tilesA, kitA, G);
-      const long long P = (long long)((sp & 1) ? total_pass - mid_ : mid_) * pw.tpe * pw.kit;
+      pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds);
+      const long long P = pw.P;
       Piece p;
       while (pw.next(p)) {
         const int4 wk = sm.work[p.ent];
