@@ -165,7 +165,7 @@ int32_t eldr_moe_workspace_layout(const eldr_moe_shape_t* shape, int32_t T, eldr
                                  32..208; default 208 (all of it) */
 #define ELDR_OPT_DP_MIN_ROUNDS 4 /* fused step: a phase whose tile count is at least this many rounds of the grid runs its
                                  whole rounds round-robin (no split tiles) and only the remainder as stream-K; below it the
-                                 whole phase is stream-K.  1..2^20; default 6 */
+                                 whole phase is stream-K.  1..2^20; default 4 */
 #define ELDR_STEP_STAGED  0
 #define ELDR_STEP_FUSED   1
 #define ELDR_FFN_MMA_SYNC 0

@@ -23,7 +23,7 @@ int g_ffn_path = ELDR_FFN_TCGEN05;   // process-wide tuning knobs (eldr_moe_set_
 int g_pdl = 1;
 int g_step_path = ELDR_STEP_FUSED;
 int g_ring_kb = 208;
-int g_dp_min_rounds = 6;
+int g_dp_min_rounds = 4;
 
 thread_local char g_err[256] = "";
 thread_local int g_launches = 0;

@@ -41,9 +41,12 @@ constexpr int kFusedThreads = 256;
 constexpr int kFusedMaxT = 256;
 constexpr int kNPCap = 128;               // token columns per accumulator pass (TMEM: 2 x 128 columns)
 constexpr int kMaxStages = 12;
+constexpr int kClaimSlots = 4;            // claimed-tile ring: weights producer -> the seven consumer warps
 
 // sync region (uint32 words) at the START of the layer workspace
 constexpr int kSyncGen = 0;
+constexpr int kSyncCntReady = 1;                // CTA 0 zeroed this step's tile counters
+constexpr int kSyncTileCnt = 2;                 // [2] next unclaimed data-parallel tile of phase A / B
 constexpr int kSyncDone = 32;                   // [256]     per CTA "all my pieces are finished"
 constexpr int kSyncGroup = kSyncDone + 256;     // [32]      per token group "ids/weights written"
 constexpr int kSyncTile = kSyncGroup + 32;      // [32][32]  gate logit tile written
@@ -313,8 +316,9 @@ __device__ __forceinline__ void warp_topk_redux(const float* __restrict__ zrow, 
 // ------------------------------------------------------------------------------------ shared-memory plan
 struct FusedSmem {
   uint32_t stage_base;     // stage_area bytes cut into S stages of [16 KiB weights | np*128 B activations]
-  uint32_t bar_base;       // full[kMaxStages], empty[kMaxStages], tfull[2], tempty[2]
+  uint32_t bar_base;       // full[kMaxStages], empty[kMaxStages], tfull[2], tempty[2], cfull[4], cempty[4]
   uint32_t tmem_slot;
+  volatile int32_t* claim; // [kClaimSlots] claimed data-parallel tile ids (-1 = part finished)
   int4* work;              // [E+ns] {expert, x_row0, out_row0, m}
   int32_t* cumpass;        // [E+ns+1] exclusive scan of accumulator passes per work entry
   int32_t* meta;           // [8] {n_work, np, S, total passes}
@@ -327,7 +331,7 @@ struct FusedSmem {
 // Bytes of everything except the stage ring (barriers, routing tables); the host gives the ring what is left.
 __host__ __device__ inline size_t fused_smem_fixed_bytes(int E, int ns, int T, int k) {
   const size_t W = (T + 31) / 32;
-  size_t o = 256;                                        // barriers + tmem slot
+  size_t o = 512;                                        // barriers + claim ring + tmem slot
   o += (size_t)(E + ns) * 16;
   o += ((size_t)(E + ns + 1) * 4 + 15) / 16 * 16;
   o += 32;
@@ -539,13 +543,14 @@ struct PieceWalker {
     ent = 0;
     cumpass = cp;
   }
-  __device__ __forceinline__ bool next(Piece& p) {
+  // data-parallel part: `claimed` is the tile this CTA drew from the phase's counter (ascending per CTA), or
+  // anything >= dp_end / negative when the part is exhausted.  Remainder part: `claimed` is ignored.
+  __device__ __forceinline__ bool next(Piece& p, int claimed) {
     if (dp) {
-      if (dp_tile >= dp_end) return false;
-      p.tile = dp_tile;
+      if (claimed < 0 || claimed >= dp_end) return false;
+      p.tile = claimed;
       p.k0 = 0;
       p.k1 = kit;
-      dp_tile += G;
     } else {
       if (g >= hi) return false;
       const int lt = (int)(g / kit);                 // tile index inside the remainder
@@ -581,8 +586,9 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     sm.stage_base = base;
     size_t o = (size_t)a.stage_area;
     sm.bar_base = base + (uint32_t)o;
-    sm.tmem_slot = base + (uint32_t)o + 240;
-    o += 256;
+    sm.tmem_slot = base + (uint32_t)o + 496;
+    sm.claim = reinterpret_cast<volatile int32_t*>(gen + o + 320);
+    o += 512;
     sm.work = reinterpret_cast<int4*>(gen + o);
     o += (size_t)(E + ns) * 16;
     sm.cumpass = reinterpret_cast<int32_t*>(gen + o);
@@ -602,11 +608,14 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
   auto empty_bar = [&](int s) { return sm.bar_base + 8u * (kMaxStages + s); };
   auto tfull_bar = [&](int b) { return sm.bar_base + 8u * (2 * kMaxStages + b); };
   auto tempty_bar = [&](int b) { return sm.bar_base + 8u * (2 * kMaxStages + 2 + b); };
+  auto cfull_bar = [&](int b) { return sm.bar_base + 8u * (2 * kMaxStages + 4 + b); };
+  auto cempty_bar = [&](int b) { return sm.bar_base + 8u * (2 * kMaxStages + 4 + kClaimSlots + b); };
 
   // ------------------------------------------------------------- prologue (overlaps the previous kernel's tail)
   if (tid == 0) {
     for (int s = 0; s < kMaxStages; ++s) { mbar_init(full_bar(s), 2); mbar_init(empty_bar(s), 1); }
     for (int b = 0; b < 2; ++b) { mbar_init(tfull_bar(b), 1); mbar_init(tempty_bar(b), 4); }
+    for (int b = 0; b < kClaimSlots; ++b) { mbar_init(cfull_bar(b), 1); mbar_init(cempty_bar(b), 7); }
     mbar_fence_init();
     tma_prefetch_desc(&tm_w13);
     tma_prefetch_desc(&tm_w2);
@@ -629,6 +638,12 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
   if (tid == 0) FSTAMP(1);
 
   const uint32_t epoch = __ldcg(a.sync + kSyncGen) + 1u;
+  if (cta == 0 && tid == 0) {
+    // this step's tile counters (the previous grid has completed: pdl_wait above)
+    a.sync[kSyncTileCnt] = 0u;
+    a.sync[kSyncTileCnt + 1] = 0u;
+    flag_release(a.sync + kSyncCntReady, epoch);
+  }
 
   // ------------------------------------------------------------------------------ G + K: gate and top-k
   if (!a.force_routing) {
@@ -683,20 +698,53 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
   uint32_t* pready = a.sync + kSyncPartial;
   (void)n_work;
 
+  // Consumer side of the claimed-tile ring (a converged warp; `cn` = claims this warp has popped so far).
+  auto claim_pop = [&](uint32_t& cn) -> int {
+    const uint32_t slot = cn & (kClaimSlots - 1);
+    int v = 0;
+    if (lane == 0) {
+      mbar_wait(cfull_bar(slot), (cn / kClaimSlots) & 1);
+      v = sm.claim[slot];
+      mbar_arrive(cempty_bar(slot));
+    }
+    ++cn;
+    return __shfl_sync(0xffffffffu, v, 0);
+  };
+  // next piece of a consumer warp: data-parallel part -> pop a claim; remainder part -> the static walker
+  auto consumer_next = [&](PieceWalker& pw, Piece& p, uint32_t& cn) -> bool {
+    if (pw.dp) {
+      if (pw.dp_end == 0) return false;
+      return pw.next(p, claim_pop(cn));
+    }
+    return pw.next(p, 0);
+  };
+
   if (warp == 4) {
     // ================================================================ weights producer (one lane)
+    // Also draws this CTA's data-parallel tiles from the phase's global counter -- SMs do not get equal shares of
+    // a saturated HBM (measured: +-8 %), so fixed rounds left the slow SMs 15-30 us behind at the grid barrier --
+    // and hands each drawn tile to the seven consumer warps through a 4-slot shared-memory ring.  The next draw is
+    // in flight while the current tile streams.
     if (lane == 0) {
       const uint64_t pol = l2_policy_evict_first();
       FSTAMP(5);
-      uint32_t it = 0;
+      uint32_t it = 0, wn = 0;
+      bool cnt_ready = false;
       long long w_wait[2] = {0, 0}, w_iss[2] = {0, 0};
       (void)w_wait; (void)w_iss;
+      auto claim_push = [&](int v) {
+        const uint32_t slot = wn & (kClaimSlots - 1);
+        mbar_wait(cempty_bar(slot), ((wn / kClaimSlots) & 1) ^ 1);
+        sm.claim[slot] = v;
+        mbar_arrive(cfull_bar(slot));
+        ++wn;
+      };
       for (int sp = 0; sp < 4; ++sp) {
-      const int ph = sp >> 1;
+        const int ph = sp >> 1;
         PieceWalker pw;
         pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds);
         Piece p;
-        while (pw.next(p)) {
+        auto stream_piece = [&]() {
           const int4 wk = sm.work[p.ent];
           const bool shared = wk.x >= E;
           const int we = shared ? wk.x - E : wk.x;
@@ -709,17 +757,31 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
 #endif
             mbar_arrive_expect_tx(full_bar(s), kUmmaWBytes);
             const uint32_t dst = sm.stage_base + s * stage_bytes;
-            if (ph == 0)
-#ifdef ELDR_EXP_W13_2D
-              tma_load_2d(dst, &tm_sw13, kc * 64, we * 2 * I + p.rt * 128, full_bar(s), pol);
-            else if (false)
-#endif
-              tma_load_5d(dst, tmw, kc * 64, 0, 0, p.rt * 4, we, full_bar(s), pol);
+            if (ph == 0) tma_load_5d(dst, tmw, kc * 64, 0, 0, p.rt * 4, we, full_bar(s), pol);
             else tma_load_2d(dst, tmw, kc * 64, we * H + p.rt * 128, full_bar(s), pol);
 #ifdef ELDR_TRACE
             w_iss[ph] += clock64() - cw_;
 #endif
           }
+        };
+        if (pw.dp) {
+          if (pw.dp_end > 0) {
+            if (!cnt_ready) {
+              uint32_t spins = 0;
+              while (flag_acquire(a.sync + kSyncCntReady) != epoch) { __nanosleep(40); if (++spins > (1u << 24)) __trap(); }
+              cnt_ready = true;
+            }
+            int cur = (int)atomicAdd(a.sync + kSyncTileCnt + ph, 1u);
+            claim_push(cur);
+            while (pw.next(p, cur)) {
+              const int nxt = (int)atomicAdd(a.sync + kSyncTileCnt + ph, 1u);     // in flight while this tile streams
+              stream_piece();
+              claim_push(nxt);
+              cur = nxt;
+            }
+          }
+        } else {
+          while (pw.next(p, 0)) stream_piece();
         }
         if (sp == 1) FSTAMP(11);
       }
@@ -736,7 +798,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     // Two warps alternate ring stages.
     const uint32_t xw = warp == 7 ? 1u : 0u;
     const uint64_t xpol = l2_policy_evict_last();
-    uint32_t it = 0;
+    uint32_t it = 0, cn = 0;
 #ifdef ELDR_TRACE
     unsigned long long stall = 0, nb = 0;
 #endif
@@ -746,7 +808,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
       pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds);
       Piece p;
       int ready_ent = -1;
-      while (pw.next(p)) {
+      while (consumer_next(pw, p, cn)) {
         const int4 wk = sm.work[p.ent];
         if (ph == 1 && p.ent != ready_ent) {
           // every h tile of this expert must have landed (written by generic stores of other CTAs, read here by
@@ -811,13 +873,13 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     const uint32_t uS = warp_uniform((uint32_t)S), ustage = warp_uniform(stage_bytes);
     const uint32_t ubase = warp_uniform(sm.stage_base), ubar = warp_uniform(sm.bar_base);
     const uint32_t utmem = warp_uniform(tmem_base);
-    uint32_t s = 0, par = 0, piece_no = 0;
+    uint32_t s = 0, par = 0, piece_no = 0, cn = 0;
     bool first = true;
     for (int sp = 0; sp < 4; ++sp) {
       PieceWalker pw;
       pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds);
       Piece p;
-      while (pw.next(p)) {
+      while (consumer_next(pw, p, cn)) {
         const int4 wk = sm.work[p.ent];
         const uint32_t n_pad = warp_uniform((uint32_t)((min(kNPCap, wk.w - p.pass * kNPCap) + 15) & ~15));
         const uint32_t nk = warp_uniform((uint32_t)(p.k1 - p.k0));
@@ -845,14 +907,14 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
   } else if (warp < 4) {
     // ================================================================ epilogue (TMEM lane quarter = warp)
     const int qtr = warp;
-    uint32_t piece_no = 0;
+    uint32_t piece_no = 0, cn = 0;
     for (int sp = 0; sp < 4; ++sp) {
       const int ph = sp >> 1;
       PieceWalker pw;
       pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds);
       const long long P = pw.P;
       Piece p;
-      while (pw.next(p)) {
+      while (consumer_next(pw, p, cn)) {
         const int4 wk = sm.work[p.ent];
         const int n0 = p.pass * kNPCap;
         const int n_here = min(kNPCap, wk.w - n0);
