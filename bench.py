@@ -92,6 +92,21 @@ class ClockSampler(threading.Thread):
                 "reasons": sorted(self.reasons), "samples": len(s)}
 
 
+def ncu_traffic(unions):
+    """dram__bytes_read.sum + dram__bytes_write.sum of moe_fused_kernel per launch, from the committed summary of
+    one `ncu --set full` capture per union size (profiles/r1_fused_full.csv; command in profiles/r1_fused_full.md).
+    Averaged over the sweep's union sizes like `achieved`; None if a size is missing."""
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "profiles", "r1_fused_full.csv")
+    try:
+        import csv
+        rows = {int(float(r["union"])): float(r["dram__bytes_read.sum"]) + float(r["dram__bytes_write.sum"])
+                for r in csv.DictReader(open(path))}
+        per = {u: rows[u] for u in unions}
+        return round(sum(per.values()) / len(per)), {str(u): round(v) for u, v in per.items()}
+    except Exception:
+        return None, None
+
+
 def run_reference(args, rank, world):
     """--impl reference: the fp64 CPU oracle as it stands, on the box's host cores, same metric and config.
     Each step = the oracle's whole layer on a bounded sample (the first 4 of the 64 tokens of the batch) at one
@@ -275,7 +290,9 @@ def main():
                 "achieved": round(top_gbs, 1), "peak": peak,
                 "peak_kind": (peak_kind + " HBM copy rate (MEASURED_PEAKS.json)") if peak_kind == "measured"
                 else "fallback 6.65 TB/s (B200_PROFILING.md)",
-                "unit": "GB/s", "frac": round(top_gbs / peak, 3), "traffic": None,
+                "unit": "GB/s", "frac": round(top_gbs / peak, 3),
+                "traffic": ncu_traffic([c["n_active"] for c in cases])[0] if fused else None,
+                "traffic_per_union": ncu_traffic([c["n_active"] for c in cases])[1] if fused else None,
                 "algorithmic_bytes_per_launch": round(kbytes / n_steps), "avg_launch_us": round(top_ms * 1e3, 2),
                 "kernel_share_of_step": {n: round(v / max(sum(kern.values()), 1e-9), 3) for n, v in kern.items()},
                 "kernel_us": {n: round(v / n_steps * 1e3, 2) for n, v in kern.items()}}

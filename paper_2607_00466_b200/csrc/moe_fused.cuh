@@ -11,17 +11,22 @@
 //      offsets -> union-compacted work list (the weights producer starts streaming here) -> token<->position
 //      maps, all in shared memory.  No second election, no route/gather kernels, no work list in HBM.
 //      CTA 0 also writes the routing outputs of the C ABI (active list, n_active, cnt/off/perm/pair_pos).
-//   F  expert FFN on tcgen05 + TMEM, swap-AB (weights = M=128 operand, the expert's tokens = N operand), as a
-//      STATIC stream-K schedule: per phase (A: w1/w3 tiles, B: w2 tiles) the flattened sequence of 16 KiB
-//      weight stages (tile-major, k-chunk minor) is cut into gridDim.x equal contiguous ranges, so every SM
-//      streams the same number of bytes (+-1 stage) whatever the union size.  A tile cut by a range boundary
-//      is finished by the CTA that owns its k=0 end: the other owner(s) -- which reach the tile FIRST, at the
-//      start of their range -- park raw fp32 accumulators in a scratch slot and raise a flag; the head owner adds
-//      them in ascending CTA order (a fixed order: results are run-to-run bit-identical).  Weights: TMA
-//      (SWIZZLE_128B, evict_first).  Activations: a producer warp gathers the expert's token rows with cp.async
-//      straight from x (A) or h (B) into the swizzled K-major B tile -- the permutation never exists in HBM.
-//      Phase B waits on per-tile epoch flags of the expert's h tiles (release/acquire through L2).  Phase A
-//      never waits on phase B and first pieces never wait on anything, so there is no cycle.
+//   F  expert FFN on tcgen05 + TMEM, swap-AB (weights = M=128 operand, the expert's tokens = N operand).  Per
+//      phase (A: w1/w3 tiles, B: w2 tiles) the tile list is entry-major (experts in order).  HYBRID schedule:
+//      whole rounds of gridDim.x tiles are "data-parallel" -- never split, drawn tile by tile from a global counter
+//      by each CTA's weights producer (SMs get unequal shares of a saturated HBM, so fast SMs draw more) -- and the
+//      remaining < gridDim.x tiles (or the whole phase when it has fewer than `dp_min_rounds` rounds) are a STATIC
+//      stream-K schedule: the flattened sequence of 16 KiB weight stages (tile-major, k-chunk minor) is cut into
+//      gridDim.x equal contiguous ranges.  A tile cut by a range boundary is finished by the CTA that owns its k=0
+//      end: the other owner(s) -- which reach the tile FIRST, at the start of their range -- park raw fp32
+//      accumulators in a scratch slot and raise a flag; the head owner adds them in ascending CTA order (a fixed
+//      order: results are run-to-run bit-identical whichever CTA computed a whole tile).  Weights: TMA
+//      (SWIZZLE_128B, evict_first).  Activations: TMA too -- tile::gather4 pulls the expert's token rows straight
+//      from x (A), 16-row boxes read h (B) -- into the swizzled K-major B tile; the permutation never exists in
+//      HBM.  Phase B waits on per-tile epoch flags of the expert's h tiles (release/acquire through L2, proxy
+//      fences around the TMA reads).  Phase A never waits on phase B and first pieces never wait on anything, so
+//      there is no cycle.  Because data-parallel tiles finish in expert order, B's first rounds find their h
+//      long finished: no pipeline drain at the hand-over when the union is large.
 //      The B-tile rows per stage adapt to the batch's largest tokens-per-expert count, so small-m steps get a
 //      deeper weight ring (more bytes in flight).
 //   C  ordered combine after a flag barrier over the grid: out[t] = sum_j w[t,j]*y[pos(t,j)] (+ shared) in
