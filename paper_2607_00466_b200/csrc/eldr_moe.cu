@@ -406,6 +406,7 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
     fa.perm = perm; fa.pair_pos = pair_pos; fa.work = work; fa.n_work = n_work;
     fa.active = active_experts; fa.n_active = n_active;
     fa.sync = reinterpret_cast<uint32_t*>(ws + L.sync);
+    fa.idt = reinterpret_cast<unsigned long long*>(fa.sync + fused_idt_word_offset(E, ns, I));
     fa.hbuf = hbuf; fa.ybuf = ybuf; fa.out = out;
     fa.partial = reinterpret_cast<float*>(ws + L.partial);
     const size_t smem_max = 227 * 1024;

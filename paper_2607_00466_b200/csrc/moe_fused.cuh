@@ -58,8 +58,16 @@ constexpr int kSyncTile = kSyncGroup + 32;      // [32][32]  gate logit tile wri
 constexpr int kSyncPartial = kSyncTile + 1024;  // [4][256]  per (sub-phase, CTA) "partial accumulators parked"
 constexpr int kSyncHReady = kSyncPartial + 1024; // [(E+ns)*2*tilesA] per phase-A tile "h tile written"
 
+// Tagged ids: one 64-bit word {epoch : 32 | four expert ids, one byte each : 32} per (token, group of four top-k
+// slots), written by the token group's owner after its top-k and polled by every CTA.  Tag and payload arrive in one
+// atomic 8-byte access, so the routing input needs no flag, no release and no second L2 round trip.  (The same
+// scheme for the logits was measured slower than tile flags + plain loads and is not used.)
+constexpr int kIdWordsPerTok = 4;         // kMaxTopK / 4
+__host__ __device__ inline size_t fused_idt_word_offset(int E, int ns, int I) {
+  return ((size_t)kSyncHReady + (size_t)(E + ns) * 2 * ((I + 63) / 64) + 1) & ~(size_t)1;
+}
 __host__ __device__ inline size_t fused_sync_words(int E, int ns, int I) {
-  return (size_t)kSyncHReady + (size_t)(E + ns) * 2 * ((I + 63) / 64);
+  return fused_idt_word_offset(E, ns, I) + (size_t)kFusedMaxT * kIdWordsPerTok * 2;
 }
 __host__ __device__ inline size_t fused_partial_bytes(int n_cta) {
   return (size_t)4 * n_cta * 128 * kNPCap * 4;
@@ -80,6 +88,7 @@ struct FusedArgs {
   int32_t* active;
   int32_t* n_active;
   uint32_t* sync;
+  unsigned long long* idt;     // [T][4] tagged top-k ids (inside the sync region)
   float* partial;              // [4][gridDim.x][128][kNPCap] fp32 scratch of the stream-K fix-up
   uint16_t* hbuf;              // [T*(k+ns), I] bf16
   float* ybuf;                 // [T*(k+ns), H] fp32
@@ -153,6 +162,14 @@ __device__ __forceinline__ bool warp_test_flags(const uint32_t* flags, int n, ui
   return __all_sync(0xffffffffu, ok);
 }
 
+__device__ __forceinline__ void st_relaxed_u64(unsigned long long* p, unsigned long long v) {
+  asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" :: "l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ unsigned long long ld_relaxed_u64(const unsigned long long* p) {
+  unsigned long long v;
+  asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+  return v;
+}
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(dst), "l"(src) : "memory");
 }
@@ -360,37 +377,23 @@ __device__ __forceinline__ void fused_route_a(const FusedArgs& a, const FusedSme
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const bool do_sig = is_cta0 && a.force_routing;
 
-  // ids: all loads in flight before the first use
-  constexpr int kIdsPer = 4;
-  int idr[kIdsPer];
-#pragma unroll
-  for (int j = 0; j < kIdsPer; ++j) {
-    const int p = tid + j * kFusedThreads;
-    idr[j] = (p < T * k) ? __ldcg(a.tk.ids + p) : 0;
-  }
   for (int i = tid; i < E * W; i += kFusedThreads) mask[i] = 0u;
-  __syncthreads();
-  for (int p0 = 0; p0 < T * k; p0 += kIdsPer * kFusedThreads) {
-    if (p0 > 0) {
-#pragma unroll
-      for (int j = 0; j < kIdsPer; ++j) {
-        const int p = p0 + tid + j * kFusedThreads;
-        idr[j] = (p < T * k) ? __ldcg(a.tk.ids + p) : 0;
-      }
-    }
-#pragma unroll
-    for (int j = 0; j < kIdsPer; ++j) {
-      const int p = p0 + tid + j * kFusedThreads;
-      if (p < T * k) {
+  if (a.force_routing) {
+    // ids were given: bring them into the shared-memory table the tagged-ids poll would have filled
+    for (int p = tid; p < T * k; p += kFusedThreads) {
+      const int id = min(max(__ldcg(a.tk.ids + p), 0), E - 1);
+      sm.ids8[p] = (uint8_t)id;
+      if (do_sig) {
         const int t = p / k;
-        const int id = min(max(idr[j], 0), E - 1);
-        sm.ids8[p] = (uint8_t)id;
-        atomicOr(&mask[id * W + (t >> 5)], 1u << (t & 31));
-        if (do_sig)
-          sig_add(a.tk.sig_req, a.tk.sig_block, a.tk.token_req ? a.tk.token_req[t] : -1,
-                  a.tk.token_block ? a.tk.token_block[t] : -1, a.tk.L, a.tk.layer, E, id);
+        sig_add(a.tk.sig_req, a.tk.sig_block, a.tk.token_req ? a.tk.token_req[t] : -1,
+                a.tk.token_block ? a.tk.token_block[t] : -1, a.tk.L, a.tk.layer, E, id);
       }
     }
+  }
+  __syncthreads();
+  for (int p = tid; p < T * k; p += kFusedThreads) {
+    const int t = p / k;
+    atomicOr(&mask[(int)sm.ids8[p] * W + (t >> 5)], 1u << (t & 31));
   }
   __syncthreads();
   for (int e = tid; e < E; e += kFusedThreads) {
@@ -661,13 +664,20 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
       if (tid == 0) flag_release(a.sync + kSyncTile + g * 32 + et, epoch);    // cumulative over the barrier
     }
     if (tid == 0) FSTAMP2(12);
-    for (int g = ((cta - n_tiles % G) + G) % G; g < n_gr; g += G) {       // owner(g) = (n_tiles + g) % G
+    // owner of token group g: waits for the group's logit tiles, warp w runs the top-k of token 8g + w and writes the
+    // ABI outputs, the signature increments and the tagged ids words every CTA routes from
+    for (int g = ((cta - n_tiles % G) + G) % G; g < n_gr; g += G) {     // owner(g) = (n_tiles + g) % G: CTAs without a gate tile first
       if (warp == 0) warp_wait_flags(a.sync + kSyncTile + g * 32, n_et, epoch, lane);
       __syncthreads();
       const int t = g * kGateTok + warp;
       if (t < T) {
         int id; float w;
         warp_topk_redux(a.tk.z + (size_t)t * E, E, k, a.tk.renorm, lane, id, w);
+        const uint32_t b = lane < k ? (uint32_t)id : 0u;
+        const uint32_t packed = b | (__shfl_down_sync(0xffffffffu, b, 1) << 8) | (__shfl_down_sync(0xffffffffu, b, 2) << 16) |
+                                (__shfl_down_sync(0xffffffffu, b, 3) << 24);
+        if ((lane & 3) == 0 && lane < k)
+          st_relaxed_u64(a.idt + (size_t)t * kIdWordsPerTok + (lane >> 2), ((unsigned long long)epoch << 32) | packed);
         if (lane < k) {
           a.tk.ids[(size_t)t * k + lane] = id;
           a.tk.w[(size_t)t * k + lane] = w;
@@ -675,11 +685,27 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
                   a.tk.token_block ? a.tk.token_block[t] : -1, a.tk.L, a.tk.layer, E, id);
         }
       }
-      __syncthreads();
-      if (tid == 0) flag_release(a.sync + kSyncGroup + g, epoch);
     }
     if (tid == 0) FSTAMP2(13);
-    if (warp == 0) warp_wait_flags(a.sync + kSyncGroup, n_gr, epoch, lane);
+    // every CTA: poll the tagged ids of all tokens into the shared-memory id table
+    {
+      const int wpt = (k + 3) >> 2;
+      const int n_words = T * wpt;
+      for (int i = tid; i < n_words; i += kFusedThreads) {
+        const int t = i / wpt, q = i - t * wpt;
+        const unsigned long long* src = a.idt + (size_t)t * kIdWordsPerTok + q;
+        unsigned long long v = ld_relaxed_u64(src);
+        uint32_t spins = 0;
+        while ((uint32_t)(v >> 32) != epoch) {
+          __nanosleep(40);
+          v = ld_relaxed_u64(src);
+          if (++spins > (1u << 24)) __trap();
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+          if (4 * q + j < k) sm.ids8[t * k + 4 * q + j] = (uint8_t)min((int)((v >> (8 * j)) & 0xffu), E - 1);
+      }
+    }
     __syncthreads();
     if (tid == 0) FSTAMP2(14);
   }
