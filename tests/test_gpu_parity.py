@@ -438,3 +438,40 @@ def test_fused_kernel_back_to_back_steps_and_graph_capture(gpu, oracle, qwen_lay
         torch.cuda.synchronize()
         assert torch.equal(dl.out[:T].view(torch.int16), ref[u].view(torch.int16))
         assert int(dl.n_active.item()) == 16
+
+
+@pytest.mark.parametrize("min_rounds", [1, 1 << 20])
+def test_schedule_variants_match_oracle_and_each_other(gpu, oracle, qwen_layer, min_rounds):
+    """The fused kernel's two schedules -- whole tile rounds drawn dynamically from a global counter (forced here
+    for every phase with at least ONE round) and the static stream-K cut of the whole phase -- must pass the same
+    parity gates, and each must be run-to-run bit-identical: the K order inside a tile and the fix-up order are
+    fixed, so it does not matter WHICH CTA draws a tile.  (Across the two schedules the fp32 sums are grouped
+    differently -- a tile is whole in one and split in the other -- so they agree to rounding, not bit for bit.)
+    Also on a small ragged layer with shared experts and a multi-pass expert, where every phase is shorter than
+    one round."""
+    import torch
+    shape, lw, dl = qwen_layer
+    T = 64
+    gpu.eldr_moe_set_option(gpu.OPT_DP_MIN_ROUNDS, min_rounds)
+    try:
+        for u in (16, 96):
+            xb, bias = synth.union_case(shape, T, u, synth.accepted_union_seed(T, u))
+            token_req, token_block = synth.decode_maps(T)
+            r = run_case(gpu, oracle, shape, lw, xb, bias, token_req, token_block, n_req=T, n_blk=T, layer_obj=dl)
+            assert gpu.eldr_moe_last_launch_count() == 1 and r["n_active"] == u
+            first = dl.run(gpu.bf16_from_bits(xb), torch.from_numpy(bias).cuda()).clone()
+            for _ in range(5):
+                again = dl.run(gpu.bf16_from_bits(xb), torch.from_numpy(bias).cuda())
+                assert torch.equal(again.view(torch.int16), first.view(torch.int16))
+        small = synth.MoEShape(hidden=512, inter=256, n_experts=8, top_k=2, n_shared=1, n_layers=1)
+        slw = synth.make_layer_weights(small, 77, w_std=0.05, gate_std=0.2)
+        run_case(gpu, oracle, small, slw, synth.make_hidden(200, small.hidden, 77))
+        assert gpu.eldr_moe_last_launch_count() == 1
+    finally:
+        gpu.eldr_moe_set_option(gpu.OPT_DP_MIN_ROUNDS, 4)
+
+
+def test_invalid_option_values_are_rejected(gpu):
+    for key, value in ((gpu.OPT_DP_MIN_ROUNDS, 0), (gpu.OPT_RING_KB, 16), (99, 1)):
+        with pytest.raises(RuntimeError):
+            gpu.eldr_moe_set_option(key, value)
