@@ -596,21 +596,44 @@ int32_t eldr_moe_decode_layer_host(const eldr_moe_shape_t* s, int32_t layer, int
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   uint8_t* ws = static_cast<uint8_t*>(workspace);
   const size_t H = s->hidden, k = s->top_k;
+  // Pinned (page-locked, mapped) host buffers are used in place by the kernels: the small inputs (token maps) are
+  // read and out / n_active are written straight through the mapping, so the step is one host-to-device copy
+  // (x, which the kernels read many times), the launch, two small device-to-host copies (ids, weights, which the
+  // kernels read back) and one synchronisation -- three copies instead of seven.
+  // Pageable buffers fall back to staged copies.
+  auto mapped = [](const void* h) -> void* {
+    if (!h) return nullptr;
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, h) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    return (at.type == cudaMemoryTypeHost && at.devicePointer && aligned16(at.devicePointer)) ? at.devicePointer : nullptr;
+  };
+  int32_t* d_req = static_cast<int32_t*>(mapped(h_token_req));
+  int32_t* d_blk = static_cast<int32_t*>(mapped(h_token_block));
+  eldr_bf16* d_out = static_cast<eldr_bf16*>(mapped(h_out));
+  int32_t* d_ids = nullptr;      // ids / weights are read back by the step's own kernels (routing, combine): they
+  float* d_w = nullptr;          // stay in device memory and are copied out
+  int32_t* d_na = static_cast<int32_t*>(mapped(h_n_active));
   if (!cuda_ok(cudaMemcpyAsync(ws + S.x, h_x, (size_t)T * H * 2, cudaMemcpyHostToDevice, st), "H2D x")) return ELDR_ERR_CUDA;
-  if (h_token_req && !cuda_ok(cudaMemcpyAsync(ws + S.req, h_token_req, (size_t)T * 4, cudaMemcpyHostToDevice, st), "H2D req")) return ELDR_ERR_CUDA;
-  if (h_token_block && !cuda_ok(cudaMemcpyAsync(ws + S.blk, h_token_block, (size_t)T * 4, cudaMemcpyHostToDevice, st), "H2D blk")) return ELDR_ERR_CUDA;
+  if (h_token_req && !d_req) {
+    if (!cuda_ok(cudaMemcpyAsync(ws + S.req, h_token_req, (size_t)T * 4, cudaMemcpyHostToDevice, st), "H2D req")) return ELDR_ERR_CUDA;
+    d_req = reinterpret_cast<int32_t*>(ws + S.req);
+  }
+  if (h_token_block && !d_blk) {
+    if (!cuda_ok(cudaMemcpyAsync(ws + S.blk, h_token_block, (size_t)T * 4, cudaMemcpyHostToDevice, st), "H2D blk")) return ELDR_ERR_CUDA;
+    d_blk = reinterpret_cast<int32_t*>(ws + S.blk);
+  }
   rc = eldr_moe_decode_layer(s, layer, T, reinterpret_cast<eldr_bf16*>(ws + S.x), gate_w, gate_bias, w13, w2,
-                             shared_w13, shared_w2, reinterpret_cast<eldr_bf16*>(ws + S.out),
-                             reinterpret_cast<int32_t*>(ws + S.ids), reinterpret_cast<float*>(ws + S.w), 0,
-                             reinterpret_cast<int32_t*>(ws + S.active), reinterpret_cast<int32_t*>(ws + S.n_active),
-                             h_token_req ? reinterpret_cast<int32_t*>(ws + S.req) : nullptr,
-                             h_token_block ? reinterpret_cast<int32_t*>(ws + S.blk) : nullptr, sig_req, sig_block,
-                             workspace, L.total, stream);
+                             shared_w13, shared_w2, d_out ? d_out : reinterpret_cast<eldr_bf16*>(ws + S.out),
+                             d_ids ? d_ids : reinterpret_cast<int32_t*>(ws + S.ids),
+                             d_w ? d_w : reinterpret_cast<float*>(ws + S.w), 0,
+                             reinterpret_cast<int32_t*>(ws + S.active),
+                             d_na ? d_na : reinterpret_cast<int32_t*>(ws + S.n_active),
+                             d_req, d_blk, sig_req, sig_block, workspace, L.total, stream);
   if (rc != ELDR_OK) return rc;
-  if (!cuda_ok(cudaMemcpyAsync(h_out, ws + S.out, (size_t)T * H * 2, cudaMemcpyDeviceToHost, st), "D2H out")) return ELDR_ERR_CUDA;
-  if (h_topk_ids && !cuda_ok(cudaMemcpyAsync(h_topk_ids, ws + S.ids, (size_t)T * k * 4, cudaMemcpyDeviceToHost, st), "D2H ids")) return ELDR_ERR_CUDA;
-  if (h_topk_w && !cuda_ok(cudaMemcpyAsync(h_topk_w, ws + S.w, (size_t)T * k * 4, cudaMemcpyDeviceToHost, st), "D2H w")) return ELDR_ERR_CUDA;
-  if (h_n_active && !cuda_ok(cudaMemcpyAsync(h_n_active, ws + S.n_active, 4, cudaMemcpyDeviceToHost, st), "D2H n_active")) return ELDR_ERR_CUDA;
+  if (!d_out && !cuda_ok(cudaMemcpyAsync(h_out, ws + S.out, (size_t)T * H * 2, cudaMemcpyDeviceToHost, st), "D2H out")) return ELDR_ERR_CUDA;
+  if (h_topk_ids && !d_ids && !cuda_ok(cudaMemcpyAsync(h_topk_ids, ws + S.ids, (size_t)T * k * 4, cudaMemcpyDeviceToHost, st), "D2H ids")) return ELDR_ERR_CUDA;
+  if (h_topk_w && !d_w && !cuda_ok(cudaMemcpyAsync(h_topk_w, ws + S.w, (size_t)T * k * 4, cudaMemcpyDeviceToHost, st), "D2H w")) return ELDR_ERR_CUDA;
+  if (h_n_active && !d_na && !cuda_ok(cudaMemcpyAsync(h_n_active, ws + S.n_active, 4, cudaMemcpyDeviceToHost, st), "D2H n_active")) return ELDR_ERR_CUDA;
   if (!cuda_ok(cudaStreamSynchronize(st), "stream sync")) return ELDR_ERR_CUDA;
   return ELDR_OK;
 }
