@@ -576,6 +576,16 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
   return ELDR_OK;
 }
 
+// ids / weights of the step copied from device memory into MAPPED pinned host buffers by one small block (a
+// kernel in the stream costs ~3 us; two cudaMemcpyAsync of 2 KB each cost ~12 us of stream time).
+__global__ void mirror_to_host_kernel(const int32_t* __restrict__ ids, int32_t* __restrict__ h_ids,
+                                      const float* __restrict__ w, float* __restrict__ h_w, int n) {
+  for (int i = threadIdx.x; i < n; i += blockDim.x) {
+    if (h_ids) h_ids[i] = ids[i];
+    if (h_w) h_w[i] = w[i];
+  }
+}
+
 int32_t eldr_moe_decode_layer_host(const eldr_moe_shape_t* s, int32_t layer, int32_t T, const eldr_bf16* h_x,
                                    const float* gate_w, const float* gate_bias, const eldr_bf16* w13,
                                    const eldr_bf16* w2, const eldr_bf16* shared_w13, const eldr_bf16* shared_w2,
@@ -598,8 +608,8 @@ int32_t eldr_moe_decode_layer_host(const eldr_moe_shape_t* s, int32_t layer, int
   const size_t H = s->hidden, k = s->top_k;
   // Pinned (page-locked, mapped) host buffers are used in place by the kernels: the small inputs (token maps) are
   // read and out / n_active are written straight through the mapping, so the step is one host-to-device copy
-  // (x, which the kernels read many times), the launch, two small device-to-host copies (ids, weights, which the
-  // kernels read back) and one synchronisation -- three copies instead of seven.
+  // (x, which the kernels read many times), the launch, one small block that mirrors ids / weights (which the
+  // kernels read back, so they stay in device memory) into the mapped buffers, and one synchronisation.
   // Pageable buffers fall back to staged copies.
   auto mapped = [](const void* h) -> void* {
     if (!h) return nullptr;
@@ -631,8 +641,15 @@ int32_t eldr_moe_decode_layer_host(const eldr_moe_shape_t* s, int32_t layer, int
                              d_req, d_blk, sig_req, sig_block, workspace, L.total, stream);
   if (rc != ELDR_OK) return rc;
   if (!d_out && !cuda_ok(cudaMemcpyAsync(h_out, ws + S.out, (size_t)T * H * 2, cudaMemcpyDeviceToHost, st), "D2H out")) return ELDR_ERR_CUDA;
-  if (h_topk_ids && !d_ids && !cuda_ok(cudaMemcpyAsync(h_topk_ids, ws + S.ids, (size_t)T * k * 4, cudaMemcpyDeviceToHost, st), "D2H ids")) return ELDR_ERR_CUDA;
-  if (h_topk_w && !d_w && !cuda_ok(cudaMemcpyAsync(h_topk_w, ws + S.w, (size_t)T * k * 4, cudaMemcpyDeviceToHost, st), "D2H w")) return ELDR_ERR_CUDA;
+  int32_t* m_ids = static_cast<int32_t*>(mapped(h_topk_ids));
+  float* m_w = static_cast<float*>(mapped(h_topk_w));
+  if (m_ids || m_w) {
+    mirror_to_host_kernel<<<1, 256, 0, st>>>(reinterpret_cast<const int32_t*>(ws + S.ids), m_ids,
+                                             reinterpret_cast<const float*>(ws + S.w), m_w, (int)(T * k));
+    if (!cuda_ok(cudaGetLastError(), "mirror_to_host_kernel")) return ELDR_ERR_CUDA;
+  }
+  if (h_topk_ids && !m_ids && !cuda_ok(cudaMemcpyAsync(h_topk_ids, ws + S.ids, (size_t)T * k * 4, cudaMemcpyDeviceToHost, st), "D2H ids")) return ELDR_ERR_CUDA;
+  if (h_topk_w && !m_w && !cuda_ok(cudaMemcpyAsync(h_topk_w, ws + S.w, (size_t)T * k * 4, cudaMemcpyDeviceToHost, st), "D2H w")) return ELDR_ERR_CUDA;
   if (h_n_active && !d_na && !cuda_ok(cudaMemcpyAsync(h_n_active, ws + S.n_active, 4, cudaMemcpyDeviceToHost, st), "D2H n_active")) return ELDR_ERR_CUDA;
   if (!cuda_ok(cudaStreamSynchronize(st), "stream sync")) return ELDR_ERR_CUDA;
   return ELDR_OK;
