@@ -313,3 +313,80 @@ int oracle_signature_readout(const oracle_shape_t *s, const int32_t *block_ids, 
   }
   return 0;
 }
+
+/* ------------------------------------------------------------------------------------------------
+ * signature -> routing decision ("Four steps build s_r",
+ * PAPER.md:239 "locality-band routing").  Followed step by step in the paper's order and notation:
+ *
+ *   2. downweight: c~_r(l,e) = c_r(l,e) * w(l,e), w(l,e) = log((|C|+1)/(df(l,e)+1))
+ *   3. select layers: x_r = [c~_r(l)]_{l in S}
+ *   4. normalise: s_r = x_r / ||x_r||_2                                                    (Eq. 2)
+ *   routing: s_k = cosine(s_r, centroid_k); s* = max_k s_k; among workers with s_k >= s* - tau pick
+ *            the one with the smallest load (in-flight decode requests), then load += 1
+ *
+ * Readings where the paper is silent: requests of one call are routed in index order and
+ * each sees the loads left by the previous ones ("updated as requests are dispatched"); equal loads in
+ * the band -> the larger similarity, then the lower worker index; an all-zero x_r (or centroid) has
+ * similarity 0 to everything; centroids need not arrive normalised (cosine divides by both norms) and
+ * their entries on layers outside S are ignored.
+ * Pins (tests/test_route_pins.py): tau = 0 => argmax cosine (numpy); tau = 1 on non-negative vectors =>
+ * join-shortest-queue; scale invariance of Eq. 2; masked layers do not matter; IDF closed form; the
+ * hand-worked 2-expert example in tests/golden/route_example.txt.
+ */
+void oracle_idf_table(int32_t n, const int32_t *df, int32_t n_calib, double *w) {
+  for (int32_t i = 0; i < n; ++i) w[i] = log(((double)n_calib + 1.0) / ((double)df[i] + 1.0));
+}
+
+int oracle_route_decide(int32_t R, int32_t L, int32_t E, int32_t K, const int32_t *counts /*[R,L,E]*/,
+                        const double *idf /*[L,E]*/, const uint8_t *layer_mask /*[L]*/,
+                        const double *centroids /*[K,L,E]*/, int64_t *loads /*[K] in/out*/, double tau,
+                        int32_t *worker /*[R]*/, double *sims /*[R,K]*/, double *band_gap /*[R] or NULL*/) {
+  if (R < 0 || L <= 0 || E <= 0 || K <= 0) return -1;
+  const size_t D = (size_t)L * E;
+  double *x = (double *)malloc(D * sizeof(double));
+  if (!x) return -2;
+  for (int32_t r = 0; r < R; ++r) {
+    double xn = 0.0;
+    for (int32_t l = 0; l < L; ++l)
+      for (int32_t e = 0; e < E; ++e) {
+        const size_t i = (size_t)l * E + e;
+        x[i] = layer_mask[l] ? (double)counts[(size_t)r * D + i] * idf[i] : 0.0;
+        xn += x[i] * x[i];
+      }
+    xn = sqrt(xn);
+    double best = -2.0;
+    for (int32_t k = 0; k < K; ++k) {
+      double dot = 0.0, cn = 0.0;
+      for (int32_t l = 0; l < L; ++l) {
+        if (!layer_mask[l]) continue;
+        for (int32_t e = 0; e < E; ++e) {
+          const size_t i = (size_t)l * E + e;
+          const double c = centroids[(size_t)k * D + i];
+          dot += (x[i] / (xn > 0.0 ? xn : 1.0)) * c;          /* s_r . centroid_k with s_r = x_r/||x_r|| (Eq. 2) */
+          cn += c * c;
+        }
+      }
+      cn = sqrt(cn);
+      const double s = (xn > 0.0 && cn > 0.0) ? dot / cn : 0.0;
+      sims[(size_t)r * K + k] = s;
+      if (s > best) best = s;
+    }
+    int32_t pick = -1;
+    double gap = 1e300;                                        /* distance of the nearest similarity to the band edge */
+    for (int32_t k = 0; k < K; ++k) {
+      const double s = sims[(size_t)r * K + k];
+      const double d = fabs(s - (best - tau));
+      if (d < gap) gap = d;
+      if (s >= best - tau) {
+        if (pick < 0 || loads[k] < loads[pick] ||
+            (loads[k] == loads[pick] && s > sims[(size_t)r * K + pick]))
+          pick = k;
+      }
+    }
+    worker[r] = pick;
+    loads[pick] += 1;
+    if (band_gap) band_gap[r] = gap;
+  }
+  free(x);
+  return 0;
+}

@@ -163,3 +163,32 @@ def signature_readout(shape, block_ids, sig_block):
     lib().oracle_signature_readout(C.byref(s), _p(block_ids), C.c_int32(len(block_ids)),
                                    _p(sig_block, np.int8), _p(out))
     return out
+
+
+# ---------------------------------------------------------------- routing decision
+def idf_table(df: np.ndarray, n_calib: int) -> np.ndarray:
+    """w(l,e) = log((|C|+1)/(df(l,e)+1)).  df int32 [L,E] -> float64 [L,E]."""
+    df = np.ascontiguousarray(df, dtype=np.int32)
+    w = np.empty(df.shape, dtype=np.float64)
+    lib().oracle_idf_table(C.c_int32(df.size), _p(df), C.c_int32(n_calib), _p(w))
+    return w
+
+
+def route_decide(counts: np.ndarray, idf: np.ndarray, layer_mask: np.ndarray, centroids: np.ndarray,
+                 loads: np.ndarray, tau: float):
+    """Locality-band routing of R requests in index order (PAPER.md:196-203, :239).  counts int32 [R,L,E];
+    idf float64 [L,E]; layer_mask uint8 [L]; centroids float64 [K,L,E]; loads int64 [K] (updated IN PLACE).
+    Returns dict(worker [R] int32, sims [R,K] float64, band_gap [R] float64 = distance of the nearest similarity
+    to the band edge s* - tau, for near-tie reporting)."""
+    R, L, E = counts.shape
+    K = centroids.shape[0]
+    assert counts.dtype == np.int32 and idf.dtype == np.float64 and centroids.dtype == np.float64
+    assert layer_mask.dtype == np.uint8 and loads.dtype == np.int64
+    worker = np.empty((R,), np.int32)
+    sims = np.empty((R, K), np.float64)
+    gap = np.empty((R,), np.float64)
+    rc = lib().oracle_route_decide(C.c_int32(R), C.c_int32(L), C.c_int32(E), C.c_int32(K), _p(counts), _p(idf),
+                                   _p(layer_mask), _p(centroids), _p(loads), C.c_double(tau), _p(worker),
+                                   _p(sims), _p(gap))
+    assert rc == 0, rc
+    return dict(worker=worker, sims=sims, band_gap=gap)

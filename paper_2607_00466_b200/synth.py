@@ -299,3 +299,44 @@ def accepted_union_seed(T: int, u: int) -> int:
     with open(path) as f:
         table = json.load(f)
     return int(table["T%d_u%d" % (T, u)]["seed"])
+
+
+# ------------------------------------------------------------------ routing-decision inputs
+@dataclasses.dataclass
+class RouteWorkload:
+    counts: np.ndarray       # [R,L,E] int32 per-request expert counts (what eldr_signature_readout returns)
+    df: np.ndarray           # [L,E] int32 document frequencies of a calibration corpus of n_calib requests
+    n_calib: int
+    layer_mask: np.ndarray   # [L] uint8, the kept layers S
+    centroids: np.ndarray    # [K,L,E] float32, non-negative, NOT normalised
+    loads: np.ndarray        # [K] int32 in-flight decode requests per worker
+    domain: np.ndarray       # [R] which prototype the request was drawn around
+
+
+def make_route_workload(R: int, L: int, E: int, K: int, k: int, seed: int, prompt_len=(512, 4096),
+                        keep_layers: Optional[int] = None) -> RouteWorkload:
+    """Stand-in for calibration artefacts and prefill signatures (the paper's corpora are not available offline):
+    K non-negative prototypes over (layer, expert) with a few dominant "specialist" experts per layer and a few
+    "generalist" experts shared by all; each request draws its prompt length and, per layer, multinomial counts of
+    len*k picks around its domain's prototype; df is a seeded table that is large on the generalists."""
+    g = np.random.default_rng(sub_seed(seed, "route", R, L, E, K))
+    proto = g.random((K, L, E)) ** 4                       # skewed: a few specialists per (prototype, layer)
+    generalists = g.permutation(E)[: max(1, E // 16)]
+    proto[:, :, generalists] += 2.0
+    centroids = (proto + 0.05 * g.random((K, L, E))).astype(np.float32)
+    domain = g.integers(0, K, size=R)
+    lens = g.integers(prompt_len[0], prompt_len[1] + 1, size=R)
+    counts = np.empty((R, L, E), np.int32)
+    for r in range(R):
+        p = proto[domain[r]] + 0.02
+        p = p / p.sum(axis=1, keepdims=True)
+        for l in range(L):
+            counts[r, l] = g.multinomial(int(lens[r]) * k, p[l]).astype(np.int32)
+    n_calib = 1000
+    df = g.integers(1, n_calib // 4, size=(L, E)).astype(np.int32)
+    df[:, generalists] = n_calib - g.integers(0, 5, size=(L, generalists.size)).astype(np.int32)
+    mask = np.zeros(L, np.uint8)
+    keep = keep_layers if keep_layers is not None else max(1, (2 * L) // 3)
+    mask[g.permutation(L)[:keep]] = 1
+    loads = g.integers(0, 6, size=K).astype(np.int32)
+    return RouteWorkload(counts, df, n_calib, mask, centroids, loads, domain)
