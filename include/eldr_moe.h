@@ -150,6 +150,22 @@ int32_t eldr_signature_readout(const eldr_moe_shape_t* shape, const int32_t* blo
                                const int32_t* req_off, int32_t n_req, const int8_t* sig_block,
                                int32_t* sig_out, eldr_stream_t stream);
 
+/* Signature -> routing decision for R requests.  PAPER.md:196-203: reweight the counts by
+ * the IDF table (step 2), keep the layers of the mask S (step 3), normalise (Eq. 2); PAPER.md:239 locality-band
+ * routing: s_k = cosine(s_r, centroid_k), s* = max_k s_k, among workers with s_k >= s* - tau pick the one with the
+ * smallest load, then loads[pick] += 1.  Requests are routed in index order, each seeing the loads left by the
+ * previous ones; equal loads in the band -> larger similarity, then lower index; an all-zero signature (or
+ * centroid) has similarity 0 (readings).
+ *   sig_req [R,L,E] int32 in (what eldr_signature_readout wrote; L = shape->n_layers, E = shape->n_experts);
+ *   idf [L,E] fp32 in (w(l,e) = log((|C|+1)/(df(l,e)+1)), fit offline); layer_mask [L] uint8 in (1 = kept);
+ *   centroids [K,L,E] fp32 in (need not be normalised; entries on dropped layers ignored), 1 <= K <= 1024;
+ *   loads [K] int32 in/out (in-flight decode requests per worker); tau >= 0;
+ *   worker [R] int32 out; sims [R,K] fp32 out (the cosine similarities; required).
+ * All pointers are device pointers; two small launches on `stream`; no host sync; R == 0 is a no-op. */
+int32_t eldr_route_decide(const eldr_moe_shape_t* shape, int32_t R, int32_t K, const int32_t* sig_req,
+                          const float* idf, const uint8_t* layer_mask, const float* centroids, int32_t* loads,
+                          float tau, int32_t* worker, float* sims, eldr_stream_t stream);
+
 size_t  eldr_moe_workspace_bytes(const eldr_moe_shape_t* shape, int32_t max_T);
 size_t  eldr_moe_workspace_bytes_host(const eldr_moe_shape_t* shape, int32_t max_T);
 int32_t eldr_moe_workspace_layout(const eldr_moe_shape_t* shape, int32_t T, eldr_moe_ws_layout_t* layout);

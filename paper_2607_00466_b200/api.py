@@ -19,7 +19,7 @@ _lib = None
 
 EXPORTS = [
     "eldr_moe_gate_topk", "eldr_moe_decode_layer", "eldr_moe_decode_layer_host",
-    "eldr_signature_accumulate", "eldr_signature_reset_blocks", "eldr_signature_readout",
+    "eldr_signature_accumulate", "eldr_signature_reset_blocks", "eldr_signature_readout", "eldr_route_decide",
     "eldr_moe_workspace_bytes", "eldr_moe_workspace_bytes_host", "eldr_moe_workspace_layout",
     "eldr_moe_last_launch_count", "eldr_status_string", "eldr_last_cuda_error",
     "eldr_moe_profile_enable", "eldr_moe_profile_read", "eldr_moe_set_option",
@@ -209,6 +209,16 @@ def eldr_signature_readout(shape, block_ids, req_off, sig_block, sig_out):
     _check(load().eldr_signature_readout(C.byref(s), _ptr(block_ids, torch.int32), _ptr(req_off, torch.int32),
                                          C.c_int32(req_off.numel() - 1), _ptr(sig_block, torch.int8),
                                          _ptr(sig_out, torch.int32), _stream()), "eldr_signature_readout")
+
+
+def eldr_route_decide(shape, sig_req, idf, layer_mask, centroids, loads, tau: float, worker, sims):
+    s = make_shape(shape)
+    R, K = sig_req.shape[0], centroids.shape[0]
+    _check(load().eldr_route_decide(C.byref(s), C.c_int32(R), C.c_int32(K), _ptr(sig_req, torch.int32),
+                                    _ptr(idf, torch.float32), _ptr(layer_mask, torch.uint8),
+                                    _ptr(centroids, torch.float32), _ptr(loads, torch.int32), C.c_float(tau),
+                                    _ptr(worker, torch.int32), _ptr(sims, torch.float32), _stream()),
+           "eldr_route_decide")
 
 
 class DecodeLayer:

@@ -14,6 +14,7 @@
 #include "ffn_umma.cuh"
 #include "gate_route.cuh"
 #include "moe_fused.cuh"
+#include "route_decide.cuh"
 
 namespace {
 
@@ -696,6 +697,22 @@ int32_t eldr_signature_readout(const eldr_moe_shape_t* s, const int32_t* block_i
   sig_readout_kernel<<<grid, 256, 0, static_cast<cudaStream_t>(stream)>>>(block_ids, req_off, sig_block, sig_out,
                                                                        cells);
   return launch_ok("sig_readout_kernel") ? ELDR_OK : ELDR_ERR_CUDA;
+}
+
+int32_t eldr_route_decide(const eldr_moe_shape_t* s, int32_t R, int32_t K, const int32_t* sig_req, const float* idf,
+                          const uint8_t* layer_mask, const float* centroids, int32_t* loads, float tau,
+                          int32_t* worker, float* sims, eldr_stream_t stream) {
+  g_launches = 0;
+  int32_t rc = check_shape(s);
+  if (rc != ELDR_OK) return rc;
+  if (R < 0 || K < 1 || K > kRouteMaxWorkers || !(tau >= 0.f)) return ELDR_ERR_INVALID_ARG;
+  if (R == 0) return ELDR_OK;
+  if (!sig_req || !idf || !layer_mask || !centroids || !loads || !worker || !sims) return ELDR_ERR_INVALID_ARG;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  route_sims_kernel<<<R, 256, 0, st>>>(sig_req, idf, layer_mask, centroids, sims, s->n_layers, s->n_experts, K);
+  if (!launch_ok("route_sims_kernel")) return ELDR_ERR_CUDA;
+  route_pick_kernel<<<1, 32, 0, st>>>(sims, loads, worker, R, K, tau);
+  return launch_ok("route_pick_kernel") ? ELDR_OK : ELDR_ERR_CUDA;
 }
 
 }  // extern "C"

@@ -93,3 +93,18 @@ def test_binding_fails_loudly_when_library_is_missing(monkeypatch, tmp_path):
     monkeypatch.setattr(api._build, "LIB", str(tmp_path / "nope.so"))
     with pytest.raises(RuntimeError, match="no CPU fallback"):
         api.load()
+
+
+def test_route_decide_rejects_bad_arguments_without_a_gpu(lib):
+    api, so = lib
+    good = api.make_shape(synth.SHAPE_C1)
+    null, p = C.c_void_p(0), C.c_void_p(4096)
+
+    def call(R, K, tau, ptr):
+        return so.eldr_route_decide(C.byref(good), C.c_int32(R), C.c_int32(K), ptr, ptr, ptr, ptr, ptr, C.c_float(tau),
+                                    ptr, ptr, null)
+    assert call(0, 4, 0.1, null) == 0                 # R == 0 is a no-op
+    assert call(3, 4, 0.1, null) == -1                # null pointers
+    assert call(-1, 4, 0.1, p) == -1
+    assert call(3, 0, 0.1, p) == -1 and call(3, 1025, 0.1, p) == -1
+    assert call(3, 4, -0.5, p) == -1 and call(3, 4, float("nan"), p) == -1
