@@ -706,12 +706,18 @@ int32_t eldr_route_decide(const eldr_moe_shape_t* s, int32_t R, int32_t K, const
   int32_t rc = check_shape(s);
   if (rc != ELDR_OK) return rc;
   if (R < 0 || K < 1 || K > kRouteMaxWorkers || !(tau >= 0.f)) return ELDR_ERR_INVALID_ARG;
+  if (s->n_layers > kRouteMaxLayers) return ELDR_ERR_UNSUPPORTED;
   if (R == 0) return ELDR_OK;
   if (!sig_req || !idf || !layer_mask || !centroids || !loads || !worker || !sims) return ELDR_ERR_INVALID_ARG;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  route_sims_kernel<<<R, 256, 0, st>>>(sig_req, idf, layer_mask, centroids, sims, s->n_layers, s->n_experts, K);
+  static bool route_attr_set = false;
+  if (!route_attr_set) {
+    if (!set_smem(route_sims_kernel, kRouteStageCells * 4)) return ELDR_ERR_CUDA;
+    route_attr_set = true;
+  }
+  route_sims_kernel<<<dim3(R, (K + 7) / 8 < 16 ? (K + 7) / 8 : 16), 256, kRouteStageCells * 4, st>>>(sig_req, idf, layer_mask, centroids, sims, s->n_layers, s->n_experts, K);
   if (!launch_ok("route_sims_kernel")) return ELDR_ERR_CUDA;
-  route_pick_kernel<<<1, 32, 0, st>>>(sims, loads, worker, R, K, tau);
+  route_pick_kernel<<<1, kRoutePickThreads, 0, st>>>(sims, loads, worker, R, K, tau);
   return launch_ok("route_pick_kernel") ? ELDR_OK : ELDR_ERR_CUDA;
 }
 

@@ -4,7 +4,8 @@ of the HBM roofline, and the two derived checks -- union scaling fit t = a + b*|
 (config 3).  Config 4 runs the 48-layer stack on single-cluster vs mixed batches, config 5 the 27-layer
 shared-expert stack plus the prefill-shaped signature accumulation.
 
-  python -m paper_2607_00466_b200.report [--configs 2,3,4,5] [--steps K] > profiles/<name>.md
+  python -m paper_2607_00466_b200.report [--configs 2,3,4,5,6] [--steps K] > profiles/<name>.md
+(6 = the routing-decision row of SURVEY.md 8(f))
 
 Timing only (parity of the same configs against the oracle is tests/test_gpu_parity.py); Gate C invariants of
 SURVEY.md 8(c) are asserted on the GPU outputs of every row.  Needs a CUDA device; there is no CPU fallback.
@@ -299,9 +300,45 @@ def config_5(api, synth, steps):
     return lines, note
 
 
+def route_rows(api, synth):
+    """eldr_signature_readout + eldr_route_decide at the prefill -> decode handoff
+    (Qwen3-shaped signature space: 48 layers x 128 experts).  Latency-bound; reported in microseconds."""
+    import torch
+    L, E = 48, 128
+    shape = synth.MoEShape(hidden=2048, inter=768, n_experts=E, top_k=8, n_layers=L)
+    out = ["| requests R | workers K | kept layers | route_decide µs per call (20 calls back to back) | bytes read (counts + K centroids per request) | GB/s |",
+           "|---|---|---|---|---|---|"]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for R, K in ((1, 8), (32, 8), (256, 8), (256, 64)):
+        w = synth.make_route_workload(R, L, E, K, 8, seed=9, prompt_len=(512, 1024))
+        idf = torch.from_numpy(np.log((w.n_calib + 1.0) / (w.df + 1.0)).astype(np.float32)).cuda()   # input table
+        d = [torch.from_numpy(a).cuda() for a in (w.counts, w.layer_mask, w.centroids)]
+        loads0 = torch.from_numpy(w.loads).cuda()
+        worker = torch.zeros(R, dtype=torch.int32, device="cuda")
+        sims = torch.zeros((R, K), device="cuda")
+        ts = []
+        for i in range(8):
+            loads = loads0.clone()
+            torch.cuda.synchronize()
+            e0.record()
+            for _ in range(20):            # back to back, so that the device and not the host's enqueue rate is timed
+                api.eldr_route_decide(shape, d[0], idf, d[1], d[2], loads, 0.1, worker, sims)
+            e1.record()
+            torch.cuda.synchronize()
+            if i >= 2:
+                ts.append(e0.elapsed_time(e1) * 1e3 / 20)
+        assert int(loads.sum().item()) == int(loads0.sum().item()) + 20 * R
+        assert 0 <= int(worker.min().item()) and int(worker.max().item()) < K
+        kept = int(w.layer_mask.sum())
+        nbytes = R * kept * E * (4 + 4) + R * K * kept * E * 4
+        us = float(np.median(ts))
+        out.append("| %d | %d | %d of %d | %.1f | %.2f MB | %.0f |" % (R, K, kept, L, us, nbytes / 1e6, nbytes / us / 1e3))
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--configs", default="2,3,4,5")
+    ap.add_argument("--configs", default="2,3,4,5,6")
     ap.add_argument("--steps", type=int, default=50)
     args = ap.parse_args()
     which = {int(c) for c in args.configs.split(",")}
@@ -321,6 +358,12 @@ def main():
     if 4 in which:
         lines, note = config_4(api, synth, max(4, min(args.steps, 8)))
         print("## Config 4 (48-layer stack, 58 GB of expert weights resident)\n\n%s\n%s\n\n%s\n" % (HEADER, "\n".join(lines), note), flush=True)
+    if 6 in which:
+        print("## Routing decision (SURVEY.md 8(f) row 1: `eldr_route_decide`, tau = 0.1)\n\n%s\n\nTwo launches "
+              "(similarities: one CTA per request, one warp per centroid; picks: one warp walks the requests in "
+              "order because each decision sees the loads left by the previous one).  Latency-bound; the paper's "
+              "'Route (tau-JSQ)' step costs 0.15 ms per request on the proxy host (PAPER.md Table 1, context).\n" %
+              "\n".join(route_rows(api, synth)), flush=True)
     if 5 in which:
         lines, note = config_5(api, synth, min(args.steps, 10))
         print("## Config 5 (27 layers, 64 routed + 2 shared experts, 31 GB resident)\n\n%s\n%s\n\n%s\n" % (HEADER, "\n".join(lines), note), flush=True)
