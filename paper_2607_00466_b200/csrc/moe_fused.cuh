@@ -377,7 +377,7 @@ __device__ __forceinline__ void fused_route_a(const FusedArgs& a, const FusedSme
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const bool do_sig = is_cta0 && a.force_routing;
 
-  for (int i = tid; i < E * W; i += kFusedThreads) mask[i] = 0u;
+  // (the membership masks were zeroed in the kernel's prologue, before the gate)
   if (a.force_routing) {
     // ids were given: bring them into the shared-memory table the tagged-ids poll would have filled
     for (int p = tid; p < T * k; p += kFusedThreads) {
@@ -389,13 +389,15 @@ __device__ __forceinline__ void fused_route_a(const FusedArgs& a, const FusedSme
                 a.tk.token_block ? a.tk.token_block[t] : -1, a.tk.L, a.tk.layer, E, id);
       }
     }
+    __syncthreads();
   }
-  __syncthreads();
+  if (threadIdx.x == 0) FSTAMP2(4);
   for (int p = tid; p < T * k; p += kFusedThreads) {
     const int t = p / k;
     atomicOr(&mask[(int)sm.ids8[p] * W + (t >> 5)], 1u << (t & 31));
   }
   __syncthreads();
+  if (threadIdx.x == 0) FSTAMP2(5);
   for (int e = tid; e < E; e += kFusedThreads) {
     int run = 0;
     for (int w = 0; w < W; ++w) {
@@ -405,13 +407,15 @@ __device__ __forceinline__ void fused_route_a(const FusedArgs& a, const FusedSme
     s_cnt[e] = run;
   }
   __syncthreads();
+  if (threadIdx.x == 0) FSTAMP2(6);
   if (warp == 0) {
     constexpr int PER = kMaxExperts / 32;
+    const int per = (E + 31) >> 5;                  // experts per lane: all 32 lanes work whatever E is
     int c[PER], csum = 0, asum = 0, cmax = 0;
 #pragma unroll
     for (int i = 0; i < PER; ++i) {
-      const int e = lane * PER + i;
-      c[i] = (e < E) ? s_cnt[e] : 0;
+      const int e = lane * per + i;
+      c[i] = (i < per && e < E) ? s_cnt[e] : 0;
       csum += c[i];
       asum += (c[i] > 0);
       cmax = max(cmax, c[i]);
@@ -430,8 +434,8 @@ __device__ __forceinline__ void fused_route_a(const FusedArgs& a, const FusedSme
     const int total = __shfl_sync(0xffffffffu, cinc, 31);
 #pragma unroll
     for (int i = 0; i < PER; ++i) {
-      const int e = lane * PER + i;
-      if (e < E) {
+      const int e = lane * per + i;
+      if (i < per && e < E) {
         s_off[e] = coff;
         if (is_cta0) { a.off[e] = coff; a.cnt[e] = c[i]; }
         if (c[i] > 0) {
@@ -454,26 +458,34 @@ __device__ __forceinline__ void fused_route_a(const FusedArgs& a, const FusedSme
     // accumulator passes per entry (1 unless an expert got more than kNPCap tokens) and their exclusive scan
     const int n_work = n_act + ns;
     constexpr int PER2 = (kMaxExperts + 8 + 31) / 32;
-    int ps = 0;
+    int pinc;
+    if (cmax <= kNPCap) {
+      // every entry fits one accumulator pass (the usual decode case): the pass table is the identity
+      for (int ent = lane; ent < n_work; ent += 32) sm.cumpass[ent] = ent;
+      pinc = n_work;
+    } else {
+      int ps = 0;
 #pragma unroll
-    for (int i = 0; i < PER2; ++i) {
-      const int ent = lane * PER2 + i;
-      if (ent < n_work) ps += (sm.work[ent].w + kNPCap - 1) / kNPCap;
-    }
-    int pinc = ps;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const int pv = __shfl_up_sync(0xffffffffu, pinc, o);
-      if (lane >= o) pinc += pv;
-    }
-    int poff = pinc - ps;
-#pragma unroll
-    for (int i = 0; i < PER2; ++i) {
-      const int ent = lane * PER2 + i;
-      if (ent < n_work) {
-        sm.cumpass[ent] = poff;
-        poff += (sm.work[ent].w + kNPCap - 1) / kNPCap;
+      for (int i = 0; i < PER2; ++i) {
+        const int ent = lane * PER2 + i;
+        if (ent < n_work) ps += (sm.work[ent].w + kNPCap - 1) / kNPCap;
       }
+      pinc = ps;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int pv = __shfl_up_sync(0xffffffffu, pinc, o);
+        if (lane >= o) pinc += pv;
+      }
+      int poff = pinc - ps;
+#pragma unroll
+      for (int i = 0; i < PER2; ++i) {
+        const int ent = lane * PER2 + i;
+        if (ent < n_work) {
+          sm.cumpass[ent] = poff;
+          poff += (sm.work[ent].w + kNPCap - 1) / kNPCap;
+        }
+      }
+      pinc = __shfl_sync(0xffffffffu, pinc, 31);
     }
     if (lane == 31) sm.cumpass[n_work] = pinc;
     if (lane == 0) {
@@ -487,6 +499,7 @@ __device__ __forceinline__ void fused_route_a(const FusedArgs& a, const FusedSme
     if (lane == 31) sm.meta[3] = pinc;
   }
   __syncthreads();
+  if (threadIdx.x == 0) FSTAMP2(7);
 }
 
 // ---------------------------------------------------------------------- R (part b): token <-> position maps
@@ -640,6 +653,11 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
   tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(sm.tmem_slot));
+  {
+    // routing membership masks [E][W]: zeroed here, long before the ids arrive (ordered by the barriers in between)
+    uint32_t* mask0 = reinterpret_cast<uint32_t*>(sm.route_scratch);
+    for (int i = tid; i < E * ((T + 31) >> 5); i += kFusedThreads) mask0[i] = 0u;
+  }
   if (tid == 0) FSTAMP(0);
   pdl_launch_dependents();
   pdl_wait();
