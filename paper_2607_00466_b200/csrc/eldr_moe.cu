@@ -13,6 +13,7 @@
 #include "ffn_stream.cuh"
 #include "ffn_umma.cuh"
 #include "gate_route.cuh"
+#include "gate_prefill.cuh"
 #include "moe_fused.cuh"
 #include "route_decide.cuh"
 
@@ -349,10 +350,25 @@ int32_t eldr_moe_gate_topk(const eldr_moe_shape_t* s, int32_t layer, int32_t T, 
   if (workspace_bytes < align_up((size_t)T * s->n_experts * 4, 256)) return ELDR_ERR_WORKSPACE_SMALL;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   float* z = static_cast<float*>(workspace);
-  rc = launch_gate_logits(s, T, x, gate_w, gate_bias, z, st);
-  if (rc != ELDR_OK) return rc;
   TopkArgs a{z, topk_ids, topk_w, token_req, token_block, sig_req, sig_block,
              T, s->n_experts, s->top_k, s->n_layers, layer, s->renormalize};
+  if (T >= 2048 && s->hidden % kGpBK == 0) {
+    // prefill-shaped: register-tiled fp32 GEMM, split-K into the fewest slices of at most 256 h (accuracy, see
+    // gate_prefill.cuh); taken when the workspace holds the S partial logit tensors
+    const int chunks = s->hidden / kGpBK;
+    int S = 0;
+    for (int c = 1; c <= 64; ++c)
+      if (chunks % c == 0 && s->hidden / c <= 256) { S = c; break; }
+    if (S > 0 && workspace_bytes >= (size_t)S * T * s->n_experts * 4) {
+      gate_logits_tiled_kernel<<<dim3((T + kGpBM - 1) / kGpBM, (s->n_experts + kGpBN - 1) / kGpBN, S), kGpThreads, 0, st>>>(
+          x, gate_w, gate_bias, z, T, s->hidden, s->n_experts, s->hidden / S);
+      if (!launch_ok("gate_logits_tiled_kernel")) return ELDR_ERR_CUDA;
+      topk_splitk_kernel<<<(T + 7) / 8, 256, 0, st>>>(a, z, S);
+      return launch_ok("topk_splitk_kernel") ? ELDR_OK : ELDR_ERR_CUDA;
+    }
+  }
+  rc = launch_gate_logits(s, T, x, gate_w, gate_bias, z, st);
+  if (rc != ELDR_OK) return rc;
   topk_kernel<<<(T + 7) / 8, 256, 0, st>>>(a);
   return launch_ok("topk_kernel") ? ELDR_OK : ELDR_ERR_CUDA;
 }

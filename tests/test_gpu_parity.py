@@ -475,3 +475,37 @@ def test_invalid_option_values_are_rejected(gpu):
     for key, value in ((gpu.OPT_DP_MIN_ROUNDS, 0), (gpu.OPT_RING_KB, 16), (99, 1)):
         with pytest.raises(RuntimeError):
             gpu.eldr_moe_set_option(key, value)
+
+
+@pytest.mark.parametrize("H,E,k,T,big_ws", [(2048, 128, 8, 4096, True), (2048, 128, 8, 2100, False), (320, 130, 3, 2050, True),
+                                            (64, 10, 2, 2049, True), (1408, 64, 6, 3001, True)])
+def test_gate_prefill_tiled_gemm(gpu, oracle, H, E, k, T, big_ws):
+    """eldr_moe_gate_topk at prefill-shaped T (>= 2048 tokens takes the register-tiled fp32 GEMM with split-K):
+    logits within 1e-5 of the fp64 oracle, ids / weights / signatures through the same gates as the decode path;
+    ragged T, E and H, with a gate bias, with a workspace that only fits one K slice, and run-to-run bit-identical."""
+    import torch
+    shape = synth.MoEShape(hidden=H, inter=64, n_experts=E, top_k=k, n_layers=1)
+    gate_w = synth.make_gate_w(shape, 17)
+    x_bits = synth.make_hidden(T, H, 17)
+    bias = (np.random.default_rng(17).standard_normal(E) * 0.5).astype(np.float32)
+    nbytes = gpu.eldr_moe_workspace_bytes(shape, T) if big_ws else ((T * E * 4 + 255) // 256) * 256
+    ws = torch.zeros(nbytes, dtype=torch.uint8, device="cuda")
+    ids = torch.empty((T, k), dtype=torch.int32, device="cuda")
+    w = torch.empty((T, k), dtype=torch.float32, device="cuda")
+    sig_req = torch.zeros((4, 1, E), dtype=torch.int32, device="cuda")
+    token_req = torch.from_numpy((np.arange(T) % 4).astype(np.int32)).cuda()
+    args = (shape, 0, gpu.bf16_from_bits(x_bits), torch.from_numpy(gate_w).cuda(), torch.from_numpy(bias).cuda(), ids, w,
+            token_req, None, sig_req, None, ws)
+    gpu.eldr_moe_gate_topk(*args)
+    torch.cuda.synchronize()
+    assert gpu.eldr_moe_last_launch_count() == 2
+    ora = oracle.gate_topk(shape, x_bits, gate_w, bias)
+    z = ws[: T * E * 4].view(torch.float32).reshape(T, E).cpu().numpy().astype(np.float64)
+    assert np.abs(z - ora["z"]).max() <= 1e-5
+    clean = check_gate(shape, ora, ids.cpu().numpy(), w.cpu().numpy())
+    assert (~clean).sum() <= max(3, T // 500)
+    assert int(sig_req.sum().item()) == T * k
+    first = (ids.clone(), w.clone())
+    gpu.eldr_moe_gate_topk(*args)
+    torch.cuda.synchronize()
+    assert torch.equal(first[0], ids) and torch.equal(first[1].view(torch.int32), w.view(torch.int32))
