@@ -104,8 +104,16 @@ __global__ void __launch_bounds__(256) topk_splitk_kernel(TopkArgs a, float* __r
   float* zrow = zp + (size_t)t * a.E;
   if (n_slices > 1) {
     for (int e = lane; e < a.E; e += 32) {
-      float s = zrow[e];
-      for (int p = 1; p < n_slices; ++p) s += zp[(size_t)p * TE + (size_t)t * a.E + e];
+      // all partials of this logit requested before the first add (a dependent chain of loads costs one L2 round
+      // trip per slice); the adds stay in slice order
+      float v[8];
+      const int n8 = min(n_slices, 8);
+#pragma unroll
+      for (int p = 0; p < 8; ++p) v[p] = p < n8 ? __ldcg(zp + (size_t)p * TE + (size_t)t * a.E + e) : 0.f;
+      float s = v[0];
+#pragma unroll
+      for (int p = 1; p < 8; ++p) s += v[p];
+      for (int p = 8; p < n_slices; ++p) s += __ldcg(zp + (size_t)p * TE + (size_t)t * a.E + e);
       zrow[e] = s;
     }
     __syncwarp();
