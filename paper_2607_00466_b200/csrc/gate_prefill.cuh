@@ -44,12 +44,14 @@ gate_logits_tiled_kernel(const uint16_t* __restrict__ x, const float* __restrict
   };
   auto sstore = [&](int buf) {
     const int kk = lhalf * 8;
-    As[buf][kk + 0][lrow] = bf16_lo(ra.x); As[buf][kk + 1][lrow] = bf16_hi(ra.x);
-    As[buf][kk + 2][lrow] = bf16_lo(ra.y); As[buf][kk + 3][lrow] = bf16_hi(ra.y);
-    As[buf][kk + 4][lrow] = bf16_lo(ra.z); As[buf][kk + 5][lrow] = bf16_hi(ra.z);
-    As[buf][kk + 6][lrow] = bf16_lo(ra.w); As[buf][kk + 7][lrow] = bf16_hi(ra.w);
-    Bs[buf][kk + 0][lrow] = rb0.x; Bs[buf][kk + 1][lrow] = rb0.y; Bs[buf][kk + 2][lrow] = rb0.z; Bs[buf][kk + 3][lrow] = rb0.w;
-    Bs[buf][kk + 4][lrow] = rb1.x; Bs[buf][kk + 5][lrow] = rb1.y; Bs[buf][kk + 6][lrow] = rb1.z; Bs[buf][kk + 7][lrow] = rb1.w;
+    const int col = lrow ^ (lhalf << 4);            // rows 8..15 of a chunk live 16 columns over: the two halves of a warp
+                                                    // (same lrow, other lhalf) no longer store to the same bank
+    As[buf][kk + 0][col] = bf16_lo(ra.x); As[buf][kk + 1][col] = bf16_hi(ra.x);
+    As[buf][kk + 2][col] = bf16_lo(ra.y); As[buf][kk + 3][col] = bf16_hi(ra.y);
+    As[buf][kk + 4][col] = bf16_lo(ra.z); As[buf][kk + 5][col] = bf16_hi(ra.z);
+    As[buf][kk + 6][col] = bf16_lo(ra.w); As[buf][kk + 7][col] = bf16_hi(ra.w);
+    Bs[buf][kk + 0][col] = rb0.x; Bs[buf][kk + 1][col] = rb0.y; Bs[buf][kk + 2][col] = rb0.z; Bs[buf][kk + 3][col] = rb0.w;
+    Bs[buf][kk + 4][col] = rb1.x; Bs[buf][kk + 5][col] = rb1.y; Bs[buf][kk + 6][col] = rb1.z; Bs[buf][kk + 7][col] = rb1.w;
   };
   const int ty = tid >> 4, tx = tid & 15;          // rows ty*8.., columns tx*8..
   float acc[8][8];
@@ -66,10 +68,11 @@ gate_logits_tiled_kernel(const uint16_t* __restrict__ x, const float* __restrict
     if (it + 1 < n_it) gload(it + 1);               // in flight during the multiply
 #pragma unroll
     for (int kk = 0; kk < kGpBK; ++kk) {
-      const float4 a0 = *reinterpret_cast<const float4*>(&As[buf][kk][ty * 8]);
-      const float4 a1 = *reinterpret_cast<const float4*>(&As[buf][kk][ty * 8 + 4]);
-      const float4 b0 = *reinterpret_cast<const float4*>(&Bs[buf][kk][tx * 8]);
-      const float4 b1 = *reinterpret_cast<const float4*>(&Bs[buf][kk][tx * 8 + 4]);
+      const int sw = (kk & 8) << 1;                 // the store-side swizzle, a compile-time constant per kk
+      const float4 a0 = *reinterpret_cast<const float4*>(&As[buf][kk][(ty * 8) ^ sw]);
+      const float4 a1 = *reinterpret_cast<const float4*>(&As[buf][kk][((ty * 8) ^ sw) + 4]);
+      const float4 b0 = *reinterpret_cast<const float4*>(&Bs[buf][kk][(tx * 8) ^ sw]);
+      const float4 b1 = *reinterpret_cast<const float4*>(&Bs[buf][kk][((tx * 8) ^ sw) + 4]);
       const float av[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
       const float bv[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
 #pragma unroll
