@@ -22,7 +22,8 @@ ms = replicas.max_over_ranks(10.0 + 5.0 * rank, dist, "cpu")        # rank 1 is 
 dist.barrier()
 out = {"rank": rank, "world": world, "ms": ms, "gbs": replicas.job_throughput_gbs(3.0e9, world, ms),
        "seed": replicas.replica_seed(100, rank)}
-print("RESULT " + json.dumps(out), flush=True)
+with open(os.path.join(os.environ["ELDR_OUT"], "rank%d.json" % rank), "w") as f:   # one file per rank: the ranks'
+    json.dump(out, f)                                                           # stdout lines can interleave
 dist.destroy_process_group()
 """
 
@@ -36,12 +37,12 @@ def _free_port():
 def test_max_over_ranks_and_job_throughput_world2(tmp_path):
     script = tmp_path / "worker.py"
     script.write_text(WORKER)
-    env = dict(os.environ, ELDR_ROOT=ROOT, MASTER_ADDR="127.0.0.1")
+    env = dict(os.environ, ELDR_ROOT=ROOT, ELDR_OUT=str(tmp_path), MASTER_ADDR="127.0.0.1")
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2",
            "--master-addr", "127.0.0.1", "--master-port", str(_free_port()), str(script)]
     r = subprocess.run(cmd, env=env, capture_output=True, text=True, timeout=240)
     assert r.returncode == 0, r.stderr[-2000:]
-    res = [json.loads(l.split("RESULT ", 1)[1]) for l in r.stdout.splitlines() if "RESULT " in l]
+    res = [json.loads((tmp_path / ("rank%d.json" % i)).read_text()) for i in range(2)]
     assert sorted(x["rank"] for x in res) == [0, 1]
     for x in res:
         assert x["world"] == 2
