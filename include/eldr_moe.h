@@ -104,7 +104,10 @@ int32_t eldr_moe_gate_topk(const eldr_moe_shape_t* shape, int32_t layer, int32_t
  *   out [T,H] bf16 (rounded once, RNE, from the fp32 combine);
  *   topk_ids/topk_w: outputs, or INPUTS if force_routing != 0 (ids must be distinct per token, in [0,E));
  *   active_experts [E] int32 out: first n_active entries = U ascending, rest -1;  n_active [1] int32 out.
- *   T in 0..1024 (decode batches; larger T -> ELDR_ERR_UNSUPPORTED).
+ *   T in 0..16384 (larger T -> ELDR_ERR_UNSUPPORTED).  T <= 256 with H, I multiples of 64: the whole step is one
+ *   persistent launch; T <= 1024: one launch per stage; T > 1024 (prefill-shaped, "prefill forward ...
+ *   captures signature"): gate GEMM, top-k + signature, a chunked counting sort, gather, the grouped FFN with 256
+ *   tokens per tcgen05 accumulator pass, combine -- same arithmetic, compute-bound instead of HBM-bound.
  * Fast path (TMA + mma) needs H % 64 == 0 and I % 64 == 0; other shapes run a plain CUDA-core path. */
 int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* shape, int32_t layer, int32_t T,
                               const eldr_bf16* x, const float* gate_w, const float* gate_bias,

@@ -10,7 +10,7 @@ _ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(CSRC, "libeldr_moe.so")
 SOURCES = ["eldr_moe.cu"]
-HEADERS = ["device_utils.cuh", "gate_route.cuh", "ffn_stream.cuh", "ffn_umma.cuh", "moe_fused.cuh", "route_decide.cuh", "gate_prefill.cuh"]
+HEADERS = ["device_utils.cuh", "gate_route.cuh", "ffn_stream.cuh", "ffn_umma.cuh", "moe_fused.cuh", "route_decide.cuh", "gate_prefill.cuh", "route_prefill.cuh"]
 
 
 def _stale() -> bool:

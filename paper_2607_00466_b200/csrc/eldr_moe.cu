@@ -16,6 +16,7 @@
 #include "gate_prefill.cuh"
 #include "moe_fused.cuh"
 #include "route_decide.cuh"
+#include "route_prefill.cuh"
 
 namespace {
 
@@ -64,6 +65,19 @@ bool launch_ok(const char* what) {
 }
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+constexpr int kDecodeMaxT = 1024;     // single-CTA routing (route_phases); above it the chunked routing kernels
+constexpr int kPrefillMaxT = 16384;   // eldr_moe_decode_layer: largest prefill-shaped T
+
+// Split-K slices of the prefill-shaped gate GEMM (gate_prefill.cuh): the fewest slices of at most 256 h; 0 when the
+// shape does not take that path.
+int gate_slices(const eldr_moe_shape_t* s, int T) {
+  if (T < 2048 || s->hidden % kGpBK != 0) return 0;
+  const int chunks = s->hidden / kGpBK;
+  for (int c = 1; c <= 64; ++c)
+    if (chunks % c == 0 && s->hidden / c <= 256) return c;
+  return 0;
+}
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 int32_t check_shape(const eldr_moe_shape_t* s) {
@@ -86,8 +100,9 @@ void make_layout(const eldr_moe_shape_t* s, int T, eldr_moe_ws_layout_t* L) {
   const size_t sync_staged = ((size_t)((kFusedMaxT > (int)Tz ? kFusedMaxT : Tz) + kGateTok - 1) / kGateTok * ((E + kGateExp - 1) / kGateExp + 2) + 1) * 4;
   const size_t sync_fused = fused_sync_words((int)E, (int)ns, (int)I) * 4;
   L->sync = take(align_up(sync_fused, 256) + sync_staged);   // [fused | staged]: never aliased (both derive epochs)
-  L->z = take(Tz * E * 4);
-  L->cnt = take(E * 4);
+  const int zs = gate_slices(s, T);
+  L->z = take(Tz * E * 4 * (zs > 1 ? zs : 1));              // prefill-shaped gate: one partial logit tensor per slice
+  L->cnt = take(align_up(E * 4, 256) + (Tz > (size_t)kDecodeMaxT ? (Tz + kRouteChunk - 1) / kRouteChunk * E * 4 : 0));   // + cnt_blk
   L->off = take((E + 1) * 4);
   L->perm = take(Tz * k * 4);
   L->pair_pos = take(Tz * k * 4);
@@ -240,6 +255,25 @@ int32_t launch_gate_logits(const eldr_moe_shape_t* s, int T, const eldr_bf16* x,
   return launch_ok("gate_logits_kernel") ? ELDR_OK : ELDR_ERR_CUDA;
 }
 
+// a1-a3 as separate launches (eldr_moe_gate_topk and the prefill-shaped layer): logits, then warp top-k + signature.
+int32_t launch_gate_topk(const eldr_moe_shape_t* s, int T, const eldr_bf16* x, const float* gate_w,
+                         const float* gate_bias, float* z, size_t z_bytes, const TopkArgs& a, cudaStream_t st) {
+  const int S = gate_slices(s, T);
+  if (S > 0 && z_bytes >= (size_t)S * T * s->n_experts * 4) {
+    // prefill-shaped: register-tiled fp32 GEMM, split-K into the fewest slices of at most 256 h (accuracy, see
+    // gate_prefill.cuh); taken when the workspace holds the S partial logit tensors
+    gate_logits_tiled_kernel<<<dim3((T + kGpBM - 1) / kGpBM, (s->n_experts + kGpBN - 1) / kGpBN, S), kGpThreads, 0, st>>>(
+        x, gate_w, gate_bias, z, T, s->hidden, s->n_experts, s->hidden / S);
+    if (!launch_ok("gate_logits_tiled_kernel")) return ELDR_ERR_CUDA;
+    topk_splitk_kernel<<<(T + 7) / 8, 256, 0, st>>>(a, z, S);
+    return launch_ok("topk_splitk_kernel") ? ELDR_OK : ELDR_ERR_CUDA;
+  }
+  const int32_t rc = launch_gate_logits(s, T, x, gate_w, gate_bias, z, st);
+  if (rc != ELDR_OK) return rc;
+  topk_kernel<<<(T + 7) / 8, 256, 0, st>>>(a);
+  return launch_ok("topk_kernel") ? ELDR_OK : ELDR_ERR_CUDA;
+}
+
 }  // namespace
 
 extern "C" {
@@ -352,25 +386,7 @@ int32_t eldr_moe_gate_topk(const eldr_moe_shape_t* s, int32_t layer, int32_t T, 
   float* z = static_cast<float*>(workspace);
   TopkArgs a{z, topk_ids, topk_w, token_req, token_block, sig_req, sig_block,
              T, s->n_experts, s->top_k, s->n_layers, layer, s->renormalize};
-  if (T >= 2048 && s->hidden % kGpBK == 0) {
-    // prefill-shaped: register-tiled fp32 GEMM, split-K into the fewest slices of at most 256 h (accuracy, see
-    // gate_prefill.cuh); taken when the workspace holds the S partial logit tensors
-    const int chunks = s->hidden / kGpBK;
-    int S = 0;
-    for (int c = 1; c <= 64; ++c)
-      if (chunks % c == 0 && s->hidden / c <= 256) { S = c; break; }
-    if (S > 0 && workspace_bytes >= (size_t)S * T * s->n_experts * 4) {
-      gate_logits_tiled_kernel<<<dim3((T + kGpBM - 1) / kGpBM, (s->n_experts + kGpBN - 1) / kGpBN, S), kGpThreads, 0, st>>>(
-          x, gate_w, gate_bias, z, T, s->hidden, s->n_experts, s->hidden / S);
-      if (!launch_ok("gate_logits_tiled_kernel")) return ELDR_ERR_CUDA;
-      topk_splitk_kernel<<<(T + 7) / 8, 256, 0, st>>>(a, z, S);
-      return launch_ok("topk_splitk_kernel") ? ELDR_OK : ELDR_ERR_CUDA;
-    }
-  }
-  rc = launch_gate_logits(s, T, x, gate_w, gate_bias, z, st);
-  if (rc != ELDR_OK) return rc;
-  topk_kernel<<<(T + 7) / 8, 256, 0, st>>>(a);
-  return launch_ok("topk_kernel") ? ELDR_OK : ELDR_ERR_CUDA;
+  return launch_gate_topk(s, T, x, gate_w, gate_bias, z, workspace_bytes, a, st);
 }
 
 int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t T, const eldr_bf16* x,
@@ -385,7 +401,7 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
   if (rc != ELDR_OK) return rc;
   if (T < 0 || layer < 0 || layer >= s->n_layers) return ELDR_ERR_INVALID_ARG;
   if (T == 0) return ELDR_OK;
-  if (T > 1024) return ELDR_ERR_UNSUPPORTED;
+  if (T > kPrefillMaxT) return ELDR_ERR_UNSUPPORTED;
   if (!x || !w13 || !w2 || !out || !topk_ids || !topk_w || !active_experts || !n_active || !workspace)
     return ELDR_ERR_INVALID_ARG;
   if (!force_routing && !gate_w) return ELDR_ERR_INVALID_ARG;
@@ -481,7 +497,29 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
   ra.n_active = n_active;
   const int W = (T + 31) / 32;
   const size_t route_smem = (size_t)E * W * 8 + (size_t)(2 * E + 1) * 4;
-  if (!force_routing) {
+  if (T > kDecodeMaxT) {
+    // prefill-shaped: gate GEMM + top-k/signature as their own launches, then the chunked
+    // counting sort (route_prefill.cuh)
+    if (!force_routing) {
+      prof_mark(0, st);
+      rc = launch_gate_topk(s, T, x, gate_w, gate_bias, z, L.cnt - L.z, ra.tk, st);
+      if (rc != ELDR_OK) return rc;
+    }
+    RouteBigArgs rb{ra, reinterpret_cast<int32_t*>(ws + L.cnt + align_up((size_t)E * 4, 256)), force_routing ? 1 : 0};
+    const int n_chunks = (T + kRouteChunk - 1) / kRouteChunk;
+    const size_t big_smem = route_big_smem_bytes(E);
+    static bool route_big_attr_set = false;
+    if (!route_big_attr_set) {
+      if (!set_smem(route_count_kernel, route_big_smem_bytes(kMaxExperts)) ||
+          !set_smem(route_scatter_kernel, route_big_smem_bytes(kMaxExperts))) return ELDR_ERR_CUDA;
+      route_big_attr_set = true;
+    }
+    prof_mark(1, st);
+    route_count_kernel<<<n_chunks, kRouteBigThreads, big_smem, st>>>(rb);
+    if (!launch_ok("route_count_kernel")) return ELDR_ERR_CUDA;
+    route_scatter_kernel<<<n_chunks, kRouteBigThreads, big_smem, st>>>(rb);
+    if (!launch_ok("route_scatter_kernel")) return ELDR_ERR_CUDA;
+  } else if (!force_routing) {
     // a1-a4 in one launch: gate GEMV tiles; last CTA of a token group runs its top-k (+signature);
     // last group runs the permutation / union compaction
     static std::atomic<uint32_t> g_epoch{0x5eed0000u};
@@ -534,8 +572,10 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
     if (!make_tmap(&tm_h16, hbuf, (uint64_t)out_rows, I, 16)) return ELDR_ERR_CUDA;
     if (!make_tmap(&tm_h64, hbuf, (uint64_t)out_rows, I, 64)) return ELDR_ERR_CUDA;
     UmmaCfg cfg;
-    cfg.np = T <= 64 ? 64 : 128;      // an expert receives at most T tokens
-    cfg.stages = T <= 64 ? 8 : 6;
+    // token columns per accumulator pass (an expert receives at most T tokens); prefill-shaped calls take the widest
+    // MMA (N = 256: each 16 KiB weight stage is reused by 256 tokens, TMEM 2 x 256 columns)
+    cfg.np = T <= 64 ? 64 : (T <= kDecodeMaxT ? 128 : 256);
+    cfg.stages = T <= 64 ? 8 : (T <= kDecodeMaxT ? 6 : 4);
     const size_t smem = (size_t)cfg.stages * (kUmmaWBytes + cfg.np * 128) + 1024 + 256;
     static bool umma_attr_set = false;
     if (!umma_attr_set) {

@@ -38,6 +38,7 @@ def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--T", type=int, default=64)
     ap.add_argument("--unions", default="16,128")
+    ap.add_argument("--opt", action="append", default=[], help="KEY=VALUE for eldr_moe_set_option (repeatable)")
     args = ap.parse_args()
     os.environ["ELDR_EXTRA_NVCC_FLAGS"] = (os.environ.get("ELDR_EXTRA_NVCC_FLAGS", "") + " -DELDR_TRACE").strip()
     import torch
@@ -46,6 +47,8 @@ def main():
     b.build(force=True)
     from paper_2607_00466_b200 import api, synth
     lib = api.load()
+    for kv in args.opt:
+        api.eldr_moe_set_option(*[int(v) for v in kv.split("=")])
     shape, T = synth.SHAPE_QWEN, args.T
     lw = synth.make_layer_weights(shape, synth.WEIGHT_SEED)
     dl = api.DecodeLayer(shape, lw, max_T=T)

@@ -73,12 +73,12 @@ def test_invalid_arguments_are_rejected_without_a_gpu(lib):
     bad = api.make_shape(synth.SHAPE_C1)
     bad.top_k = 17
     assert so.eldr_moe_workspace_bytes(C.byref(bad), C.c_int32(8)) == 0
-    # decode layer: T above the decode-batch limit is "unsupported", misaligned pointer is "invalid"
+    # decode layer: T above the prefill-shaped limit (16384) is "unsupported", misaligned pointer is "invalid"
     def layer_call(T, ptr):
         p = C.c_void_p(ptr)
         return so.eldr_moe_decode_layer(C.byref(good), C.c_int32(0), C.c_int32(T), p, p, null, p, p, null, null, p,
                                         p, p, C.c_int32(0), p, p, null, null, null, null, p, C.c_size_t(1 << 30), null)
-    assert layer_call(2000, 4096) == -2
+    assert layer_call(20000, 4096) == -2
     assert layer_call(8, 4096 + 4) == -1
     assert so.eldr_moe_decode_layer(C.byref(good), C.c_int32(0), C.c_int32(8), C.c_void_p(4096), C.c_void_p(4096),
                                     null, C.c_void_p(4096), C.c_void_p(4096), null, null, C.c_void_p(4096),

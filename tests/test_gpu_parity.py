@@ -509,3 +509,63 @@ def test_gate_prefill_tiled_gemm(gpu, oracle, H, E, k, T, big_ws):
     gpu.eldr_moe_gate_topk(*args)
     torch.cuda.synchronize()
     assert torch.equal(first[0], ids) and torch.equal(first[1].view(torch.int32), w.view(torch.int32))
+
+
+# ------------------------------------------------------------------------- prefill-shaped layer
+@pytest.mark.gpu
+@pytest.mark.parametrize("H,I,E,k,T,ns", [(256, 128, 16, 4, 1500, 0),     # two routing chunks, 375 tokens per expert: 2 passes
+                                          (320, 192, 10, 3, 2300, 1),     # tiled gate GEMM (T >= 2048), ragged E, shared expert
+                                          (128, 64, 130, 2, 1025, 0),     # one token past the decode-shaped limit, many experts
+                                          (72, 40, 6, 2, 1100, 0)])       # H, I not multiples of 64: plain CUDA-core FFN
+def test_prefill_shaped_layer_ragged(gpu, oracle, H, I, E, k, T, ns):
+    """T > 1024: gate + top-k/signature, chunked counting sort (route_prefill.cuh), gather, grouped FFN with 256-token
+    accumulator passes, combine -- every stage against the oracle, signatures included."""
+    shape = synth.MoEShape(hidden=H, inter=I, n_experts=E, top_k=k, n_shared=ns, n_layers=2, kv_block_size=16)
+    lw = synth.make_layer_weights(shape, 31, w_std=0.05, gate_std=0.2)
+    x = synth.make_hidden(T, H, 32)
+    n_req = 7
+    token_req = (np.arange(T) % n_req).astype(np.int32)
+    token_req[::11] = -1                                     # padding tokens are not recorded
+    token_block = (np.arange(T) // 16).astype(np.int32)
+    n_blk = int(token_block.max()) + 1
+    r = run_case(gpu, oracle, shape, lw, x, None, token_req, token_block, n_req=n_req, n_blk=n_blk, layer=1)
+    assert r["n_active"] == len(np.unique(r["ids"]))
+    assert gpu.eldr_moe_last_launch_count() == 8             # logits, top-k, count, scatter, gather, w1/w3, w2, combine
+
+
+@pytest.mark.gpu
+def test_prefill_shaped_layer_qwen_2048(gpu, oracle, qwen_layer):
+    """Qwen3-30B-A3B-shaped layer at T = 2048 prefill tokens (every expert active, ~128 tokens each): Gates A/B."""
+    shape, lw, _ = qwen_layer
+    T = 2048
+    x = synth.make_hidden(T, shape.hidden, 77)
+    r = run_case(gpu, oracle, shape, lw, x, check_pairs=False)
+    assert r["n_active"] == shape.n_experts
+
+
+@pytest.mark.gpu
+def test_prefill_shaped_forced_routing_and_determinism(gpu, oracle):
+    """ids given (force_routing): the chunked routing records the signatures itself; two runs are bit-identical."""
+    import torch
+    shape = synth.MoEShape(hidden=256, inter=128, n_experts=24, top_k=3, n_layers=1, kv_block_size=16)
+    lw = synth.make_layer_weights(shape, 41, w_std=0.05, gate_std=0.2)
+    T = 1800
+    x = synth.make_hidden(T, shape.hidden, 42)
+    rng = np.random.default_rng(43)
+    ids = np.stack([rng.choice(12, size=3, replace=False) * 2 for _ in range(T)]).astype(np.int32)   # even experts only
+    w = rng.random((T, 3)).astype(np.float32)
+    w /= w.sum(1, keepdims=True)
+    token_req = (np.arange(T) % 5).astype(np.int32)
+    token_block = (np.arange(T) // 16).astype(np.int32)
+    r = run_case(gpu, oracle, shape, lw, x, None, token_req, token_block, n_req=5, n_blk=int(token_block.max()) + 1,
+                 force=(ids, w))
+    assert r["n_active"] == 12
+    dl = r["layer"]
+    xg = gpu.bf16_from_bits(x)
+    outs = []
+    for _ in range(2):
+        dl.ids[:T].copy_(torch.from_numpy(ids))
+        dl.w[:T].copy_(torch.from_numpy(w))
+        outs.append(dl.run(xg, None, force_routing=1).clone())
+        torch.cuda.synchronize()
+    assert torch.equal(outs[0], outs[1])
