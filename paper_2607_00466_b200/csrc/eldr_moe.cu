@@ -544,6 +544,8 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
   // gather token rows in expert-sorted order (+ plain copy for the shared experts)
   const int x_rows = T * k + (ns ? T : 0);
   const int out_rows = T * (k + ns);
+  // (Gathering inside the w1/w3 kernel by TMA tile::gather4, as the fused decode kernel does, was measured for the
+  // prefill-shaped calls and rejected: 256 single-row requests per stage instead of four boxes made w1/w3 3.7x slower.)
   prof_mark(2, st);
   launch_dep(gather_x_kernel, dim3((x_rows + 7) / 8), dim3(256), 0, st, x, perm, x_perm, T, H, k, x_rows);
   if (!launch_ok("gather_x_kernel")) return ELDR_ERR_CUDA;
@@ -627,7 +629,8 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
   }
   // a7: weighted combine
   prof_mark(5, st);
-  launch_dep(combine_kernel, dim3((T * (H / 4) + 255) / 256), dim3(256), 0, st, ybuf, topk_w, pair_pos, out, T, H, k, ns);
+  launch_dep(k <= 8 ? combine_kernel<8> : combine_kernel<kMaxTopK>, dim3((T * (H / 4) + 255) / 256), dim3(256), 0, st,
+             ybuf, topk_w, pair_pos, out, T, H, k, ns);
   if (!launch_ok("combine_kernel")) return ELDR_ERR_CUDA;
   prof_mark(ELDR_PROFILE_SLOTS, st);
   return ELDR_OK;

@@ -421,6 +421,9 @@ __global__ void __launch_bounds__(256) gather_x_kernel(const uint16_t* __restric
 // --------------------------------------------------------------------------- a7: weighted combine
 // out[t] = sum_j w[t,j]*y[pos(t,j)] (slot order) + sum_s y[shared s, t]; fp32, one RNE rounding to bf16.
 // Staged + ordered instead of fp32 atomics so that results are run-to-run bit-identical.
+// KMAX = compile-time bound on k (8 or kMaxTopK): with 8 slots the kernel needs half the registers, so twice as many
+// warps keep loads in flight -- the prefill-shaped step reads a gigabyte of y here.
+template <int KMAX>
 __global__ void __launch_bounds__(256) combine_kernel(const float* __restrict__ y,
                                                       const float* __restrict__ w,
                                                       const int32_t* __restrict__ pair_pos,
@@ -433,17 +436,17 @@ __global__ void __launch_bounds__(256) combine_kernel(const float* __restrict__ 
   const int t = idx / q_per_row, c4 = idx - t * q_per_row;
   float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
   // two dependent loads per slot (position, then the staged row): issue all of them before the first FMA
-  int pos[kMaxTopK];
-  float wt[kMaxTopK];
-  float4 v[kMaxTopK];
+  int pos[KMAX];
+  float wt[KMAX];
+  float4 v[KMAX];
 #pragma unroll
-  for (int j = 0; j < kMaxTopK; ++j)
-    if (j < k) { pos[j] = __ldg(pair_pos + t * k + j); wt[j] = __ldg(w + t * k + j); }
+  for (int j = 0; j < KMAX; ++j)
+    if (j < k) { pos[j] = __ldg(pair_pos + (size_t)t * k + j); wt[j] = __ldg(w + (size_t)t * k + j); }
 #pragma unroll
-  for (int j = 0; j < kMaxTopK; ++j)
+  for (int j = 0; j < KMAX; ++j)
     if (j < k) v[j] = __ldcs(reinterpret_cast<const float4*>(y + (size_t)pos[j] * H + (size_t)c4 * 4));
 #pragma unroll
-  for (int j = 0; j < kMaxTopK; ++j)
+  for (int j = 0; j < KMAX; ++j)
     if (j < k) {
       acc.x = fmaf(wt[j], v[j].x, acc.x); acc.y = fmaf(wt[j], v[j].y, acc.y);
       acc.z = fmaf(wt[j], v[j].z, acc.z); acc.w = fmaf(wt[j], v[j].w, acc.w);

@@ -5,7 +5,7 @@ of the HBM roofline, and the two derived checks -- union scaling fit t = a + b*|
 shared-expert stack plus the prefill-shaped signature accumulation.
 
   python -m paper_2607_00466_b200.report [--configs 2,3,4,5,6] [--steps K] > profiles/<name>.md
-(6 = the routing-decision row of SURVEY.md 8(f))
+(6 = the routing-decision row of SURVEY.md 8(f), 7 = its prefill-shaped layer row)
 
 Timing only (parity of the same configs against the oracle is tests/test_gpu_parity.py); Gate C invariants of
 SURVEY.md 8(c) are asserted on the GPU outputs of every row.  Needs a CUDA device; there is no CPU fallback.
@@ -336,10 +336,58 @@ def route_rows(api, synth):
     return out
 
 
+def _tensor_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            j = json.load(f)
+        return float(j["bf16_tflops"]), float(j.get("bf16_tflops_sustained", j["bf16_tflops"]))
+    return 1700.0, 1400.0
+
+
+def prefill_rows(api, synth, steps, Ts=(1024, 2048, 4096, 8192, 16384)):
+    """the same layer call with prefill-shaped T (every expert active, hundreds of tokens per
+    expert): the bound moves from HBM to the tensor pipe.  Algorithmic flops = T*k*6*H*I + 2*T*H*E."""
+    import torch
+    shape = synth.SHAPE_QWEN
+    H, I, E, k = shape.hidden, shape.inter, shape.n_experts, shape.top_k
+    lw = synth.make_layer_weights(shape, synth.WEIGHT_SEED)
+    burst, sustained = _tensor_peaks()
+    out = ["| T | realised \\|U\\| | tokens per expert | ms/step median (p10, p90) | tokens/s | algorithmic GFLOP | TFLOP/s | of measured "
+           "bf16 %.0f (sustained) | of %.0f (burst) | algorithmic GB/s | gate+top-k / route / gather / w1,w3 / w2 / combine µs |" % (sustained, burst),
+           "|---|---|---|---|---|---|---|---|---|---|---|"]
+    dl = api.DecodeLayer(shape, lw, max_T=max(Ts))
+    for T in Ts:
+        x = api.bf16_from_bits(synth.make_hidden(T, H, 1000 + T))
+
+        def fn(i):
+            dl.run(x, None)
+        fn(0)
+        torch.cuda.synchronize()
+        na = gate_c(api, dl, shape, T)
+        us, p10, p90 = time_blocks(fn, max(3, min(steps, 20)), blocks=5, warm=2)
+        api.eldr_moe_profile_enable(True)
+        try:
+            fn(0)
+            prof = api.eldr_moe_profile_read()
+        finally:
+            api.eldr_moe_profile_enable(False)
+        flop = T * k * 6.0 * H * I + 2.0 * T * H * E
+        tf = flop / us / 1e6
+        b = algorithmic_bytes(shape, T, na)
+        out.append("| %d | %d | %.0f | %.3f (%.3f, %.3f) | %.0f | %.1f | %.0f | %.3f | %.3f | %.0f | %s |" % (
+            T, na, T * k / max(na, 1), us / 1e3, p10 / 1e3, p90 / 1e3, T / us * 1e6, flop / 1e9, tf, tf / sustained,
+            tf / burst, b / us / 1e3, " / ".join("%.0f" % (v * 1e3) for v in prof.values())))
+    del dl
+    torch.cuda.empty_cache()
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--configs", default="2,3,4,5,6")
     ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--prefill-T", default="1024,2048,4096,8192,16384", help="token counts of the config-7 rows")
     args = ap.parse_args()
     which = {int(c) for c in args.configs.split(",")}
     import torch
@@ -364,6 +412,13 @@ def main():
               "order because each decision sees the loads left by the previous one).  Latency-bound; the paper's "
               "'Route (tau-JSQ)' step costs 0.15 ms per request on the proxy host (PAPER.md Table 1, context).\n" %
               "\n".join(route_rows(api, synth)), flush=True)
+    if 7 in which:
+        print("## Prefill-shaped layer (SURVEY.md 8(f) row 2: `eldr_moe_decode_layer` with T > 1024; Qwen3-30B-A3B-shaped, "
+              "x ~ N(0,1), no gate bias)\n\n%s\n\nEight launches (gate GEMM, top-k + signature, routing count / scatter, "
+              "gather, w1/w3, w2, combine); the per-kernel column is one step with CUDA events between the launches "
+              "(programmatic dependent launch off), the step time is back-to-back steps without them.  T = 1024 still "
+              "takes the decode-shaped staged path (128-token passes).  Parity: `tests/test_gpu_parity.py -k prefill_shaped`.\n" %
+              "\n".join(prefill_rows(api, synth, args.steps, tuple(int(v) for v in args.prefill_T.split(",")))), flush=True)
     if 5 in which:
         lines, note = config_5(api, synth, min(args.steps, 10))
         print("## Config 5 (27 layers, 64 routed + 2 shared experts, 31 GB resident)\n\n%s\n%s\n\n%s\n" % (HEADER, "\n".join(lines), note), flush=True)
