@@ -138,7 +138,7 @@ ffn_umma_kernel(const __grid_constant__ CUtensorMap tm_w, const __grid_constant_
     // ================================================================ weights producer
     if (lane == 0) {
       tma_prefetch_desc(&tm_w);
-      const uint64_t pol = l2_policy_evict_first();
+      const uint64_t pol_once = l2_policy_evict_first(), pol_again = l2_policy_evict_last();
       uint32_t it = 0;
       for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
         const int ent = tile / a.tiles_per_expert, rt = tile - ent * a.tiles_per_expert;
@@ -146,7 +146,12 @@ ffn_umma_kernel(const __grid_constant__ CUtensorMap tm_w, const __grid_constant_
         const bool shared = wk.x >= a.E;
         const CUtensorMap* tmw = shared ? &tm_ws : &tm_w;
         const int we = shared ? wk.x - a.E : wk.x;
+        // (Pulling this CTA's NEXT weight tile into L2 with cp.async.bulk.prefetch.tensor while the current one is
+        // multiplied was measured for the prefill-shaped calls, as a burst and one box per stage: 10-25 % slower both
+        // ways -- the prefetches hold TMA request slots for a DRAM latency each and the demand loads queue behind them.)
         for (int n0 = 0; n0 < wk.w; n0 += NP) {
+          // the tile is streamed once per accumulator pass: keep it in L2 until the last pass has read it
+          const uint64_t pol = (n0 + NP < wk.w) ? pol_again : pol_once;
           for (int kc = 0; kc < k_iters; ++kc, ++it) {
             const int s = it % S;
             mbar_wait(empty_bar(s), ((it / S) & 1) ^ 1);
