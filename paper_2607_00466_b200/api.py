@@ -29,6 +29,7 @@ OPT_PDL = 1
 OPT_STEP_PATH, STEP_STAGED, STEP_FUSED = 2, 0, 1
 OPT_RING_KB = 3
 OPT_DP_MIN_ROUNDS = 4
+OPT_FFN_PAIR = 5
 PROFILE_SLOTS = ("gate", "route", "gather", "ffn13", "ffn2", "combine")
 
 

@@ -12,6 +12,7 @@
 #include "eldr_moe.h"
 #include "ffn_stream.cuh"
 #include "ffn_umma.cuh"
+#include "ffn_umma2.cuh"
 #include "gate_route.cuh"
 #include "gate_prefill.cuh"
 #include "moe_fused.cuh"
@@ -22,6 +23,7 @@ namespace {
 
 using namespace eldr;
 
+int g_ffn_pair = 1;               // prefill-shaped calls: cta_group::2 FFN tiles over SM pairs (ELDR_OPT_FFN_PAIR)
 int g_ffn_path = ELDR_FFN_TCGEN05;   // process-wide tuning knobs (eldr_moe_set_option)
 int g_pdl = 1;
 int g_step_path = ELDR_STEP_FUSED;
@@ -239,6 +241,26 @@ cudaError_t launch_dep(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
   return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
 }
 
+// Same, as thread-block clusters of two CTAs (an SM pair for tcgen05 cta_group::2); grid.x must be even.
+template <typename... KArgs, typename... Args>
+cudaError_t launch_dep_pair(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[2];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = 2;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[1].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = (g_pdl && !g_prof_on) ? 2 : 1;
+  return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 template <typename K>
 bool set_smem(K kernel, size_t bytes) {
   return cuda_ok(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes),
@@ -307,6 +329,10 @@ const char* eldr_last_cuda_error(void) { return g_err; }
 int32_t eldr_moe_set_option(int32_t key, int32_t value) {
   if (key == ELDR_OPT_FFN_PATH && (value == ELDR_FFN_MMA_SYNC || value == ELDR_FFN_TCGEN05)) {
     g_ffn_path = value;
+    return ELDR_OK;
+  }
+  if (key == ELDR_OPT_FFN_PAIR && value >= 0 && value <= 2) {
+    g_ffn_pair = value;
     return ELDR_OK;
   }
   if (key == ELDR_OPT_PDL && (value == 0 || value == 1)) {
@@ -586,12 +612,34 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
       umma_attr_set = true;
     }
     f13.tiles_per_expert = I / 64;
-    prof_mark(3, st);
-    launch_dep(ffn_umma_kernel<0>, dim3(g13), dim3(kUmmaThreads), smem, st, tm_w13, tm_sw13, tm_x16, tm_x64, f13, cfg);
-    if (!launch_ok("ffn_umma_kernel<w13>")) return ELDR_ERR_CUDA;
-    prof_mark(4, st);
-    launch_dep(ffn_umma_kernel<1>, dim3(g2), dim3(kUmmaThreads), smem, st, tm_w2, tm_sw2, tm_h16, tm_h64, f2, cfg);
-    if (!launch_ok("ffn_umma_kernel<w2>")) return ELDR_ERR_CUDA;
+    // auto: from ~192 tokens per expert the pair tile's smaller operand traffic wins (T = 4096 on the Qwen shape; at
+    // 128 tokens per expert the single-CTA tile is 6 % faster)
+    const bool pair_pays = g_ffn_pair == 2 || (g_ffn_pair == 1 && (size_t)T * k >= (size_t)192 * E);
+    if (T > kDecodeMaxT && pair_pays && I % 128 == 0 && H % 256 == 0 && sms >= 2) {
+      // prefill-shaped: M = 256 tiles over SM pairs (ffn_umma2.cuh), six 32 KiB stages per CTA
+      const int stages = 6;
+      const size_t smem2 = (size_t)stages * kPairStageBytes + 1024 + 256 + (size_t)(2 * max_work + 2) * 4 + 16;
+      static bool pair_attr_set = false;
+      if (!pair_attr_set) {
+        const size_t mx2 = (size_t)stages * kPairStageBytes + 1024 + 256 + (size_t)(2 * (256 + 64) + 4) * 4 + 16;
+        if (!set_smem(ffn_umma2_kernel<0>, mx2) || !set_smem(ffn_umma2_kernel<1>, mx2)) return ELDR_ERR_CUDA;
+        pair_attr_set = true;
+      }
+      const int grid2 = sms & ~1;
+      prof_mark(3, st);
+      launch_dep_pair(ffn_umma2_kernel<0>, dim3(grid2), dim3(kUmmaThreads), smem2, st, tm_w13, tm_sw13, tm_x16, tm_x64, f13, stages, max_work + 1);
+      if (!launch_ok("ffn_umma2_kernel<w13>")) return ELDR_ERR_CUDA;
+      prof_mark(4, st);
+      launch_dep_pair(ffn_umma2_kernel<1>, dim3(grid2), dim3(kUmmaThreads), smem2, st, tm_w2, tm_sw2, tm_h16, tm_h64, f2, stages, max_work + 1);
+      if (!launch_ok("ffn_umma2_kernel<w2>")) return ELDR_ERR_CUDA;
+    } else {
+      prof_mark(3, st);
+      launch_dep(ffn_umma_kernel<0>, dim3(g13), dim3(kUmmaThreads), smem, st, tm_w13, tm_sw13, tm_x16, tm_x64, f13, cfg);
+      if (!launch_ok("ffn_umma_kernel<w13>")) return ELDR_ERR_CUDA;
+      prof_mark(4, st);
+      launch_dep(ffn_umma_kernel<1>, dim3(g2), dim3(kUmmaThreads), smem, st, tm_w2, tm_sw2, tm_h16, tm_h64, f2, cfg);
+      if (!launch_ok("ffn_umma_kernel<w2>")) return ELDR_ERR_CUDA;
+    }
   } else if (H % 64 == 0 && I % 64 == 0) {
     // legacy tensor-core path (mma.sync), kept selectable for comparison
     CUtensorMap tm_w13, tm_sw13, tm_x, tm_w2, tm_sw2, tm_h;

@@ -534,6 +534,31 @@ def test_prefill_shaped_layer_ragged(gpu, oracle, H, I, E, k, T, ns):
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("pair", [2, 0])
+@pytest.mark.parametrize("H,I,E,k,T,ns", [(512, 256, 10, 3, 2300, 1),     # ragged passes (690 tokens per expert), shared expert with 2300 tokens
+                                          (256, 128, 40, 2, 1300, 0)])    # 65 tokens per expert: one narrow pass per pair tile
+def test_prefill_shaped_pair_tiles(gpu, oracle, pair, H, I, E, k, T, ns):
+    """Prefill-shaped FFN as cta_group::2 tiles over SM pairs (ffn_umma2.cuh; forced with ELDR_OPT_FFN_PAIR = 2,
+    the default from 192 tokens per expert) and as single-CTA tiles (ELDR_OPT_FFN_PAIR = 0): both against the oracle, run-to-run bit-identical."""
+    import torch
+    shape = synth.MoEShape(hidden=H, inter=I, n_experts=E, top_k=k, n_shared=ns, n_layers=1, kv_block_size=16)
+    lw = synth.make_layer_weights(shape, 51, w_std=0.05, gate_std=0.2)
+    x = synth.make_hidden(T, H, 52)
+    gpu.eldr_moe_set_option(gpu.OPT_FFN_PAIR, pair)
+    try:
+        dl = gpu.DecodeLayer(shape, lw, max_T=T)
+        r = run_case(gpu, oracle, shape, lw, x, layer_obj=dl)
+        assert r["n_active"] == len(np.unique(r["ids"]))
+        xb = gpu.bf16_from_bits(x)
+        o1 = dl.run(xb, None).clone()
+        o2 = dl.run(xb, None).clone()
+        torch.cuda.synchronize()
+        assert torch.equal(o1.view(torch.int16), o2.view(torch.int16))
+    finally:
+        gpu.eldr_moe_set_option(gpu.OPT_FFN_PAIR, 1)
+
+
+@pytest.mark.gpu
 def test_prefill_shaped_layer_qwen_2048(gpu, oracle, qwen_layer):
     """Qwen3-30B-A3B-shaped layer at T = 2048 prefill tokens (every expert active, ~128 tokens each): Gates A/B."""
     shape, lw, _ = qwen_layer
