@@ -108,3 +108,19 @@ def test_route_decide_rejects_bad_arguments_without_a_gpu(lib):
     assert call(-1, 4, 0.1, p) == -1
     assert call(3, 0, 0.1, p) == -1 and call(3, 1025, 0.1, p) == -1
     assert call(3, 4, -0.5, p) == -1 and call(3, 4, float("nan"), p) == -1
+
+
+def test_tuning_options_validate_their_values(lib):
+    """eldr_moe_set_option (include/eldr_moe.h): process-wide knobs; out-of-range values and unknown keys are
+    ELDR_ERR_INVALID_ARG, valid ones take effect without a GPU (they are read at the next call)."""
+    api, so = lib
+    set_opt = so.eldr_moe_set_option
+    for key, good, bad in [(api.OPT_FFN_PATH, [api.FFN_MMA_SYNC, api.FFN_TCGEN05], [-1, 2]),
+                           (api.OPT_PDL, [0, 1], [2]),
+                           (api.OPT_STEP_PATH, [api.STEP_STAGED, api.STEP_FUSED], [3]),
+                           (api.OPT_FFN_PAIR, [0, 2, 1], [-1, 3])]:
+        for v in bad:
+            assert set_opt(C.c_int32(key), C.c_int32(v)) == -1
+        for v in good:                      # the last one is the default
+            assert set_opt(C.c_int32(key), C.c_int32(v)) == 0
+    assert set_opt(C.c_int32(99), C.c_int32(0)) == -1
