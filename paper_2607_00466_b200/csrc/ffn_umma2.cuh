@@ -88,6 +88,9 @@ __device__ __forceinline__ void umma2_commit_both(uint32_t bar) {
       :: "r"(bar), "h"((uint16_t)3) : "memory");
 }
 
+// SiLU with the fast exponential and division (2 ulp each; h is rounded to bf16, 2^-9, right after)
+__device__ __forceinline__ float silu_fast(float v) { return __fdividef(v, 1.0f + __expf(-v)); }
+
 template <int MODE>
 __global__ void __launch_bounds__(kUmmaThreads, 1)
 ffn_umma2_kernel(const __grid_constant__ CUtensorMap tm_w, const __grid_constant__ CUtensorMap tm_ws,
@@ -259,7 +262,7 @@ ffn_umma2_kernel(const __grid_constant__ CUtensorMap tm_w, const __grid_constant
             const float gv = lo ? v[k] : recv;
             const float uv = lo ? recv : v[8 + k];
             const int tok = n0 + c0 + (lo ? k : 8 + k);
-            if (tok < wk.w) a.h_out[(size_t)(wk.z + tok) * a.I + i] = f32_to_bf16_rn(silu_f(gv) * uv);
+            if (tok < wk.w) a.h_out[(size_t)(wk.z + tok) * a.I + i] = f32_to_bf16_rn(silu_fast(gv) * uv);
           }
         } else {
           const int r = rt * 128 + 32 * qtr + lane;
