@@ -559,6 +559,35 @@ def test_prefill_shaped_pair_tiles(gpu, oracle, pair, H, I, E, k, T, ns):
 
 
 @pytest.mark.gpu
+def test_prefill_shaped_graph_capture(gpu, oracle):
+    """The eight launches of a prefill-shaped call (2-CTA cluster launches of ffn_umma2 and programmatic dependent
+    launch edges included) captured in a CUDA graph: every replay reproduces the eager result bit for bit."""
+    import torch
+    shape = synth.MoEShape(hidden=512, inter=256, n_experts=8, top_k=2, n_layers=1, kv_block_size=16)
+    lw = synth.make_layer_weights(shape, 61, w_std=0.05, gate_std=0.2)
+    T = 2100                                      # 525 tokens per expert: pair tiles, three passes
+    x = gpu.bf16_from_bits(synth.make_hidden(T, shape.hidden, 62))
+    dl = gpu.DecodeLayer(shape, lw, max_T=T)
+    ref = dl.run(x, None).clone()
+    torch.cuda.synchronize()
+    assert gpu.eldr_moe_last_launch_count() == 8
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        dl.run(x, None)
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            dl.run(x, None)
+    torch.cuda.current_stream().wait_stream(side)
+    for _ in range(3):
+        dl.out.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(dl.out[:T].view(torch.int16), ref.view(torch.int16))
+        assert int(dl.n_active.item()) == 8
+
+
+@pytest.mark.gpu
 def test_prefill_shaped_layer_qwen_2048(gpu, oracle, qwen_layer):
     """Qwen3-30B-A3B-shaped layer at T = 2048 prefill tokens (every expert active, ~128 tokens each): Gates A/B."""
     shape, lw, _ = qwen_layer
