@@ -598,6 +598,19 @@ def test_prefill_shaped_layer_qwen_2048(gpu, oracle, qwen_layer):
 
 
 @pytest.mark.gpu
+def test_prefill_shaped_layer_c5_shape_2048(gpu, oracle):
+    """Config-5-shaped layer (64 routed top-6 + 2 shared experts, I = 1408) at T = 2048 prefill tokens: 192 tokens per
+    routed expert (the pair-tile threshold) and 2048 per shared expert (eight passes), against the full oracle."""
+    shape = dataclasses.replace(synth.SHAPE_C5, n_layers=1)
+    lw = synth.make_layer_weights(shape, 5)
+    T = 2048
+    x = synth.make_hidden(T, shape.hidden, 78)
+    r = run_case(gpu, oracle, shape, lw, x, check_pairs=False)
+    assert r["n_active"] == shape.n_experts
+    assert gpu.eldr_moe_last_launch_count() == 8
+
+
+@pytest.mark.gpu
 def test_prefill_shaped_forced_routing_and_determinism(gpu, oracle):
     """ids given (force_routing): the chunked routing records the signatures itself; two runs are bit-identical."""
     import torch
