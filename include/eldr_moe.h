@@ -177,9 +177,11 @@ int32_t eldr_moe_workspace_layout(const eldr_moe_shape_t* shape, int32_t T, eldr
  *   ELDR_OPT_FFN_PATH: ELDR_FFN_TCGEN05 (default; tcgen05.mma + TMEM) or ELDR_FFN_MMA_SYNC (legacy mma.sync). */
 #define ELDR_OPT_FFN_PATH 0
 #define ELDR_OPT_PDL      1   /* 1 (default): programmatic dependent launch between the step's kernels; 0: plain */
-#define ELDR_OPT_STEP_PATH 2  /* ELDR_STEP_FUSED (default): the whole step in ONE persistent launch (T <= 256,
-                                 H,I % 64 == 0); ELDR_STEP_STAGED: one launch per stage (gate+route, gather, w1/w3, w2,
-                                 combine), also the path for shapes the fused kernel does not take */
+#define ELDR_OPT_STEP_PATH 2  /* ELDR_STEP_FUSED: the whole step in ONE persistent launch (T <= 256, H,I % 64 == 0);
+                                 ELDR_STEP_STAGED: one launch per stage (gate+route, gather, w1/w3, w2, combine), also
+                                 the path for shapes the fused kernel does not take; ELDR_STEP_AUTO (default): fused,
+                                 except for layers with shared experts at T >= 224 (every token goes through a shared
+                                 expert, and the staged path handles such wide activation tiles faster) */
 #define ELDR_OPT_RING_KB  3   /* fused step: cap on the shared-memory stage ring in KiB per SM (bytes in flight);
                                  32..208; default 208 (all of it) */
 #define ELDR_OPT_DP_MIN_ROUNDS 4 /* fused step: a phase whose tile count is at least this many rounds of the grid runs its
@@ -191,6 +193,7 @@ int32_t eldr_moe_workspace_layout(const eldr_moe_shape_t* shape, int32_t T, eldr
                                  per 128-row tile) */
 #define ELDR_STEP_STAGED  0
 #define ELDR_STEP_FUSED   1
+#define ELDR_STEP_AUTO    2
 #define ELDR_FFN_MMA_SYNC 0
 #define ELDR_FFN_TCGEN05  1
 int32_t eldr_moe_set_option(int32_t key, int32_t value);

@@ -26,7 +26,7 @@ EXPORTS = [
 ]
 OPT_FFN_PATH, FFN_MMA_SYNC, FFN_TCGEN05 = 0, 0, 1
 OPT_PDL = 1
-OPT_STEP_PATH, STEP_STAGED, STEP_FUSED = 2, 0, 1
+OPT_STEP_PATH, STEP_STAGED, STEP_FUSED, STEP_AUTO = 2, 0, 1, 2
 OPT_RING_KB = 3
 OPT_DP_MIN_ROUNDS = 4
 OPT_FFN_PAIR = 5

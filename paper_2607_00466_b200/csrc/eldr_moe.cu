@@ -26,7 +26,7 @@ using namespace eldr;
 int g_ffn_pair = 1;               // prefill-shaped calls: cta_group::2 FFN tiles over SM pairs (ELDR_OPT_FFN_PAIR)
 int g_ffn_path = ELDR_FFN_TCGEN05;   // process-wide tuning knobs (eldr_moe_set_option)
 int g_pdl = 1;
-int g_step_path = ELDR_STEP_FUSED;
+int g_step_path = ELDR_STEP_AUTO;
 int g_ring_kb = 208;
 int g_dp_min_rounds = 4;
 
@@ -339,7 +339,7 @@ int32_t eldr_moe_set_option(int32_t key, int32_t value) {
     g_pdl = value;
     return ELDR_OK;
   }
-  if (key == ELDR_OPT_STEP_PATH && (value == ELDR_STEP_STAGED || value == ELDR_STEP_FUSED)) {
+  if (key == ELDR_OPT_STEP_PATH && (value == ELDR_STEP_STAGED || value == ELDR_STEP_FUSED || value == ELDR_STEP_AUTO)) {
     g_step_path = value;
     return ELDR_OK;
   }
@@ -452,7 +452,10 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
   float* ybuf = reinterpret_cast<float*>(ws + L.y);
 
   // ------------------------------------------------------------------ whole step in one persistent launch
-  if (g_step_path == ELDR_STEP_FUSED && g_ffn_path == ELDR_FFN_TCGEN05 && H % 64 == 0 && I % 64 == 0 &&
+  // AUTO: shared experts receive every token, so from ~224 tokens their activation tiles are as wide as the weight
+  // tiles and the staged path (rows gathered once, plain TMA boxes) is faster: config-5 shape at T = 256 280 -> 257 us
+  const bool want_fused = g_step_path == ELDR_STEP_FUSED || (g_step_path == ELDR_STEP_AUTO && !(ns > 0 && T >= 224));
+  if (want_fused && g_ffn_path == ELDR_FFN_TCGEN05 && H % 64 == 0 && I % 64 == 0 &&
       T <= kFusedMaxT && num_sms() <= 256) {
     FusedArgs fa;
     fa.x = x; fa.gate_w = gate_w; fa.gate_bias = gate_bias;

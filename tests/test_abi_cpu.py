@@ -117,7 +117,7 @@ def test_tuning_options_validate_their_values(lib):
     set_opt = so.eldr_moe_set_option
     for key, good, bad in [(api.OPT_FFN_PATH, [api.FFN_MMA_SYNC, api.FFN_TCGEN05], [-1, 2]),
                            (api.OPT_PDL, [0, 1], [2]),
-                           (api.OPT_STEP_PATH, [api.STEP_STAGED, api.STEP_FUSED], [3]),
+                           (api.OPT_STEP_PATH, [api.STEP_STAGED, api.STEP_FUSED, api.STEP_AUTO], [3]),
                            (api.OPT_FFN_PAIR, [0, 2, 1], [-1, 3])]:
         for v in bad:
             assert set_opt(C.c_int32(key), C.c_int32(v)) == -1

@@ -234,6 +234,13 @@ def test_c5_shared_experts_layer(gpu, oracle):
     token_req, token_block = synth.decode_maps(256)
     r = run_case(gpu, oracle, shape, lw, x, None, token_req, token_block, n_req=256, n_blk=256, check_pairs=False)
     assert r["n_active"] == 64
+    assert gpu.eldr_moe_last_launch_count() == 5      # ELDR_STEP_AUTO: shared experts at T >= 224 take the staged path
+    gpu.eldr_moe_set_option(gpu.OPT_STEP_PATH, gpu.STEP_FUSED)
+    try:
+        r = run_case(gpu, oracle, shape, lw, x, None, token_req, token_block, n_req=256, n_blk=256, check_pairs=False)
+        assert r["n_active"] == 64 and gpu.eldr_moe_last_launch_count() == 1
+    finally:
+        gpu.eldr_moe_set_option(gpu.OPT_STEP_PATH, gpu.STEP_AUTO)
 
 
 def test_c5_signature_accumulate_prefill_shaped(gpu, oracle):
@@ -370,7 +377,7 @@ def test_alternate_paths_match_oracle(gpu, oracle, step_path, ffn_path, pdl):
         r = run_case(gpu, oracle, shape, lw, x, None, token_req, token_block, n_req=150, n_blk=150, layer=1)
         assert gpu.eldr_moe_last_launch_count() == (1 if (step_path == 1 and ffn_path == 1) else 5)
     finally:
-        gpu.eldr_moe_set_option(gpu.OPT_STEP_PATH, gpu.STEP_FUSED)
+        gpu.eldr_moe_set_option(gpu.OPT_STEP_PATH, gpu.STEP_AUTO)
         gpu.eldr_moe_set_option(gpu.OPT_FFN_PATH, gpu.FFN_TCGEN05)
         gpu.eldr_moe_set_option(gpu.OPT_PDL, 1)
 
@@ -388,7 +395,7 @@ def test_staged_path_qwen_union(gpu, oracle, qwen_layer, u):
         r = run_case(gpu, oracle, shape, lw, x, bias, token_req, token_block, n_req=T, n_blk=T, layer_obj=dl)
         assert gpu.eldr_moe_last_launch_count() == 5 and r["n_active"] == u
     finally:
-        gpu.eldr_moe_set_option(gpu.OPT_STEP_PATH, gpu.STEP_FUSED)
+        gpu.eldr_moe_set_option(gpu.OPT_STEP_PATH, gpu.STEP_AUTO)
     r2 = run_case(gpu, oracle, shape, lw, x, bias, token_req, token_block, n_req=T, n_blk=T, layer_obj=dl)
     assert gpu.eldr_moe_last_launch_count() == 1 and r2["n_active"] == u
 
