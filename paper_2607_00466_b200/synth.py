@@ -112,6 +112,19 @@ def make_layer_weights(shape: MoEShape, seed: int, layer: int = 0,
     return LayerWeights(gate_w, w13, w2, s13, s2)
 
 
+def make_mxfp4_tensor(rows: int, K: int, seed: int, tag="mx", scale_lo: int = 118, scale_hi: int = 122):
+    """Seeded MXFP4-shaped raw bytes for SURVEY.md 8(f) row 3 (GPT-OSS-style experts): packed 4-bit codes
+    [rows, K/2] uint8 (uniform over the 16 codes) and one scale byte per 32 elements [rows, K/32] uint8, uniform in
+    scale_lo..scale_hi (2^-9..2^-5, so the decoded magnitudes are those of ~N(0,0.02) weights).  The generator draws
+    BYTES only -- what they mean is defined by the oracle (oracle/mxfp4.py) and, later, by the kernels."""
+    if K % 32:
+        raise ValueError("K must be a multiple of 32")
+    rng = np.random.default_rng(sub_seed(seed, tag, rows, K))
+    packed = rng.integers(0, 256, size=(rows, K // 2), dtype=np.uint8)
+    scales = rng.integers(scale_lo, scale_hi + 1, size=(rows, K // 32), dtype=np.uint8)
+    return packed, scales
+
+
 def make_hidden(T: int, H: int, seed: int, tag="x") -> np.ndarray:
     """Decode-token hiddens ~N(0,1) rounded to bf16 bits, [T,H]."""
     return _normal_bf16(np.random.default_rng(sub_seed(seed, tag, T)), (T, H), 1.0)
