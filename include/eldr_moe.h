@@ -189,7 +189,7 @@ int32_t eldr_moe_workspace_layout(const eldr_moe_shape_t* shape, int32_t T, eldr
                                  whole phase is stream-K.  1..2^20; default 4 */
 #define ELDR_OPT_FFN_PAIR 5   /* prefill-shaped calls (T > 1024, I % 128 == 0, H % 256 == 0): the expert FFN as tcgen05
                                  cta_group::2 tiles (M = 256 over an SM pair, ffn_umma2.cuh).  1 (default): when the call
-                                 has >= 192 tokens per expert on average (T*k >= 192*E); 2: always; 0: never (one CTA
+                                 has >= 256 tokens per expert on average (T*k >= 256*E); 2: always; 0: never (one CTA
                                  per 128-row tile) */
 #define ELDR_STEP_STAGED  0
 #define ELDR_STEP_FUSED   1

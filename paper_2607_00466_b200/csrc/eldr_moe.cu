@@ -615,9 +615,10 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
       umma_attr_set = true;
     }
     f13.tiles_per_expert = I / 64;
-    // auto: from ~192 tokens per expert the pair tile's smaller operand traffic wins (T = 4096 on the Qwen shape; at
-    // 128 tokens per expert the single-CTA tile is 6 % faster)
-    const bool pair_pays = g_ffn_pair == 2 || (g_ffn_pair == 1 && (size_t)T * k >= (size_t)192 * E);
+    // auto: from 256 tokens per expert on average (half of the experts then need a second 256-token pass and the pass-
+    // level unit list pays): T = 4096 on the Qwen shape 0.605 vs 0.632 ms; below it single-CTA tiles win (T = 3072:
+    // 0.462 vs 0.528 ms, T = 3584: 0.510 vs 0.524 ms)
+    const bool pair_pays = g_ffn_pair == 2 || (g_ffn_pair == 1 && (size_t)T * k >= (size_t)256 * E);
     if (T > kDecodeMaxT && pair_pays && I % 128 == 0 && H % 256 == 0 && sms >= 2) {
       // prefill-shaped: M = 256 tiles over SM pairs (ffn_umma2.cuh), six 32 KiB stages per CTA
       const int stages = 6;

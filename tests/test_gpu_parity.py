@@ -546,7 +546,7 @@ def test_prefill_shaped_layer_ragged(gpu, oracle, H, I, E, k, T, ns):
                                           (256, 128, 40, 2, 1300, 0)])    # 65 tokens per expert: one narrow pass per pair tile
 def test_prefill_shaped_pair_tiles(gpu, oracle, pair, H, I, E, k, T, ns):
     """Prefill-shaped FFN as cta_group::2 tiles over SM pairs (ffn_umma2.cuh; forced with ELDR_OPT_FFN_PAIR = 2,
-    the default from 192 tokens per expert) and as single-CTA tiles (ELDR_OPT_FFN_PAIR = 0): both against the oracle, run-to-run bit-identical."""
+    the default from 256 tokens per expert) and as single-CTA tiles (ELDR_OPT_FFN_PAIR = 0): both against the oracle, run-to-run bit-identical."""
     import torch
     shape = synth.MoEShape(hidden=H, inter=I, n_experts=E, top_k=k, n_shared=ns, n_layers=1, kv_block_size=16)
     lw = synth.make_layer_weights(shape, 51, w_std=0.05, gate_std=0.2)
@@ -607,14 +607,19 @@ def test_prefill_shaped_layer_qwen_2048(gpu, oracle, qwen_layer):
 @pytest.mark.gpu
 def test_prefill_shaped_layer_c5_shape_2048(gpu, oracle):
     """Config-5-shaped layer (64 routed top-6 + 2 shared experts, I = 1408) at T = 2048 prefill tokens: 192 tokens per
-    routed expert (the pair-tile threshold) and 2048 per shared expert (eight passes), against the full oracle."""
+    routed expert and 2048 per shared expert (eight passes), against the full oracle, with the SM-pair tiles forced
+    (I = 1408: 22 k-chunks per w2 stage row, 11 pair tiles per expert in w1/w3)."""
     shape = dataclasses.replace(synth.SHAPE_C5, n_layers=1)
     lw = synth.make_layer_weights(shape, 5)
     T = 2048
     x = synth.make_hidden(T, shape.hidden, 78)
-    r = run_case(gpu, oracle, shape, lw, x, check_pairs=False)
-    assert r["n_active"] == shape.n_experts
-    assert gpu.eldr_moe_last_launch_count() == 8
+    gpu.eldr_moe_set_option(gpu.OPT_FFN_PAIR, 2)
+    try:
+        r = run_case(gpu, oracle, shape, lw, x, check_pairs=False)
+        assert r["n_active"] == shape.n_experts
+        assert gpu.eldr_moe_last_launch_count() == 8
+    finally:
+        gpu.eldr_moe_set_option(gpu.OPT_FFN_PAIR, 1)
 
 
 @pytest.mark.gpu
