@@ -1,5 +1,7 @@
 """Rejection-sample the try seeds of BASELINE.json configs 2 and 3: for each (T, u)
-find the first seed whose gate-driven active-expert union has exactly min(u, T*k) experts.
+find the first seed whose gate-driven active-expert union has exactly min(u, T*k) experts.  The realised union is
+the ONLY acceptance criterion: near-tie tokens are not filtered out here -- the parity tests
+classify them per token (margin <= 1e-5) and report them; the recorded min_margin is information only.
 
 Calls ONLY the oracle (oracle/eldr_oracle.c) and the seeded generators; writes
 paper_2607_00466_b200/union_seeds.json (an input recipe, not an expected value).
@@ -29,7 +31,7 @@ def main():
             x, bias = synth.union_case(shape, T, u, seed)
             r = oracle.gate_topk(shape, x, gate_w, bias)
             realised = len(np.unique(r["ids"]))
-            if realised == want and r["margin"].min() > 1e-4:
+            if realised == want:
                 out["T%d_u%d" % (T, u)] = {"seed": seed, "union": realised, "tries": seed - 999,
                                            "min_margin": float(r["margin"].min())}
                 print(T, u, out["T%d_u%d" % (T, u)])

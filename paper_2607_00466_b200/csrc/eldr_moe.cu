@@ -99,7 +99,7 @@ void make_layout(const eldr_moe_shape_t* s, int T, eldr_moe_ws_layout_t* L) {
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + bytes, 256); return r; };
   // epoch flags first, at a T-independent offset and size: the fused kernel keeps its generation word there
-  const size_t sync_staged = ((size_t)((kFusedMaxT > (int)Tz ? kFusedMaxT : Tz) + kGateTok - 1) / kGateTok * ((E + kGateExp - 1) / kGateExp + 2) + 1) * 4;
+  const size_t sync_staged = ((size_t)((kFusedMaxT > (int)Tz ? kFusedMaxT : Tz) + kGateTok - 1) / kGateTok * ((E + kGateExp - 1) / kGateExp + 2) + 2) * 4;
   const size_t sync_fused = fused_sync_words((int)E, (int)ns, (int)I) * 4;
   L->sync = take(align_up(sync_fused, 256) + sync_staged);   // [fused | staged]: never aliased (both derive epochs)
   const int zs = gate_slices(s, T);
@@ -551,11 +551,9 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
   } else if (!force_routing) {
     // a1-a4 in one launch: gate GEMV tiles; last CTA of a token group runs its top-k (+signature);
     // last group runs the permutation / union compaction
-    static std::atomic<uint32_t> g_epoch{0x5eed0000u};
     GateRouteArgs ga;
     ga.x = x; ga.gate_w = gate_w; ga.gate_bias = gate_bias; ga.r = ra;
     ga.sync = reinterpret_cast<uint32_t*>(ws + L.sync + align_up(fused_sync_words(E, ns, I) * 4, 256));
-    ga.epoch = ++g_epoch;
     size_t smem = (size_t)kGateTok * H * 2;
     if (route_smem > smem) smem = route_smem;
     if (smem > 200 * 1024) return ELDR_ERR_UNSUPPORTED;

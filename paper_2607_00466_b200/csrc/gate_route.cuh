@@ -318,13 +318,15 @@ __global__ void __launch_bounds__(1024) route_only_kernel(RouteArgs a) {
 // publish its tile (epoch flags + one atomicExch election; no counters to zero, so no memset in the stream)
 // runs the warp top-k + signature accumulation for that group's 8 tokens, one token per warp; the last GROUP to
 // finish runs the permutation / union compaction.  Latency ~ one GEMV tile + one top-k + one routing pass.
+// The epoch the flags are compared with is generation + 1, the generation word living in the workspace and bumped
+// by the very last CTA (every other CTA read it before publishing the tile flag that CTA waited for): nothing from
+// the host is frozen into the launch, so a CUDA-graph replay elects and routes like an eager call.
 struct GateRouteArgs {
   const uint16_t* x;
   const float* gate_w;
   const float* gate_bias;
   RouteArgs r;
-  uint32_t* sync;      // [n_groups*n_etiles] tile flags | [n_groups] elected | [n_groups] group flags | [1] elected
-  uint32_t epoch;      // unique per call
+  uint32_t* sync;      // [1] generation | [n_groups*n_etiles] tile flags | [n_groups] elected | [n_groups] group flags | [1] elected
 };
 
 __device__ __forceinline__ uint32_t ld_volatile_u32(const uint32_t* p) {
@@ -371,15 +373,16 @@ __global__ void __launch_bounds__(256) gate_topk_route_kernel(GateRouteArgs a) {
   const int n_etiles = gridDim.x, n_groups = gridDim.y;
   ELDR_STAMP(0);
   pdl_launch_dependents();
+  const uint32_t epoch = ld_volatile_u32(a.sync) + 1u;
   gate_tile(a.x, a.gate_w, a.gate_bias, const_cast<float*>(tk.z), T, a.r.H, E, smem_raw);
   ELDR_STAMP(2);
 
-  uint32_t* tile_flags = a.sync;
+  uint32_t* tile_flags = a.sync + 1;
   uint32_t* elected = tile_flags + n_groups * n_etiles;
   uint32_t* group_flags = elected + n_groups;
   uint32_t* elected2 = group_flags + n_groups;
   const int g = blockIdx.y;
-  if (!publish_and_elect(tile_flags + g * n_etiles, n_etiles, blockIdx.x, elected + g, a.epoch, &s_flag)) return;
+  if (!publish_and_elect(tile_flags + g * n_etiles, n_etiles, blockIdx.x, elected + g, epoch, &s_flag)) return;
   ELDR_STAMP(3);
 
   // top-k + signature for this group's tokens: one token per warp
@@ -396,9 +399,10 @@ __global__ void __launch_bounds__(256) gate_topk_route_kernel(GateRouteArgs a) {
     }
   }
   ELDR_STAMP(4);
-  if (!publish_and_elect(group_flags, n_groups, g, elected2, a.epoch, &s_flag)) return;
+  if (!publish_and_elect(group_flags, n_groups, g, elected2, epoch, &s_flag)) return;
   ELDR_STAMP(5);
   route_phases(a.r, smem_raw, 256, false);
+  if (threadIdx.x == 0) st_volatile_u32(a.sync, epoch);
   ELDR_STAMP(10);
 }
 

@@ -171,6 +171,75 @@ def test_c2_union_sweep(gpu, oracle, qwen_layer, u):
     assert r["n_active"] == u
 
 
+@pytest.mark.parametrize("u", [16, 128])
+def test_c2_gate_exact_on_unfiltered_seeds(gpu, oracle, qwen_layer, u, capsys):
+    """PAPER.md:43 ("expert selections ... identical to standard top-k gating") on inputs NOBODY selected: 50
+    consecutive try seeds of the config-2 recipe (T = 64, +40 bias on a seeded subset of u experts, |z| ~ 45, one
+    fp32 ulp = 3.8e-6), no rejection on union size or margin.  Gate A on every token whose oracle margin exceeds
+    1e-5 (ids set-equal, weights, logits abs <= 1e-5), through BOTH gate implementations: the fused step's
+    in-kernel gate and eldr_moe_gate_topk.  Near-ties (margin <= 1e-5) are counted and reported separately
+    (north_star), and whether the GPU agreed with the oracle on them anyway."""
+    import torch
+    shape, lw, dl = qwen_layer
+    T, k, E = 64, shape.top_k, shape.n_experts
+    ws = torch.empty(gpu.eldr_moe_workspace_bytes(shape, T), dtype=torch.uint8, device="cuda")
+    ids2 = torch.empty((T, k), dtype=torch.int32, device="cuda")
+    w2 = torch.empty((T, k), dtype=torch.float32, device="cuda")
+    n_tok = n_near = n_near_agree = 0
+    min_clean_margin, max_zerr = np.inf, 0.0
+    for seed in range(5000, 5050):
+        xb, bias = synth.union_case(shape, T, u, seed)
+        ora = oracle.gate_topk(shape, xb, lw.gate_w, bias)
+        x, b = gpu.bf16_from_bits(xb), torch.from_numpy(bias).cuda()
+        dl.run(x, b)
+        torch.cuda.synchronize()
+        ids_f, z_f = dl.ids[:T].cpu().numpy(), dl.ws_view("z", T).cpu().numpy()
+        clean = check_gate(shape, ora, ids_f, dl.w[:T].cpu().numpy(), z_f)
+        gpu.eldr_moe_gate_topk(shape, 0, x, dl.gate_w, b, ids2, w2, None, None, None, None, ws)
+        torch.cuda.synchronize()
+        check_gate(shape, ora, ids2.cpu().numpy(), w2.cpu().numpy(), ws[: T * E * 4].view(torch.float32).reshape(T, E).cpu().numpy())
+        n_tok += T
+        n_near += int((~clean).sum())
+        for t in np.nonzero(~clean)[0]:
+            n_near_agree += set(ids_f[t].tolist()) == set(ora["ids"][t].tolist())
+        if clean.any():
+            min_clean_margin = min(min_clean_margin, float(ora["margin"][clean].min()))
+        max_zerr = max(max_zerr, float(np.abs(z_f.astype(np.float64) - ora["z"]).max()))
+    with capsys.disabled():
+        print("\n[near-ties] u=%d: %d tokens over 50 unfiltered seeds, %d near-tie (margin <= 1e-5), GPU agreed with the "
+              "oracle on %d of them; smallest clean margin %.3e; max |z_gpu - z_oracle| %.2e"
+              % (u, n_tok, n_near, n_near_agree, min_clean_margin, max_zerr))
+
+
+def test_exact_ties_take_the_lower_id_and_near_ties_are_reported(gpu, oracle, capsys):
+    """Constructed ties at the top-k boundary.  Experts 0/1 have IDENTICAL gate rows (margin exactly 0 whenever the
+    k-th pick falls between them: both sides must take the lower id -- the tie-break reading of DESIGN.md 2, an exact
+    comparison in any precision); experts 2/3 differ by one fp32 ulp in a single gate element (margin ~1e-8: a
+    near-tie the contract excludes from Gate A; counted and printed, never asserted)."""
+    import torch
+    shape = synth.MoEShape(hidden=128, inter=64, n_experts=8, top_k=1, n_layers=1)
+    lw = synth.make_layer_weights(shape, 11, w_std=0.05, gate_std=0.05)
+    lw.gate_w[:4] *= 8.0                        # experts 0..3 win almost always
+    lw.gate_w[1] = lw.gate_w[0]
+    lw.gate_w[3] = lw.gate_w[2]
+    lw.gate_w[3, 5] = np.nextafter(lw.gate_w[3, 5], np.float32(10.0))
+    T = 96
+    x = synth.make_hidden(T, shape.hidden, 12)
+    dl = gpu.DecodeLayer(shape, lw, max_T=T)
+    dl.run(gpu.bf16_from_bits(x))
+    torch.cuda.synchronize()
+    ora = oracle.gate_topk(shape, x, lw.gate_w, None)
+    ids = dl.ids[:T].cpu().numpy()
+    exact = ora["margin"] == 0.0
+    near = (ora["margin"] <= 1e-5) & ~exact
+    assert exact.sum() >= 10 and near.sum() >= 10, (exact.sum(), near.sum())
+    assert np.array_equal(ids[exact], ora["ids"][exact]) and set(ids[exact].ravel().tolist()) == {0}
+    check_gate(shape, ora, ids, dl.w[:T].cpu().numpy(), dl.ws_view("z", T).cpu().numpy())
+    with capsys.disabled():
+        print("\n[near-ties] constructed: %d exact ties (all -> lower id), %d near-ties (margin <= 1e-5, excluded), GPU "
+              "agreed with the oracle on %d of the near-ties" % (exact.sum(), near.sum(), int((ids[near] == ora["ids"][near]).sum())))
+
+
 @pytest.mark.parametrize("T", [1, 8, 32, 128, 256])
 def test_c3_batch_sweep(gpu, oracle, qwen_layer, T):
     """BASELINE.json config 3: union 32 (8 at T=1), batch swept."""
@@ -445,6 +514,60 @@ def test_fused_kernel_back_to_back_steps_and_graph_capture(gpu, oracle, qwen_lay
         torch.cuda.synchronize()
         assert torch.equal(dl.out[:T].view(torch.int16), ref[u].view(torch.int16))
         assert int(dl.n_active.item()) == 16
+
+
+@pytest.mark.parametrize("case", ["small_T300", "c5_T256", "qwen_fused_T64"])
+def test_graph_replay_with_new_inputs_matches_oracle(gpu, oracle, case):
+    """A captured step must route from the x it finds at replay time, not from the capture-time step: x is
+    overwritten in place between replays, ids / weights / signatures are zeroed, and every replay is compared with
+    the oracle on that replay's x.  Covers the staged path (T = 300; config-5 shape at T = 256, which
+    ELDR_STEP_AUTO sends to the staged kernels) -- whose election epoch used to be a host counter frozen into the
+    captured launch, so replays silently reused the first step's routing -- and the fused launch."""
+    import torch
+    if case == "small_T300":
+        shape = synth.MoEShape(hidden=256, inter=128, n_experts=16, top_k=4, n_layers=1)
+        lw = synth.make_layer_weights(shape, 5, w_std=0.05, gate_std=0.2)
+        T, want_launches = 300, 5
+    elif case == "c5_T256":
+        shape = dataclasses.replace(synth.SHAPE_C5, n_layers=1)
+        lw = synth.make_layer_weights(shape, 5)
+        T, want_launches = 256, 5
+    else:
+        shape = synth.SHAPE_QWEN
+        lw = synth.make_layer_weights(shape, synth.WEIGHT_SEED)
+        T, want_launches = 64, 1
+    E, k = shape.n_experts, shape.top_k
+    dl = gpu.DecodeLayer(shape, lw, max_T=T)
+    xs = [synth.make_hidden(T, shape.hidden, 900 + i) for i in range(3)]
+    x = gpu.bf16_from_bits(xs[0]).clone()
+    token_req, token_block = synth.decode_maps(T)
+    d_req, d_blk = torch.from_numpy(token_req).cuda(), torch.from_numpy(token_block).cuda()
+    sig_req = torch.zeros((T, 1, E), dtype=torch.int32, device="cuda")
+    sig_blk = torch.zeros((T, 1, E), dtype=torch.int8, device="cuda")
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        dl.run(x, None, token_req=d_req, token_block=d_blk, sig_req=sig_req, sig_block=sig_blk)     # warm-up (attributes)
+        assert gpu.eldr_moe_last_launch_count() == want_launches
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            dl.run(x, None, token_req=d_req, token_block=d_blk, sig_req=sig_req, sig_block=sig_blk)
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    for rep in (1, 2, 0, 2):
+        x.copy_(gpu.bf16_from_bits(xs[rep]))
+        dl.out.zero_(); dl.ids.zero_(); dl.w.zero_(); sig_req.zero_(); sig_blk.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        ora = oracle.moe_decode_layer(shape, xs[rep], lw.gate_w, None, lw.w13, lw.w2, lw.shared_w13, lw.shared_w2)
+        clean = check_gate(shape, ora, dl.ids[:T].cpu().numpy(), dl.w[:T].cpu().numpy())
+        check_numeric(dl.out[:T].float().cpu().numpy()[clean], ora["out"][clean], "out (replay on x%d)" % rep)
+        if clean.all():
+            o_req = np.zeros((T, 1, E), np.int32)
+            o_blk = np.zeros((T, 1, E), np.int8)
+            oracle.signature_accumulate(shape, 0, ora["ids"], token_req, token_block, o_req, o_blk)
+            assert np.array_equal(sig_req.cpu().numpy(), o_req) and np.array_equal(sig_blk.cpu().numpy(), o_blk)
+            assert int(dl.n_active.item()) == ora["n_active"]
 
 
 @pytest.mark.parametrize("min_rounds", [1, 1 << 20])
