@@ -187,6 +187,11 @@ int32_t eldr_moe_workspace_layout(const eldr_moe_shape_t* shape, int32_t T, eldr
 #define ELDR_OPT_DP_MIN_ROUNDS 4 /* fused step: a phase whose tile count is at least this many rounds of the grid runs its
                                  whole rounds round-robin (no split tiles) and only the remainder as stream-K; below it the
                                  whole phase is stream-K.  1..2^20; default 4 */
+#define ELDR_OPT_SK_SPLIT_PCT 6 /* fused step, small unions (w1/w3 phase shorter than ELDR_OPT_DP_MIN_ROUNDS rounds of tiles): the
+                                 active experts are cut into two groups and the step runs w1/w3(g0) w1/w3(g1) w2(g0) w2(g1);
+                                 value = percentage of the experts in g0 (0 or 100: one group).  0..100; default 0: measured on
+                                 B200 the two-group order is SLOWER (|U| = 16: 76 vs 60 us) -- each group's share per SM is
+                                 shorter than one weight tile, so every tile is cut three ways and the fix-ups have no slack */
 #define ELDR_OPT_FFN_PAIR 5   /* prefill-shaped calls (T > 1024, I % 128 == 0, H % 256 == 0): the expert FFN as tcgen05
                                  cta_group::2 tiles (M = 256 over an SM pair, ffn_umma2.cuh).  1 (default): when the call
                                  has >= 256 tokens per expert on average (T*k >= 256*E); 2: always; 0: never (one CTA

@@ -30,6 +30,7 @@ OPT_STEP_PATH, STEP_STAGED, STEP_FUSED, STEP_AUTO = 2, 0, 1, 2
 OPT_RING_KB = 3
 OPT_DP_MIN_ROUNDS = 4
 OPT_FFN_PAIR = 5
+OPT_SK_SPLIT_PCT = 6
 PROFILE_SLOTS = ("gate", "route", "gather", "ffn13", "ffn2", "combine")
 
 

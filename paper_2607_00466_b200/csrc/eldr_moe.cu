@@ -29,6 +29,7 @@ int g_pdl = 1;
 int g_step_path = ELDR_STEP_AUTO;
 int g_ring_kb = 208;
 int g_dp_min_rounds = 4;
+int g_sk_split_pct = 0;
 
 thread_local char g_err[256] = "";
 thread_local int g_launches = 0;
@@ -100,7 +101,7 @@ void make_layout(const eldr_moe_shape_t* s, int T, eldr_moe_ws_layout_t* L) {
   auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + bytes, 256); return r; };
   // epoch flags first, at a T-independent offset and size: the fused kernel keeps its generation word there
   const size_t sync_staged = ((size_t)((kFusedMaxT > (int)Tz ? kFusedMaxT : Tz) + kGateTok - 1) / kGateTok * ((E + kGateExp - 1) / kGateExp + 2) + 2) * 4;
-  const size_t sync_fused = fused_sync_words((int)E, (int)ns, (int)I) * 4;
+  const size_t sync_fused = fused_sync_words((int)E, (int)ns, (int)I, (int)H) * 4;
   L->sync = take(align_up(sync_fused, 256) + sync_staged);   // [fused | staged]: never aliased (both derive epochs)
   const int zs = gate_slices(s, T);
   L->z = take(Tz * E * 4 * (zs > 1 ? zs : 1));              // prefill-shaped gate: one partial logit tensor per slice
@@ -351,6 +352,10 @@ int32_t eldr_moe_set_option(int32_t key, int32_t value) {
     g_dp_min_rounds = value;
     return ELDR_OK;
   }
+  if (key == ELDR_OPT_SK_SPLIT_PCT && value >= 0 && value <= 100) {
+    g_sk_split_pct = value;
+    return ELDR_OK;
+  }
   return ELDR_ERR_INVALID_ARG;
 }
 
@@ -468,7 +473,8 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
     fa.perm = perm; fa.pair_pos = pair_pos; fa.work = work; fa.n_work = n_work;
     fa.active = active_experts; fa.n_active = n_active;
     fa.sync = reinterpret_cast<uint32_t*>(ws + L.sync);
-    fa.idt = reinterpret_cast<unsigned long long*>(fa.sync + fused_idt_word_offset(E, ns, I));
+    fa.idt = reinterpret_cast<unsigned long long*>(fa.sync + fused_idt_word_offset(E, ns, I, H));
+    fa.wtag = reinterpret_cast<unsigned long long*>(fa.sync + fused_wtag_word_offset(E, ns, I, H));
     fa.hbuf = hbuf; fa.ybuf = ybuf; fa.out = out;
     fa.partial = reinterpret_cast<float*>(ws + L.partial);
     const size_t smem_max = 227 * 1024;
@@ -478,6 +484,7 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
     fa.stage_area = fixed < smem_max ? (int)((smem_max - fixed) / 1024 * 1024) : 0;
     fa.ring_bytes = g_ring_kb * 1024;
     fa.dp_min_rounds = g_dp_min_rounds;
+    fa.sk_split_pct = g_sk_split_pct;
     const size_t smem = fixed + fa.stage_area;
     if ((size_t)fa.stage_area >= min_area) {
       CUtensorMap tm_w13, tm_sw13, tm_w2, tm_sw2, tm_x, tm_h;
@@ -491,9 +498,6 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
       } else {
         tm_sw13 = tm_w13;
         tm_sw2 = tm_w2;
-#ifdef ELDR_EXP_W13_2D
-        if (!make_tmap(&tm_sw13, w13, (uint64_t)E * 2 * I, H, 128)) return ELDR_ERR_CUDA;
-#endif
       }
       static bool fused_attr_set = false;
       if (!fused_attr_set) {
@@ -553,7 +557,7 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
     // last group runs the permutation / union compaction
     GateRouteArgs ga;
     ga.x = x; ga.gate_w = gate_w; ga.gate_bias = gate_bias; ga.r = ra;
-    ga.sync = reinterpret_cast<uint32_t*>(ws + L.sync + align_up(fused_sync_words(E, ns, I) * 4, 256));
+    ga.sync = reinterpret_cast<uint32_t*>(ws + L.sync + align_up(fused_sync_words(E, ns, I, H) * 4, 256));
     size_t smem = (size_t)kGateTok * H * 2;
     if (route_smem > smem) smem = route_smem;
     if (smem > 200 * 1024) return ELDR_ERR_UNSUPPORTED;

@@ -52,22 +52,32 @@ constexpr int kClaimSlots = 4;            // claimed-tile ring: weights producer
 constexpr int kSyncGen = 0;
 constexpr int kSyncCntReady = 1;                // CTA 0 zeroed this step's tile counters
 constexpr int kSyncTileCnt = 2;                 // [2] next unclaimed data-parallel tile of phase A / B
-constexpr int kSyncDone = 32;                   // [256]     per CTA "all my pieces are finished"
+constexpr int kSyncExit = 4;                    // CTAs that have left the step (zeroed by CTA 0 with the tile counters; the last one bumps the generation)
+constexpr int kSyncDone = 32;                   // [256]     (unused since the flag-driven combine; kept for layout stability)
 constexpr int kSyncGroup = kSyncDone + 256;     // [32]      per token group "ids/weights written"
 constexpr int kSyncTile = kSyncGroup + 32;      // [32][32]  gate logit tile written
 constexpr int kSyncPartial = kSyncTile + 1024;  // [4][256]  per (sub-phase, CTA) "partial accumulators parked"
-constexpr int kSyncHReady = kSyncPartial + 1024; // [(E+ns)*2*tilesA] per phase-A tile "h tile written"
+constexpr int kSyncHReady = kSyncPartial + 1024; // [(E+ns)*2*tilesA] per phase-A tile "h tile written", then
+                                                 // [(E+ns)*2*tilesB] per phase-B tile "y tile written"
 
 // Tagged ids: one 64-bit word {epoch : 32 | four expert ids, one byte each : 32} per (token, group of four top-k
 // slots), written by the token group's owner after its top-k and polled by every CTA.  Tag and payload arrive in one
 // atomic 8-byte access, so the routing input needs no flag, no release and no second L2 round trip.  (The same
 // scheme for the logits was measured slower than tile flags + plain loads and is not used.)
 constexpr int kIdWordsPerTok = 4;         // kMaxTopK / 4
-__host__ __device__ inline size_t fused_idt_word_offset(int E, int ns, int I) {
-  return ((size_t)kSyncHReady + (size_t)(E + ns) * 2 * ((I + 63) / 64) + 1) & ~(size_t)1;
+__host__ __device__ inline size_t fused_ydone_word_offset(int E, int ns, int I) {
+  return (size_t)kSyncHReady + (size_t)(E + ns) * 2 * ((I + 63) / 64);
 }
-__host__ __device__ inline size_t fused_sync_words(int E, int ns, int I) {
-  return fused_idt_word_offset(E, ns, I) + (size_t)kFusedMaxT * kIdWordsPerTok * 2;
+__host__ __device__ inline size_t fused_idt_word_offset(int E, int ns, int I, int H) {
+  return (fused_ydone_word_offset(E, ns, I) + (size_t)(E + ns) * 2 * ((H + 127) / 128) + 1) & ~(size_t)1;
+}
+// Tagged weights: {epoch : 32 | fp32 weight : 32} per (token, slot), written by the top-k owner and polled by the
+// warp that combines the token -- value and tag in one atomic word, so the combine needs no fence for them.
+__host__ __device__ inline size_t fused_wtag_word_offset(int E, int ns, int I, int H) {
+  return fused_idt_word_offset(E, ns, I, H) + (size_t)kFusedMaxT * kIdWordsPerTok * 2;
+}
+__host__ __device__ inline size_t fused_sync_words(int E, int ns, int I, int H) {
+  return fused_wtag_word_offset(E, ns, I, H) + (size_t)kFusedMaxT * 16 * 2;
 }
 __host__ __device__ inline size_t fused_partial_bytes(int n_cta) {
   return (size_t)4 * n_cta * 128 * kNPCap * 4;
@@ -89,6 +99,7 @@ struct FusedArgs {
   int32_t* n_active;
   uint32_t* sync;
   unsigned long long* idt;     // [T][4] tagged top-k ids (inside the sync region)
+  unsigned long long* wtag;    // [T][16] tagged top-k weights (inside the sync region)
   float* partial;              // [4][gridDim.x][128][kNPCap] fp32 scratch of the stream-K fix-up
   uint16_t* hbuf;              // [T*(k+ns), I] bf16
   float* ybuf;                 // [T*(k+ns), H] fp32
@@ -96,6 +107,7 @@ struct FusedArgs {
   int stage_area;              // bytes of shared memory cut into ring stages (multiple of 1024; set by the host)
   int ring_bytes;              // cap on the bytes the ring keeps in flight (<= stage_area)
   int dp_min_rounds;           // hybrid schedule: data-parallel part only if a phase has at least this many tile rounds
+  int sk_split_pct;            // small unions (whole phase stream-K): share of the accumulator passes in the first expert group
 };
 
 #ifdef ELDR_TRACE
@@ -109,7 +121,11 @@ __device__ __forceinline__ unsigned long long gtime() {
 #define FVALUE2(id, v) do { g_trace[((blockIdx.x + 2048) & 4095) * 16 + (id)] = (unsigned long long)(v); } while (0)
 #define FSTAMP2(id) do { g_trace[((blockIdx.x + 2048) & 4095) * 16 + (id)] = gtime(); } while (0)
 #define FTIMED(acc, stmt) do { const long long c0_ = clock64(); stmt; acc += clock64() - c0_; } while (0)
+#define FSTAMP3(id) do { g_trace[((blockIdx.x + 1024) & 4095) * 16 + (id)] = gtime(); } while (0)
+#define FADD3(id, v) do { g_trace[((blockIdx.x + 1024) & 4095) * 16 + (id)] += (unsigned long long)(v); } while (0)
 #else
+#define FSTAMP3(id) do {} while (0)
+#define FADD3(id, v) do {} while (0)
 #define FSTAMP2(id) do {} while (0)
 #define FVALUE2(id, v) do {} while (0)
 #define FTIMED(acc, stmt) do { stmt; } while (0)
@@ -347,7 +363,7 @@ struct FusedSmem {
   uint16_t* tok_of_pos;    // [T*k (+T)]
   uint16_t* pos_of_pair;   // [T*k]
   uint8_t* ids8;           // [T*k] expert id of each pair (E <= 256)
-  uint8_t* route_scratch;  // mask [E][W], pref [E][W], cnt [E], off [E+1] (part a -> part b)
+  uint8_t* route_scratch;  // mask [E][W], pref [E][W], ent [E], off [E+1], scan totals [32] (part a -> part b, combine)
 };
 
 // Bytes of everything except the stage ring (barriers, routing tables); the host gives the ring what is left.
@@ -360,20 +376,24 @@ __host__ __device__ inline size_t fused_smem_fixed_bytes(int E, int ns, int T, i
   o += (((size_t)T * k + T) * 2 + 15) / 16 * 16;
   o += ((size_t)T * k * 2 + 15) / 16 * 16;
   o += ((size_t)T * k + 15) / 16 * 16;
-  o += ((size_t)E * W * 8 + (size_t)(2 * E + 1) * 4 + 15) / 16 * 16;   // route scratch: mask, pref, cnt, off
+  o += ((size_t)E * W * 8 + (size_t)(2 * E + 1 + 32) * 4 + 15) / 16 * 16;   // route scratch: mask, pref, ent, off, scan totals
   return o + 1024;                                       // alignment slack
 }
 
 // ------------------------------------------------------------------------------ R (part a): union + work list
-// Scratch (mask, pref, s_cnt, s_off) has its own shared-memory region: part b still reads it while the weights
-// producer is already filling the stage ring.
+// Scratch (mask, pref, s_ent, s_off, s_blk) has its own shared-memory region: part b still reads it while the weights
+// producer is already filling the stage ring.  All 256 threads take part: thread e owns expert e (E <= 256) -- its
+// count from the membership words, then one block-wide scan (warp shuffles + eight warp totals) gives the offsets
+// and, through a ballot, the slot of every active expert in the union-compacted work list.  (The one-warp scan of
+// round 1 cost 2.5 us of the serial prelude.)
 __device__ __forceinline__ void fused_route_a(const FusedArgs& a, const FusedSmem& sm, uint8_t* scratch, bool is_cta0) {
   const int T = a.tk.T, E = a.tk.E, k = a.tk.k, ns = a.n_shared;
   const int W = (T + 31) >> 5;
   uint32_t* mask = reinterpret_cast<uint32_t*>(scratch);     // [E][W]
   uint32_t* pref = mask + (size_t)E * W;                      // [E][W]
-  int32_t* s_cnt = reinterpret_cast<int32_t*>(pref + (size_t)E * W);
-  int32_t* s_off = s_cnt + E;                                 // [E+1]
+  int32_t* s_ent = reinterpret_cast<int32_t*>(pref + (size_t)E * W);   // [E] work-list entry of expert e (-1: inactive)
+  int32_t* s_off = s_ent + E;                                 // [E+1]
+  int32_t* s_blk = s_off + E + 1;                             // [32] warp totals of the block scans
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const bool do_sig = is_cta0 && a.force_routing;
 
@@ -398,107 +418,98 @@ __device__ __forceinline__ void fused_route_a(const FusedArgs& a, const FusedSme
   }
   __syncthreads();
   if (threadIdx.x == 0) FSTAMP2(5);
-  for (int e = tid; e < E; e += kFusedThreads) {
-    int run = 0;
+  // thread e: count of expert e and the per-word prefixes the position maps need
+  int c = 0;
+  if (tid < E) {
     for (int w = 0; w < W; ++w) {
-      pref[e * W + w] = run;
-      run += __popc(mask[e * W + w]);
+      pref[tid * W + w] = c;
+      c += __popc(mask[tid * W + w]);
     }
-    s_cnt[e] = run;
   }
+  const uint32_t act_ballot = __ballot_sync(0xffffffffu, c > 0);
+  int cinc = c;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int cv = __shfl_up_sync(0xffffffffu, cinc, o);
+    if (lane >= o) cinc += cv;
+  }
+  const int wmax = (int)__reduce_max_sync(0xffffffffu, (unsigned)c);
+  if (lane == 31) { s_blk[warp] = cinc; s_blk[8 + warp] = __popc(act_ballot); s_blk[16 + warp] = wmax; }
   __syncthreads();
   if (threadIdx.x == 0) FSTAMP2(6);
-  if (warp == 0) {
-    constexpr int PER = kMaxExperts / 32;
-    const int per = (E + 31) >> 5;                  // experts per lane: all 32 lanes work whatever E is
-    int c[PER], csum = 0, asum = 0, cmax = 0;
+  int cbase = 0, abase = 0, total = 0, n_act = 0, cmax = 0;
 #pragma unroll
-    for (int i = 0; i < PER; ++i) {
-      const int e = lane * per + i;
-      c[i] = (i < per && e < E) ? s_cnt[e] : 0;
-      csum += c[i];
-      asum += (c[i] > 0);
-      cmax = max(cmax, c[i]);
+  for (int w = 0; w < kFusedThreads / 32; ++w) {
+    const int cw = s_blk[w], aw = s_blk[8 + w];
+    if (w < warp) { cbase += cw; abase += aw; }
+    total += cw; n_act += aw;
+    cmax = max(cmax, s_blk[16 + w]);
+  }
+  if (ns) cmax = T;
+  const int n_work = n_act + ns;
+  if (tid < E) {
+    const int coff = cbase + cinc - c;
+    const int aoff = abase + __popc(act_ballot & ((1u << lane) - 1u));
+    s_off[tid] = coff;
+    s_ent[tid] = c > 0 ? aoff : -1;
+    if (is_cta0) { a.off[tid] = coff; a.cnt[tid] = c; }
+    if (c > 0) {
+      const int4 wk = make_int4(tid, coff, coff, c);
+      sm.work[aoff] = wk;
+      if (is_cta0) { a.active[aoff] = tid; a.work[aoff] = wk; }
     }
-    int cinc = csum, ainc = asum;
+    if (is_cta0 && tid >= n_act) a.active[tid] = -1;
+  }
+  if (tid < ns) {
+    const int4 wk = make_int4(E + tid, T * k, T * k + tid * T, T);
+    sm.work[n_act + tid] = wk;
+    if (is_cta0) a.work[n_act + tid] = wk;
+  }
+  if (tid == 0) {
+    const int np = (min(cmax, kNPCap) + 15) & ~15;
+    s_off[E] = total;
+    sm.meta[0] = n_work;
+    sm.meta[1] = np;
+    sm.meta[2] = min(kMaxStages, max(min(a.stage_area, a.ring_bytes), 3 * (kUmmaWBytes + np * 128)) / (kUmmaWBytes + np * 128));
+    if (is_cta0) { a.off[E] = total; *a.n_active = n_act; *a.n_work = n_work; }
+  }
+  // accumulator passes per entry (1 unless an expert got more than kNPCap tokens) and their exclusive scan
+  if (cmax <= kNPCap) {
+    // every entry fits one accumulator pass (the usual decode case): the pass table is the identity
+    for (int ent = tid; ent <= n_work; ent += kFusedThreads) sm.cumpass[ent] = ent;
+    if (tid == 0) sm.meta[3] = n_work;
+    __syncthreads();
+  } else {
+    __syncthreads();                                 // the work list is complete
+    // entries <= E + ns <= 264: thread `tid` takes entry tid, thread 0..7 also entry 256 + tid; two-level scan again
+    const int ps0 = tid < n_work ? (sm.work[tid].w + kNPCap - 1) / kNPCap : 0;
+    int pinc = ps0;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
-      const int cv = __shfl_up_sync(0xffffffffu, cinc, o);
-      const int av = __shfl_up_sync(0xffffffffu, ainc, o);
-      if (lane >= o) { cinc += cv; ainc += av; }
+      const int pv = __shfl_up_sync(0xffffffffu, pinc, o);
+      if (lane >= o) pinc += pv;
     }
-    cmax = (int)__reduce_max_sync(0xffffffffu, (unsigned)cmax);
-    if (ns) cmax = T;
-    int coff = cinc - csum, aoff = ainc - asum;
-    const int n_act = __shfl_sync(0xffffffffu, ainc, 31);
-    const int total = __shfl_sync(0xffffffffu, cinc, 31);
+    if (lane == 31) s_blk[24 + warp] = pinc;
+    __syncthreads();
+    int pbase = 0, ptot = 0;
 #pragma unroll
-    for (int i = 0; i < PER; ++i) {
-      const int e = lane * per + i;
-      if (i < per && e < E) {
-        s_off[e] = coff;
-        if (is_cta0) { a.off[e] = coff; a.cnt[e] = c[i]; }
-        if (c[i] > 0) {
-          const int4 wk = make_int4(e, coff, coff, c[i]);
-          sm.work[aoff] = wk;
-          if (is_cta0) { a.active[aoff] = e; a.work[aoff] = wk; }
-          ++aoff;
-        }
-        coff += c[i];
-      }
+    for (int w = 0; w < kFusedThreads / 32; ++w) {
+      const int pw_ = s_blk[24 + w];
+      if (w < warp) pbase += pw_;
+      ptot += pw_;
     }
-    if (is_cta0)
-      for (int i = n_act + lane; i < E; i += 32) a.active[i] = -1;
-    if (lane < ns) {
-      const int4 wk = make_int4(E + lane, T * k, T * k + lane * T, T);
-      sm.work[n_act + lane] = wk;
-      if (is_cta0) a.work[n_act + lane] = wk;
-    }
-    __syncwarp();
-    // accumulator passes per entry (1 unless an expert got more than kNPCap tokens) and their exclusive scan
-    const int n_work = n_act + ns;
-    constexpr int PER2 = (kMaxExperts + 8 + 31) / 32;
-    int pinc;
-    if (cmax <= kNPCap) {
-      // every entry fits one accumulator pass (the usual decode case): the pass table is the identity
-      for (int ent = lane; ent < n_work; ent += 32) sm.cumpass[ent] = ent;
-      pinc = n_work;
-    } else {
-      int ps = 0;
-#pragma unroll
-      for (int i = 0; i < PER2; ++i) {
-        const int ent = lane * PER2 + i;
-        if (ent < n_work) ps += (sm.work[ent].w + kNPCap - 1) / kNPCap;
+    if (tid < n_work) sm.cumpass[tid] = pbase + pinc - ps0;
+    if (tid == 0) {
+      int run = ptot;
+      for (int ent = kFusedThreads; ent < n_work; ++ent) {          // at most ns = 8 entries past the block
+        sm.cumpass[ent] = run;
+        run += (sm.work[ent].w + kNPCap - 1) / kNPCap;
       }
-      pinc = ps;
-#pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        const int pv = __shfl_up_sync(0xffffffffu, pinc, o);
-        if (lane >= o) pinc += pv;
-      }
-      int poff = pinc - ps;
-#pragma unroll
-      for (int i = 0; i < PER2; ++i) {
-        const int ent = lane * PER2 + i;
-        if (ent < n_work) {
-          sm.cumpass[ent] = poff;
-          poff += (sm.work[ent].w + kNPCap - 1) / kNPCap;
-        }
-      }
-      pinc = __shfl_sync(0xffffffffu, pinc, 31);
+      sm.cumpass[n_work] = run;
+      sm.meta[3] = run;
     }
-    if (lane == 31) sm.cumpass[n_work] = pinc;
-    if (lane == 0) {
-      const int np = (min(cmax, kNPCap) + 15) & ~15;
-      s_off[E] = total;
-      sm.meta[0] = n_work;
-      sm.meta[1] = np;
-      sm.meta[2] = min(kMaxStages, max(min(a.stage_area, a.ring_bytes), 3 * (kUmmaWBytes + np * 128)) / (kUmmaWBytes + np * 128));
-      if (is_cta0) { a.off[E] = total; *a.n_active = n_act; *a.n_work = n_work; }
-    }
-    if (lane == 31) sm.meta[3] = pinc;
+    __syncthreads();
   }
-  __syncthreads();
   if (threadIdx.x == 0) FSTAMP2(7);
 }
 
@@ -547,22 +558,38 @@ struct PieceWalker {
   int dp_tile, dp_end, G;
   bool dp;
   __device__ __forceinline__ void init(int sp, int tilesA, int tilesB, int kitA, int kitB, int total_pass,
-                                       const int32_t* cp, int cta, int G_, int min_rounds) {
+                                       const int32_t* cp, int cta, int G_, int min_rounds, int split_pct) {
     const int ph = sp >> 1;
     tpe = ph == 0 ? tilesA : tilesB;
     kit = ph == 0 ? kitA : kitB;
     G = G_;
     const int n_tiles = total_pass * tpe;
-    const int R0 = (n_tiles / G >= min_rounds) ? (n_tiles / G) * G : 0;   // few rounds: all stream-K
-    dp = (sp & 1) == 0;
-    dp_tile = cta;
-    dp_end = R0;
-    tile0 = R0;
-    P = (long long)(n_tiles - R0) * kit;
-    g = P * cta / G;
-    hi = P * (cta + 1) / G;
     ent = 0;
     cumpass = cp;
+    dp_tile = cta;
+    if (total_pass * tilesA / G >= min_rounds) {
+      // large union: sub-phases A-dp, A-remainder, B-dp, B-remainder
+      const int R0 = (n_tiles / G >= min_rounds) ? (n_tiles / G) * G : 0;   // few rounds: all stream-K
+      dp = (sp & 1) == 0;
+      dp_end = R0;
+      tile0 = R0;
+      P = (long long)(n_tiles - R0) * kit;
+    } else {
+      // small union (phase A shorter than min_rounds rounds of tiles): the accumulator passes -- experts, in order --
+      // are cut into two groups and the sub-phases run A(g0) A(g1) B(g0) B(g1), each a static stream-K cut of its own
+      // stage sequence.  B(g0) starts on h tiles that were finished a whole A(g1) earlier and B(g1) on tiles finished a
+      // whole B(g0) earlier, so the w1/w3 -> w2 hand-over no longer drains the pipeline (with one stream-K cut per
+      // phase every expert had an h tile finished in the last microsecond of A: the activation producers idled a
+      // median 8 us at |U| = 16).  The decision needs n_active, so it is taken here, in the kernel.
+      const int p_split = min(total_pass, (total_pass * split_pct + 50) / 100);
+      const int t_lo = (sp & 1) ? p_split * tpe : 0, t_hi = (sp & 1) ? n_tiles : p_split * tpe;
+      dp = false;
+      dp_end = 0;
+      tile0 = t_lo;
+      P = (long long)(t_hi - t_lo) * kit;
+    }
+    g = P * cta / G;
+    hi = P * (cta + 1) / G;
   }
   // data-parallel part: `claimed` is the tile this CTA drew from the phase's counter (ascending per CTA), or
   // anything >= dp_end / negative when the part is exhausted.  Remainder part: `claimed` is ignored.
@@ -633,6 +660,10 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
   auto cempty_bar = [&](int b) { return sm.bar_base + 8u * (2 * kMaxStages + 4 + kClaimSlots + b); };
 
   // ------------------------------------------------------------- prologue (overlaps the previous kernel's tail)
+  if (tid == 0) FSTAMP2(8);
+#ifdef ELDR_TRACE
+  const unsigned long long t_entry_ = gtime();
+#endif
   if (tid == 0) {
     for (int s = 0; s < kMaxStages; ++s) { mbar_init(full_bar(s), 2); mbar_init(empty_bar(s), 1); }
     for (int b = 0; b < 2; ++b) { mbar_init(tfull_bar(b), 1); mbar_init(tempty_bar(b), 4); }
@@ -664,10 +695,14 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
   if (tid == 0) FSTAMP(1);
 
   const uint32_t epoch = __ldcg(a.sync + kSyncGen) + 1u;
+#ifdef ELDR_TRACE
+  if (tid == 0) atomicMax(&g_trace[(3000 + (epoch & 63)) * 16 + 0], ~t_entry_);     // earliest CTA entry of this step
+#endif
   if (cta == 0 && tid == 0) {
     // this step's tile counters (the previous grid has completed: pdl_wait above)
     a.sync[kSyncTileCnt] = 0u;
     a.sync[kSyncTileCnt + 1] = 0u;
+    a.sync[kSyncExit] = 0u;
     flag_release(a.sync + kSyncCntReady, epoch);
   }
 
@@ -699,6 +734,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
         if (lane < k) {
           a.tk.ids[(size_t)t * k + lane] = id;
           a.tk.w[(size_t)t * k + lane] = w;
+          st_relaxed_u64(a.wtag + (size_t)t * kMaxTopK + lane, ((unsigned long long)epoch << 32) | __float_as_uint(w));
           sig_add(a.tk.sig_req, a.tk.sig_block, a.tk.token_req ? a.tk.token_req[t] : -1,
                   a.tk.token_block ? a.tk.token_block[t] : -1, a.tk.L, a.tk.layer, E, id);
         }
@@ -745,7 +781,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
   const int kitA = H / 64, kitB = I / 64;
   uint32_t* hready = a.sync + kSyncHReady;
   uint32_t* pready = a.sync + kSyncPartial;
-  (void)n_work;
+  uint32_t* ydone = a.sync + fused_ydone_word_offset(E, ns, I);
 
   // Consumer side of the claimed-tile ring (a converged warp; `cn` = claims this warp has popped so far).
   auto claim_pop = [&](uint32_t& cn) -> int {
@@ -791,7 +827,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
       for (int sp = 0; sp < 4; ++sp) {
         const int ph = sp >> 1;
         PieceWalker pw;
-        pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds);
+        pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds, a.sk_split_pct);
         Piece p;
         auto stream_piece = [&]() {
           const int4 wk = sm.work[p.ent];
@@ -833,6 +869,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
           while (pw.next(p, 0)) stream_piece();
         }
         if (sp == 1) FSTAMP(11);
+        FSTAMP3(sp);
       }
       FSTAMP(7);
       FVALUE2(0, w_wait[0]); FVALUE2(1, w_wait[1]); FVALUE2(10, w_iss[0]); FVALUE2(11, w_iss[1]);
@@ -847,6 +884,12 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     // Two warps alternate ring stages.
     const uint32_t xw = warp == 7 ? 1u : 0u;
     const uint64_t xpol = l2_policy_evict_last();
+    if (warp == 5 && lane == 0) {
+      // CTA 0 zeroed this step's counters (tile draws, leavers): observed once per CTA, off the critical path
+      uint32_t spins = 0;
+      while (flag_acquire(a.sync + kSyncCntReady) != epoch) { __nanosleep(100); if (++spins > (1u << 22)) __trap(); }
+    }
+    __syncwarp();
     uint32_t it = 0, cn = 0;
 #ifdef ELDR_TRACE
     unsigned long long stall = 0, nb = 0;
@@ -854,7 +897,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     for (int sp = 0; sp < 4; ++sp) {
       const int ph = sp >> 1;
       PieceWalker pw;
-      pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds);
+      pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds, a.sk_split_pct);
       Piece p;
       int ready_ent = -1;
       while (consumer_next(pw, p, cn)) {
@@ -871,6 +914,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
             warp_wait_flags(fl, nfl, epoch, lane);
 #ifdef ELDR_TRACE
             stall += gtime() - t0_; ++nb;
+            if (lane == 0 && xw == 0) FADD3(8 + sp, gtime() - t0_);
 #endif
           }
           fence_proxy_async_all();
@@ -926,7 +970,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     bool first = true;
     for (int sp = 0; sp < 4; ++sp) {
       PieceWalker pw;
-      pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds);
+      pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds, a.sk_split_pct);
       Piece p;
       while (consumer_next(pw, p, cn)) {
         const int4 wk = sm.work[p.ent];
@@ -960,7 +1004,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     for (int sp = 0; sp < 4; ++sp) {
       const int ph = sp >> 1;
       PieceWalker pw;
-      pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds);
+      pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds, a.sk_split_pct);
       const long long P = pw.P;
       Piece p;
       while (consumer_next(pw, p, cn)) {
@@ -985,7 +1029,13 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
             if (hj > covered) {                              // CTA j owns a non-empty piece of this tile
               if (lane == 0) {
                 uint32_t spins = 0;
+#ifdef ELDR_TRACE
+                const unsigned long long tp0_ = gtime();
+#endif
                 while (flag_acquire(pready + sp * 256 + j) != epoch) { __nanosleep(40); if (++spins > (1u << 24)) __trap(); }
+#ifdef ELDR_TRACE
+                if (tid == 0) FADD3(12 + sp, gtime() - tp0_);
+#endif
               }
               covered = min(hj, tile_end);
               n_partner = j - cta;
@@ -1059,11 +1109,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
                 const float gv = lo ? v[kk] : recv;
                 const float uv = lo ? recv : v[8 + kk];
                 const int tok = n0 + c0 + (lo ? kk : 8 + kk);
-#ifdef ELDR_EXP_NOEPI
-                if (tok < 0)
-#else
                 if (tok < wk.w)
-#endif
                   a.hbuf[(size_t)(wk.z + tok) * I + i] = f32_to_bf16_rn(__fdividef(gv, 1.0f + __expf(-gv)) * uv);
               }
             } else {
@@ -1072,11 +1118,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
 #pragma unroll
                 for (int kk = 0; kk < 16; ++kk) {
                   const int tok = n0 + c0 + kk;
-#ifdef ELDR_EXP_NOEPI
-                  if (tok < 0)
-#else
                   if (tok < wk.w)
-#endif
                     a.ybuf[(size_t)(wk.z + tok) * H + r] = v[kk];
                 }
               }
@@ -1097,20 +1139,34 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
             fence_proxy_async_all();
             asm volatile("bar.sync 1, 128;" ::: "memory");
             if (tid == 0) { flag_release(hready + p.tile, epoch); FSTAMP(15); }
+          } else {
+            // publish "y tile written" for the flag-driven combine
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+            if (tid == 0) flag_release(ydone + p.tile, epoch);
           }
         }
         ++piece_no;
       }
+      if (tid == 0) FSTAMP3(4 + sp);
     }
   }
 
-  // ------------------------------------------------------------------------------ grid barrier, then C: combine
+  // ------------------------------------------------------------------------------ C: flag-driven combine
+  // No grid barrier: the unit of combine work is (token t, 128-column tile rt) = one warp pass; lane j < k looks up
+  // slot j's y tile (work entry of the expert, accumulator pass of the position, rt) and polls that tile's "y
+  // written" flag, lanes k..k+ns-1 do the same for the shared experts; when all are up the warp sums the k (+ns) rows
+  // in slot order -- a fixed order, so results stay run-to-run bit-identical -- and rounds once to bf16.  Every warp
+  // CTA starts on its units as soon as its own FFN roles have run out of pieces, so the combine of tokens whose
+  // experts finished early overlaps the last tiles of the slow SMs (round 1: every SM waited for the slowest one, then
+  // combined: barrier + combine 3.4 us after the last tile).  Polls are one 4-byte load per slot and sleep 250 ns in
+  // between: warps that polled from the moment their role ended, all lanes, every 100 ns, hot-spotted the flags' L2
+  // lines and cost every step 40 us (measured).
+#ifdef ELDR_OLD_TAIL
   if (tid == 0) FSTAMP(8);
   __syncthreads();
   if (tid == 0) flag_release(a.sync + kSyncDone + cta, epoch);
   if (warp == 0) warp_wait_flags(a.sync + kSyncDone, G, epoch, lane);
   __syncthreads();
-  if (tid == 0) FSTAMP(9);
   {
     const int q_per_row = H >> 2;
     for (int idx = cta * kFusedThreads + tid; idx < T * q_per_row; idx += G * kFusedThreads) {
@@ -1142,13 +1198,103 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     }
   }
   if (tid == 0) FSTAMP(10);
-  if (cta == 0 && tid == 0) a.sync[kSyncGen] = epoch;      // every CTA read gen before its done flag
+  if (cta == 0 && tid == 0) a.sync[kSyncGen] = epoch;
+  tc_fence_before();
+  __syncthreads();
+#else
+  if (tid == 0) FSTAMP(8);
+  __syncthreads();
+  {
+    const int32_t* s_ent = reinterpret_cast<const int32_t*>(sm.route_scratch + (size_t)E * ((T + 31) >> 5) * 8);
+    const int q_per_row = H >> 2;
+    const int n_units = T * tilesB;
+    const int n_act_ = n_work - ns;
+    for (int u = cta * (kFusedThreads / 32) + warp; u < n_units; u += G * (kFusedThreads / 32)) {
+      const int t = u / tilesB, rt = u - t * tilesB;
+      int pos = 0, fl = -1;
+      float wt = 0.f;
+      const unsigned long long* wsrc = nullptr;
+      if (lane < k) {
+        const int ent = s_ent[sm.ids8[t * k + lane]];
+        pos = sm.pos_of_pair[t * k + lane];
+        fl = (sm.cumpass[ent] + (pos - sm.work[ent].y) / kNPCap) * tilesB + rt;
+        if (a.force_routing) wt = __ldcg(a.tk.w + t * k + lane);
+        else wsrc = a.wtag + (size_t)t * kMaxTopK + lane;
+      } else if (lane < k + ns) {
+        const int ent = n_act_ + (lane - k);
+        pos = T * k + (lane - k) * T + t;
+        fl = (sm.cumpass[ent] + t / kNPCap) * tilesB + rt;
+        wt = 1.0f;
+      }
+      bool w_ok = wsrc == nullptr;
+      for (uint32_t spins = 0;; ++spins) {
+        const bool ok = fl < 0 || flag_relaxed(ydone + fl) == epoch;
+        if (!w_ok) {                                  // written by the top-k owner in the prelude: up on the first look
+          const unsigned long long wv = ld_relaxed_u64(wsrc);
+          w_ok = (uint32_t)(wv >> 32) == epoch;
+          wt = __uint_as_float((uint32_t)wv);
+        }
+        if (__all_sync(0xffffffffu, ok && w_ok)) break;
+        __nanosleep(250);
+        if (spins > (1u << 22)) __trap();
+      }
+      fence_acq_rel_gpu();
+      __syncwarp();
+      const int c4 = rt * 32 + lane;
+      const bool in = c4 < q_per_row;
+      float4 v[kMaxTopK];
+      float wj[kMaxTopK];
+#pragma unroll
+      for (int j = 0; j < kMaxTopK; ++j)
+        if (j < k) {
+          const int pj = __shfl_sync(0xffffffffu, pos, j);
+          wj[j] = __shfl_sync(0xffffffffu, wt, j);
+          if (in) v[j] = __ldcg(reinterpret_cast<const float4*>(a.ybuf + (size_t)pj * H + (size_t)c4 * 4));
+        }
+      float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (in) {
+#pragma unroll
+        for (int j = 0; j < kMaxTopK; ++j)
+          if (j < k) {
+            acc.x = fmaf(wj[j], v[j].x, acc.x); acc.y = fmaf(wj[j], v[j].y, acc.y);
+            acc.z = fmaf(wj[j], v[j].z, acc.z); acc.w = fmaf(wj[j], v[j].w, acc.w);
+          }
+      }
+      for (int s_ = 0; s_ < ns; ++s_) {
+        const int ps = __shfl_sync(0xffffffffu, pos, k + s_);
+        if (in) {
+          const float4 sv = __ldcg(reinterpret_cast<const float4*>(a.ybuf + (size_t)ps * H + (size_t)c4 * 4));
+          acc.x += sv.x; acc.y += sv.y; acc.z += sv.z; acc.w += sv.w;
+        }
+      }
+      if (in) {
+        uint2 o;
+        o.x = (uint32_t)f32_to_bf16_rn(acc.x) | ((uint32_t)f32_to_bf16_rn(acc.y) << 16);
+        o.y = (uint32_t)f32_to_bf16_rn(acc.z) | ((uint32_t)f32_to_bf16_rn(acc.w) << 16);
+        *reinterpret_cast<uint2*>(a.out + (size_t)t * H + (size_t)c4 * 4) = o;
+      }
+    }
+  }
+  if (tid == 0) FSTAMP(10);
 
   tc_fence_before();
   __syncthreads();
+  if (tid == 0) FSTAMP(9);
+  if (tid == 0) {
+    // Leave the step.  The counter was zeroed by CTA 0 in this step's first microsecond (seen here: warp 5 acquired
+    // kSyncCntReady == epoch before its first piece, and the barrier above orders that before this add); the last CTA
+    // to leave publishes the new generation -- every CTA read the old one long before it got here.  One atomicAdd per
+    // CTA: a compare-and-swap loop on an epoch-tagged word serialised the 148 leavers by L2 round trips and cost
+    // every step 30 us (measured).
+    if (atomicAdd(a.sync + kSyncExit, 1u) == (uint32_t)G - 1u) a.sync[kSyncGen] = epoch;
+  }
+#endif
   if (warp == 6) {
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_base), "r"(tmem_cols) : "memory");
   }
+#ifdef ELDR_TRACE
+  if (tid == 0) atomicMax(&g_trace[(3000 + (epoch & 63)) * 16 + 1], gtime());        // latest CTA exit of this step
+#endif
 }
 
 }  // namespace eldr

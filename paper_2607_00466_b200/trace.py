@@ -27,8 +27,8 @@ ROW0 = [(0, "kernel start (after barrier init / TMEM alloc)"), (5, "weights prod
         (13, "MMA issuer: phase A fully issued"), (2, "epilogue: accumulator of the LAST phase-A piece ready"),
         (4, "epilogue: last phase-A piece written (h)"), (15, "last h-tile flag raised"),
         (14, "activations producer: first phase-B (w2) expert ready"), (7, "weights producer: done"),
-        (8, "all FFN roles done"), (9, "grid barrier passed"), (10, "combine done")]
-ROW1 = [(12, "prelude: own gate tiles done"), (13, "prelude: own top-k groups done (owners only)"),
+        (8, "all FFN roles done"), (10, "combine done (warp 0)"), (9, "combine done (all warps)")]
+ROW1 = [(8, "kernel entry (before barrier init / TMEM alloc)"), (12, "prelude: own gate tiles done"), (13, "prelude: own top-k groups done (owners only)"),
         (14, "prelude: tagged ids of all tokens seen"), (4, "route_a: masks zeroed (+ forced ids loaded)"),
         (5, "route_a: membership bitmasks built"), (6, "route_a: per-expert counts and prefixes"),
         (7, "route_a: scan, work list, pass table (warp 0)"), (15, "prelude: routing tables built (route_a)")]
@@ -38,6 +38,7 @@ def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--T", type=int, default=64)
     ap.add_argument("--unions", default="16,128")
+    ap.add_argument("--steady", action="store_true", help="trace the last of 12 back-to-back steps (no sync before it)")
     ap.add_argument("--opt", action="append", default=[], help="KEY=VALUE for eldr_moe_set_option (repeatable)")
     args = ap.parse_args()
     os.environ["ELDR_EXTRA_NVCC_FLAGS"] = (os.environ.get("ELDR_EXTRA_NVCC_FLAGS", "") + " -DELDR_TRACE").strip()
@@ -65,8 +66,8 @@ def main():
             seed = 1000
         xb, bias = synth.union_case(shape, T, u, seed)
         x, bias_t = api.bf16_from_bits(xb), torch.from_numpy(bias).cuda()
-        for it in range(6):
-            if it == 5:
+        for it in range(12 if args.steady else 6):
+            if it == 5 and not args.steady:
                 torch.cuda.synchronize()
                 lib.eldr_debug_clear_trace()
             dl.w13, dl.w2 = copies[it % 4]
@@ -87,6 +88,19 @@ def main():
                 if len(v):
                     print("| %s | %d | %.2f | %.2f | %.2f |" % (name, len(v), (v.min() - t0) / 1e3,
                                                                (np.median(v) - t0) / 1e3, (v.max() - t0) / 1e3))
+        r2 = tr[1024:1024 + n_cta]
+        print("\n| per sub-phase (0..3) | min | median | max |\n|---|---|---|---|")
+        for base, name, is_time in ((0, "weights producer: sub-phase %d fully issued", True), (4, "epilogue: sub-phase %d finished", True),
+                                    (8, "activations producer: waited for h flags in sub-phase %d (us)", False),
+                                    (12, "epilogue warp 0: waited for partners' parked partials in sub-phase %d (us)", False)):
+            for sp in range(4):
+                v = r2[:, base + sp]
+                if is_time:
+                    v = v[v > 0]
+                    if len(v):
+                        print("| %s | %.2f | %.2f | %.2f |" % (name % sp, (v.min() - t0) / 1e3, (np.median(v) - t0) / 1e3, (v.max() - t0) / 1e3))
+                else:
+                    print("| %s | %.2f | %.2f | %.2f |" % (name % sp, v.min() / 1e3, np.median(v) / 1e3, v.max() / 1e3))
         stall = r0[:, 12] / 1e3
         print("\nActivations producer waited for h flags: median %.2f us, max %.2f us per CTA.\n" %
               (float(np.median(stall)), float(stall.max())), flush=True)
