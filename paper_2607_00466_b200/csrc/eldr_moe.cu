@@ -479,8 +479,9 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
     fa.partial = reinterpret_cast<float*>(ws + L.partial);
     const size_t smem_max = 227 * 1024;
     const size_t fixed = fused_smem_fixed_bytes(E, ns, T, k);
-    const size_t min_area = (size_t)3 * (kUmmaWBytes + kNPCap * 128) > (size_t)kGateTok * H * 2
-                                ? (size_t)3 * (kUmmaWBytes + kNPCap * 128) : (size_t)kGateTok * H * 2;
+    const int gate_tok = T <= 64 ? 8 : (T <= 128 ? 16 : 32);      // gate tile height: one round of tiles over the grid
+    const size_t min_area = (size_t)3 * (kUmmaWBytes + kNPCap * 128) > (size_t)gate_tok * H * 2
+                                ? (size_t)3 * (kUmmaWBytes + kNPCap * 128) : (size_t)gate_tok * H * 2;
     fa.stage_area = fixed < smem_max ? (int)((smem_max - fixed) / 1024 * 1024) : 0;
     fa.ring_bytes = g_ring_kb * 1024;
     fa.dp_min_rounds = g_dp_min_rounds;
@@ -501,12 +502,14 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
       }
       static bool fused_attr_set = false;
       if (!fused_attr_set) {
-        if (!set_smem(moe_fused_kernel, 227 * 1024)) return ELDR_ERR_CUDA;
+        if (!set_smem(moe_fused_kernel<8>, 227 * 1024) || !set_smem(moe_fused_kernel<16>, 227 * 1024) ||
+            !set_smem(moe_fused_kernel<32>, 227 * 1024)) return ELDR_ERR_CUDA;
         fused_attr_set = true;
       }
       prof_begin();
       prof_mark(0, st);
-      launch_dep(moe_fused_kernel, dim3(num_sms()), dim3(kFusedThreads), smem, st, tm_w13, tm_sw13, tm_w2, tm_sw2, tm_x, tm_h, fa);
+      auto kern = gate_tok == 8 ? moe_fused_kernel<8> : (gate_tok == 16 ? moe_fused_kernel<16> : moe_fused_kernel<32>);
+      launch_dep(kern, dim3(num_sms()), dim3(kFusedThreads), smem, st, tm_w13, tm_sw13, tm_w2, tm_sw2, tm_x, tm_h, fa);
       if (!launch_ok("moe_fused_kernel")) return ELDR_ERR_CUDA;
       prof_mark(ELDR_PROFILE_SLOTS, st);
       return ELDR_OK;

@@ -195,15 +195,21 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 // ------------------------------------------------------------------------------------ G: one logit tile
-// 8 tokens (group g) x 8 experts (tile et).  Warp w: experts 2*(w&3), 2*(w&3)+1 of the tile, tokens 4*(w>>2)..+3.
-__device__ __forceinline__ void fused_gate_tile(const FusedArgs& a, int et, int g, uint8_t* smem_raw) {
+// GT tokens (token tile g) x 8 experts (tile et).  Warp w: experts 2*(w&3), 2*(w&3)+1 of the tile, tokens
+// (GT/2)*(w>>2)..+GT/2-1.  GT = 8 for T <= 64; 16 / 32 for T <= 128 / 256 so that the whole gate stays ONE round of
+// tiles over the grid (8-token tiles took 2 / 4 rounds of ~4 us there).  GT is a template parameter of the whole
+// kernel: the wider tiles live in their own instantiations and do not perturb the code generated for T <= 64.
+template <int GT>
+__device__ __forceinline__ void fused_gate_tile(const FusedArgs& a, int et, int g, uint8_t* smem_raw, uint32_t gbar,
+                                                uint32_t gpar) {
+  constexpr int TW = GT / 2;              // tokens per warp
   const int T = a.tk.T, H = a.H, E = a.tk.E;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int t0 = g * kGateTok;
+  const int t0 = g * GT;
   const int ep = warp & 3, th = warp >> 2;
   const int e0 = et * kGateExp + 2 * ep, e1 = e0 + 1;
   const int q_per_row = H >> 2;
-  constexpr int kDepth = 8;
+  constexpr int kDepth = 8;                    // float4 per gate row requested before the x tile is staged (16: no faster, measured)
   const float4* wrow0 = reinterpret_cast<const float4*>(a.gate_w + (size_t)(e0 < E ? e0 : 0) * H);
   const float4* wrow1 = reinterpret_cast<const float4*>(a.gate_w + (size_t)(e1 < E ? e1 : 0) * H);
   const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -216,8 +222,21 @@ __device__ __forceinline__ void fused_gate_tile(const FusedArgs& a, int et, int 
   }
   uint4* xs4 = reinterpret_cast<uint4*>(smem_raw);
   const int vec_per_row = H >> 3;
-  const int n_vec = kGateTok * vec_per_row;
+  const int n_vec = GT * vec_per_row;
   __syncthreads();                       // the previous tile's readers are done with the x tile
+  if (GT > 8) {
+    // wide tiles (64 / 128 KiB of x): the tile's token rows are contiguous in x -- ONE bulk copy by the TMA engine
+    // instead of four register round trips per thread (T = 256: gate tiles done 11.5 us after the start)
+    const int rows = min(GT, T - t0);
+    if (tid == 0) {
+      const uint32_t bytes = (uint32_t)rows * (uint32_t)H * 2u;
+      mbar_arrive_expect_tx(gbar, bytes);
+      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                   :: "r"(smem_u32(smem_raw)), "l"(a.x + (size_t)t0 * H), "r"(bytes), "r"(gbar) : "memory");
+    }
+    for (int v = rows * vec_per_row + tid; v < n_vec; v += kFusedThreads) xs4[v] = make_uint4(0u, 0u, 0u, 0u);
+    mbar_wait(gbar, gpar);
+  } else
   for (int v0 = 0; v0 < n_vec; v0 += 8 * kFusedThreads) {
     uint4 val[8];
 #pragma unroll
@@ -234,10 +253,10 @@ __device__ __forceinline__ void fused_gate_tile(const FusedArgs& a, int et, int 
     }
   }
   __syncthreads();
-  float acc0[4], acc1[4];
+  float acc0[TW], acc1[TW];
 #pragma unroll
-  for (int t = 0; t < 4; ++t) { acc0[t] = 0.f; acc1[t] = 0.f; }
-  const uint2* xs2 = reinterpret_cast<const uint2*>(smem_raw) + (size_t)(4 * th) * q_per_row;
+  for (int t = 0; t < TW; ++t) { acc0[t] = 0.f; acc1[t] = 0.f; }
+  const uint2* xs2 = reinterpret_cast<const uint2*>(smem_raw) + (size_t)(TW * th) * q_per_row;
   for (int base = 0; base < q_per_row; base += 32 * kDepth) {
     if (base > 0) {
 #pragma unroll
@@ -252,7 +271,7 @@ __device__ __forceinline__ void fused_gate_tile(const FusedArgs& a, int et, int 
       const int c4 = base + lane + 32 * u;
       if (c4 < q_per_row) {
 #pragma unroll
-        for (int t = 0; t < 4; ++t) {
+        for (int t = 0; t < TW; ++t) {
           const uint2 xv = xs2[t * q_per_row + c4];
           const float x0 = bf16_lo(xv.x), x1 = bf16_hi(xv.x), x2 = bf16_lo(xv.y), x3 = bf16_hi(xv.y);
           float s0 = acc0[t], s1 = acc1[t];
@@ -266,7 +285,7 @@ __device__ __forceinline__ void fused_gate_tile(const FusedArgs& a, int et, int 
     }
   }
 #pragma unroll
-  for (int t = 0; t < 4; ++t) {
+  for (int t = 0; t < TW; ++t) {
     float s0 = acc0[t], s1 = acc1[t];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
@@ -280,8 +299,8 @@ __device__ __forceinline__ void fused_gate_tile(const FusedArgs& a, int et, int 
     const float b0 = (a.gate_bias && e0 < E) ? a.gate_bias[e0] : 0.f;
     const float b1 = (a.gate_bias && e1 < E) ? a.gate_bias[e1] : 0.f;
 #pragma unroll
-    for (int t = 0; t < 4; ++t) {
-      const int tt = t0 + 4 * th + t;
+    for (int t = 0; t < TW; ++t) {
+      const int tt = t0 + TW * th + t;
       if (tt < T) {
         if (e0 < E) z[(size_t)tt * E + e0] = acc0[t] + b0;
         if (e1 < E) z[(size_t)tt * E + e1] = acc1[t] + b1;
@@ -616,7 +635,113 @@ struct PieceWalker {
   }
 };
 
+// ------------------------------------------------------------------------------ C: flag-driven combine
+template <int KMAX>
+__device__ __forceinline__ void fused_combine(const FusedArgs& a, const FusedSmem& sm, const uint32_t* ydone, uint32_t epoch,
+                                              int n_work, int tilesB, int cta, int G, int warp, int lane) {
+  const int T = a.tk.T, E = a.tk.E, k = a.tk.k, H = a.H, ns = a.n_shared;
+  {
+    const int32_t* s_ent = reinterpret_cast<const int32_t*>(sm.route_scratch + (size_t)E * ((T + 31) >> 5) * 8);
+    const int q_per_row = H >> 2;
+    const int n_units = T * tilesB;
+    const int n_act_ = n_work - ns;
+    // Two units per iteration: both units' flag polls, then both units' k row loads, are in flight together (one
+    // unit at a time cost a poll + fence + load round trip each: 13 us of combine at T = 256).
+    const int u_step = G * (kFusedThreads / 32);
+    for (int u0 = cta * (kFusedThreads / 32) + warp; u0 < n_units; u0 += 2 * u_step) {
+      int t_[2], rt_[2], pos_[2], fl_[2];
+      float wt_[2];
+      const unsigned long long* wsrc_[2];
+      bool have_[2];
+#pragma unroll
+      for (int q = 0; q < 2; ++q) {
+        const int u = u0 + q * u_step;
+        have_[q] = u < n_units;
+        const int uu = have_[q] ? u : u0;
+        const int t = uu / tilesB, rt = uu - t * tilesB;
+        t_[q] = t; rt_[q] = rt; pos_[q] = 0; fl_[q] = -1; wt_[q] = 0.f; wsrc_[q] = nullptr;
+        if (have_[q]) {
+          if (lane < k) {
+            const int ent = s_ent[sm.ids8[t * k + lane]];
+            pos_[q] = sm.pos_of_pair[t * k + lane];
+            fl_[q] = (sm.cumpass[ent] + (pos_[q] - sm.work[ent].y) / kNPCap) * tilesB + rt;
+            if (a.force_routing) wt_[q] = __ldcg(a.tk.w + t * k + lane);
+            else wsrc_[q] = a.wtag + (size_t)t * kMaxTopK + lane;
+          } else if (lane < k + ns) {
+            const int ent = n_act_ + (lane - k);
+            pos_[q] = T * k + (lane - k) * T + t;
+            fl_[q] = (sm.cumpass[ent] + t / kNPCap) * tilesB + rt;
+            wt_[q] = 1.0f;
+          }
+        }
+      }
+      bool f_ok[2] = {fl_[0] < 0, fl_[1] < 0}, w_ok[2] = {wsrc_[0] == nullptr, wsrc_[1] == nullptr};
+      for (uint32_t spins = 0;; ++spins) {
+        uint32_t fv[2] = {0u, 0u};
+        unsigned long long wv[2] = {0ull, 0ull};
+#pragma unroll
+        for (int q = 0; q < 2; ++q) {
+          if (!f_ok[q]) fv[q] = flag_relaxed(ydone + fl_[q]);
+          if (!w_ok[q]) wv[q] = ld_relaxed_u64(wsrc_[q]);       // written by the top-k owner in the prelude: up on the first look
+        }
+#pragma unroll
+        for (int q = 0; q < 2; ++q) {
+          if (!f_ok[q]) f_ok[q] = fv[q] == epoch;
+          if (!w_ok[q] && (uint32_t)(wv[q] >> 32) == epoch) { w_ok[q] = true; wt_[q] = __uint_as_float((uint32_t)wv[q]); }
+        }
+        if (__all_sync(0xffffffffu, f_ok[0] && f_ok[1] && w_ok[0] && w_ok[1])) break;
+        __nanosleep(250);
+        if (spins > (1u << 22)) __trap();
+      }
+      fence_acq_rel_gpu();
+      __syncwarp();
+      float4 v[2][KMAX];
+      float wj[2][KMAX];
+      bool in_[2];
+#pragma unroll
+      for (int q = 0; q < 2; ++q) {
+        const int c4 = rt_[q] * 32 + lane;
+        in_[q] = have_[q] && c4 < q_per_row;
+#pragma unroll
+        for (int j = 0; j < KMAX; ++j)
+          if (j < k) {
+            const int pj = __shfl_sync(0xffffffffu, pos_[q], j);
+            wj[q][j] = __shfl_sync(0xffffffffu, wt_[q], j);
+            if (in_[q]) v[q][j] = __ldcg(reinterpret_cast<const float4*>(a.ybuf + (size_t)pj * H + (size_t)c4 * 4));
+          }
+      }
+#pragma unroll
+      for (int q = 0; q < 2; ++q) {
+        const int c4 = rt_[q] * 32 + lane;
+        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (in_[q]) {
+#pragma unroll
+          for (int j = 0; j < KMAX; ++j)
+            if (j < k) {
+              acc.x = fmaf(wj[q][j], v[q][j].x, acc.x); acc.y = fmaf(wj[q][j], v[q][j].y, acc.y);
+              acc.z = fmaf(wj[q][j], v[q][j].z, acc.z); acc.w = fmaf(wj[q][j], v[q][j].w, acc.w);
+            }
+        }
+        for (int s_ = 0; s_ < ns; ++s_) {
+          const int ps = __shfl_sync(0xffffffffu, pos_[q], k + s_);
+          if (in_[q]) {
+            const float4 sv = __ldcg(reinterpret_cast<const float4*>(a.ybuf + (size_t)ps * H + (size_t)c4 * 4));
+            acc.x += sv.x; acc.y += sv.y; acc.z += sv.z; acc.w += sv.w;
+          }
+        }
+        if (in_[q]) {
+          uint2 o;
+          o.x = (uint32_t)f32_to_bf16_rn(acc.x) | ((uint32_t)f32_to_bf16_rn(acc.y) << 16);
+          o.y = (uint32_t)f32_to_bf16_rn(acc.z) | ((uint32_t)f32_to_bf16_rn(acc.w) << 16);
+          *reinterpret_cast<uint2*>(a.out + (size_t)t_[q] * H + (size_t)c4 * 4) = o;
+        }
+      }
+    }
+  }
+}
+
 // ------------------------------------------------------------------------------------------- the kernel
+template <int GT>
 __global__ void __launch_bounds__(kFusedThreads, 1)
 moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_constant__ CUtensorMap tm_sw13,
                  const __grid_constant__ CUtensorMap tm_w2, const __grid_constant__ CUtensorMap tm_sw2,
@@ -668,6 +793,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     for (int s = 0; s < kMaxStages; ++s) { mbar_init(full_bar(s), 2); mbar_init(empty_bar(s), 1); }
     for (int b = 0; b < 2; ++b) { mbar_init(tfull_bar(b), 1); mbar_init(tempty_bar(b), 4); }
     for (int b = 0; b < kClaimSlots; ++b) { mbar_init(cfull_bar(b), 1); mbar_init(cempty_bar(b), 7); }
+    mbar_init(sm.bar_base + 400u, 1);                 // x tile of the wide gate tiles (bulk copy)
     mbar_fence_init();
     tma_prefetch_desc(&tm_w13);
     tma_prefetch_desc(&tm_w2);
@@ -709,10 +835,11 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
   // ------------------------------------------------------------------------------ G + K: gate and top-k
   if (!a.force_routing) {
     const int n_et = (E + kGateExp - 1) / kGateExp, n_gr = (T + kGateTok - 1) / kGateTok;
-    const int n_tiles = n_et * n_gr;
-    for (int tile = cta; tile < n_tiles; tile += G) {
+    const int n_tiles = n_et * ((T + GT - 1) / GT);
+    uint32_t gpar = 0;
+    for (int tile = cta; tile < n_tiles; tile += G, gpar ^= 1u) {
       const int g = tile / n_et, et = tile - g * n_et;
-      fused_gate_tile(a, et, g, scratch);
+      fused_gate_tile<GT>(a, et, g, scratch, sm.bar_base + 400u, gpar);
       __syncthreads();
       if (tid == 0) flag_release(a.sync + kSyncTile + g * 32 + et, epoch);    // cumulative over the barrier
     }
@@ -720,7 +847,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     // owner of token group g: waits for the group's logit tiles, warp w runs the top-k of token 8g + w and writes the
     // ABI outputs, the signature increments and the tagged ids words every CTA routes from
     for (int g = ((cta - n_tiles % G) + G) % G; g < n_gr; g += G) {     // owner(g) = (n_tiles + g) % G: CTAs without a gate tile first
-      if (warp == 0) warp_wait_flags(a.sync + kSyncTile + g * 32, n_et, epoch, lane);
+      if (warp == 0) warp_wait_flags(a.sync + kSyncTile + (g * kGateTok / GT) * 32, n_et, epoch, lane);
       __syncthreads();
       const int t = g * kGateTok + warp;
       if (t < T) {
@@ -1204,77 +1331,8 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
 #else
   if (tid == 0) FSTAMP(8);
   __syncthreads();
-  {
-    const int32_t* s_ent = reinterpret_cast<const int32_t*>(sm.route_scratch + (size_t)E * ((T + 31) >> 5) * 8);
-    const int q_per_row = H >> 2;
-    const int n_units = T * tilesB;
-    const int n_act_ = n_work - ns;
-    for (int u = cta * (kFusedThreads / 32) + warp; u < n_units; u += G * (kFusedThreads / 32)) {
-      const int t = u / tilesB, rt = u - t * tilesB;
-      int pos = 0, fl = -1;
-      float wt = 0.f;
-      const unsigned long long* wsrc = nullptr;
-      if (lane < k) {
-        const int ent = s_ent[sm.ids8[t * k + lane]];
-        pos = sm.pos_of_pair[t * k + lane];
-        fl = (sm.cumpass[ent] + (pos - sm.work[ent].y) / kNPCap) * tilesB + rt;
-        if (a.force_routing) wt = __ldcg(a.tk.w + t * k + lane);
-        else wsrc = a.wtag + (size_t)t * kMaxTopK + lane;
-      } else if (lane < k + ns) {
-        const int ent = n_act_ + (lane - k);
-        pos = T * k + (lane - k) * T + t;
-        fl = (sm.cumpass[ent] + t / kNPCap) * tilesB + rt;
-        wt = 1.0f;
-      }
-      bool w_ok = wsrc == nullptr;
-      for (uint32_t spins = 0;; ++spins) {
-        const bool ok = fl < 0 || flag_relaxed(ydone + fl) == epoch;
-        if (!w_ok) {                                  // written by the top-k owner in the prelude: up on the first look
-          const unsigned long long wv = ld_relaxed_u64(wsrc);
-          w_ok = (uint32_t)(wv >> 32) == epoch;
-          wt = __uint_as_float((uint32_t)wv);
-        }
-        if (__all_sync(0xffffffffu, ok && w_ok)) break;
-        __nanosleep(250);
-        if (spins > (1u << 22)) __trap();
-      }
-      fence_acq_rel_gpu();
-      __syncwarp();
-      const int c4 = rt * 32 + lane;
-      const bool in = c4 < q_per_row;
-      float4 v[kMaxTopK];
-      float wj[kMaxTopK];
-#pragma unroll
-      for (int j = 0; j < kMaxTopK; ++j)
-        if (j < k) {
-          const int pj = __shfl_sync(0xffffffffu, pos, j);
-          wj[j] = __shfl_sync(0xffffffffu, wt, j);
-          if (in) v[j] = __ldcg(reinterpret_cast<const float4*>(a.ybuf + (size_t)pj * H + (size_t)c4 * 4));
-        }
-      float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (in) {
-#pragma unroll
-        for (int j = 0; j < kMaxTopK; ++j)
-          if (j < k) {
-            acc.x = fmaf(wj[j], v[j].x, acc.x); acc.y = fmaf(wj[j], v[j].y, acc.y);
-            acc.z = fmaf(wj[j], v[j].z, acc.z); acc.w = fmaf(wj[j], v[j].w, acc.w);
-          }
-      }
-      for (int s_ = 0; s_ < ns; ++s_) {
-        const int ps = __shfl_sync(0xffffffffu, pos, k + s_);
-        if (in) {
-          const float4 sv = __ldcg(reinterpret_cast<const float4*>(a.ybuf + (size_t)ps * H + (size_t)c4 * 4));
-          acc.x += sv.x; acc.y += sv.y; acc.z += sv.z; acc.w += sv.w;
-        }
-      }
-      if (in) {
-        uint2 o;
-        o.x = (uint32_t)f32_to_bf16_rn(acc.x) | ((uint32_t)f32_to_bf16_rn(acc.y) << 16);
-        o.y = (uint32_t)f32_to_bf16_rn(acc.z) | ((uint32_t)f32_to_bf16_rn(acc.w) << 16);
-        *reinterpret_cast<uint2*>(a.out + (size_t)t * H + (size_t)c4 * 4) = o;
-      }
-    }
-  }
+  if (k <= 8) fused_combine<8>(a, sm, ydone, epoch, n_work, tilesB, cta, G, warp, lane);
+  else fused_combine<kMaxTopK>(a, sm, ydone, epoch, n_work, tilesB, cta, G, warp, lane);
   if (tid == 0) FSTAMP(10);
 
   tc_fence_before();

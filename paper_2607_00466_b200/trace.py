@@ -101,6 +101,10 @@ def main():
                         print("| %s | %.2f | %.2f | %.2f |" % (name % sp, (v.min() - t0) / 1e3, (np.median(v) - t0) / 1e3, (v.max() - t0) / 1e3))
                 else:
                     print("| %s | %.2f | %.2f | %.2f |" % (name % sp, v.min() / 1e3, np.median(v) / 1e3, v.max() / 1e3))
+        for col, name in ((0, "weights producer: waited for free ring slots, phase A (us @1.965 GHz)"), (1, "weights producer: waited for free ring slots, phase B (us @1.965 GHz)"),
+                          (10, "weights producer: TMA issue, phase A (us @1.965 GHz)"), (11, "weights producer: TMA issue, phase B (us @1.965 GHz)")):
+            v = r1[:, col] / 1965.0
+            print("| %s | %.2f | %.2f | %.2f |" % (name, v.min(), np.median(v), v.max()))
         stall = r0[:, 12] / 1e3
         print("\nActivations producer waited for h flags: median %.2f us, max %.2f us per CTA.\n" %
               (float(np.median(stall)), float(stall.max())), flush=True)
