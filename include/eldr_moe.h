@@ -74,11 +74,11 @@ typedef struct {
   size_t pair_pos;   /* int32   [T*k]            inverse of perm                                         */
   size_t work;       /* int32x4 [E+n_shared]     {expert, x_row0, out_row0, m} per streamed expert       */
   size_t n_work;     /* int32   [1]              n_active + n_shared                                     */
-  size_t sync;       /* uint32  [...]            epoch flags + generation word (internal); offset 0, size independent of T */
+  size_t sync;       /* uint32  [...]            epoch flags + generation words (internal); offset 0                       */
   size_t x_perm;     /* bf16    [T*k + T, H]     x gathered in sorted order, then a plain copy of x      */
   size_t h;          /* bf16    [T*(k+ns), I]    silu(W1 x)*(W3 x) per sorted pair, then shared experts  */
   size_t y;          /* float   [T*(k+ns), H]    W2 h per sorted pair, then shared experts               */
-  size_t partial;    /* float   [2][256][128][128] parked fp32 accumulators of tiles split between two SMs (internal) */
+  size_t partial;    /* float   [4][256][128][128] parked fp32 accumulators of tiles split between SMs (internal; 64 MiB for T <= 256, unused above) */
   size_t total;      /* bytes needed                                                                    */
 } eldr_moe_ws_layout_t;
 
@@ -192,6 +192,11 @@ int32_t eldr_moe_workspace_layout(const eldr_moe_shape_t* shape, int32_t T, eldr
                                  value = percentage of the experts in g0 (0 or 100: one group).  0..100; default 0: measured on
                                  B200 the two-group order is SLOWER (|U| = 16: 76 vs 60 us) -- each group's share per SM is
                                  shorter than one weight tile, so every tile is cut three ways and the fix-ups have no slack */
+#define ELDR_OPT_COOPERATIVE 7 /* fused step: 1 (default) = cooperative launch: the persistent grid, whose CTAs wait on one another,
+                                 starts only when ALL of its CTAs can be resident (safe next to kernels of other streams, MPS or
+                                 green-context SM partitions; a grid that cannot fit returns to the staged path).  Measured on
+                                 B200 the driver does not overlap a cooperative launch with its predecessor (PDL has no effect):
+                                 +2.5 us per step.  0 = plain launch + PDL, for a GPU the process has to itself */
 #define ELDR_OPT_FFN_PAIR 5   /* prefill-shaped calls (T > 1024, I % 128 == 0, H % 256 == 0): the expert FFN as tcgen05
                                  cta_group::2 tiles (M = 256 over an SM pair, ffn_umma2.cuh).  1 (default): when the call
                                  has >= 256 tokens per expert on average (T*k >= 256*E); 2: always; 0: never (one CTA

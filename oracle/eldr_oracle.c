@@ -272,6 +272,9 @@ int oracle_permutation(const oracle_shape_t *s, int32_t T, const int32_t *ids, i
  * signature row"; "one int8 per (block, MoE layer, expert)".
  * sig_req [R,L,E] int32, sig_block [NB,L,E] int8.  token_req/token_block < 0 => token not recorded
  * (padding; reading R9).  Either table or map may be NULL.  Serial loop in token order.
+ * An int8 cell holds at most 127: under PAPER.md:255's layout a cell counts the tokens of ONE KV block that picked
+ * the expert (<= block size <= 127), so the bound is never reached by a conforming caller; past it the cell stays at
+ * 127 (reading "int8 cells saturate") instead of wrapping to -128.
  * ---------------------------------------------------------------------------------------------- */
 int oracle_signature_accumulate(const oracle_shape_t *s, int32_t layer, int32_t T,
                                 const int32_t *ids, const int32_t *token_req,
@@ -284,8 +287,10 @@ int oracle_signature_accumulate(const oracle_shape_t *s, int32_t layer, int32_t 
       if (e < 0 || e >= E) return -1;
       if (sig_req && token_req && token_req[t] >= 0)
         sig_req[((size_t)token_req[t] * L + layer) * E + e] += 1;
-      if (sig_block && token_block && token_block[t] >= 0)
-        sig_block[((size_t)token_block[t] * L + layer) * E + e] += 1;
+      if (sig_block && token_block && token_block[t] >= 0) {
+        int8_t *cell = &sig_block[((size_t)token_block[t] * L + layer) * E + e];
+        if (*cell < 127) *cell += 1;
+      }
     }
   }
   return 0;

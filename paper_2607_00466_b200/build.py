@@ -10,14 +10,19 @@ _ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(CSRC, "libeldr_moe.so")
 SOURCES = ["eldr_moe.cu"]
-HEADERS = ["device_utils.cuh", "gate_route.cuh", "ffn_stream.cuh", "ffn_umma.cuh", "moe_fused.cuh", "route_decide.cuh", "gate_prefill.cuh", "route_prefill.cuh"]
+
+
+def _headers():
+    """Every header the translation unit can include: a change to any of them rebuilds the library."""
+    import glob
+    return sorted(glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(CSRC, "*.h")))
 
 
 def _stale() -> bool:
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS] + [os.path.join(_ROOT, "include", "eldr_moe.h")]
+    deps = [os.path.join(CSRC, f) for f in SOURCES] + _headers() + [os.path.join(_ROOT, "include", "eldr_moe.h")]
     return any(os.path.getmtime(d) > t for d in deps)
 
 

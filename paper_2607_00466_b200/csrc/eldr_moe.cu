@@ -23,13 +23,16 @@ namespace {
 
 using namespace eldr;
 
-int g_ffn_pair = 1;               // prefill-shaped calls: cta_group::2 FFN tiles over SM pairs (ELDR_OPT_FFN_PAIR)
-int g_ffn_path = ELDR_FFN_TCGEN05;   // process-wide tuning knobs (eldr_moe_set_option)
-int g_pdl = 1;
-int g_step_path = ELDR_STEP_AUTO;
-int g_ring_kb = 208;
-int g_dp_min_rounds = 4;
-int g_sk_split_pct = 0;
+// Process-wide tuning knobs (eldr_moe_set_option).  Relaxed atomics: a call reads each knob once, so a concurrent
+// set_option from another host thread changes whole calls, never half of one.
+std::atomic<int> g_ffn_pair{1};   // prefill-shaped calls: cta_group::2 FFN tiles over SM pairs (ELDR_OPT_FFN_PAIR)
+std::atomic<int> g_ffn_path{ELDR_FFN_TCGEN05};
+std::atomic<int> g_pdl{1};
+std::atomic<int> g_step_path{ELDR_STEP_AUTO};
+std::atomic<int> g_ring_kb{208};
+std::atomic<int> g_dp_min_rounds{4};
+std::atomic<int> g_sk_split_pct{0};
+std::atomic<int> g_coop{1};
 
 thread_local char g_err[256] = "";
 thread_local int g_launches = 0;
@@ -114,7 +117,7 @@ void make_layout(const eldr_moe_shape_t* s, int T, eldr_moe_ws_layout_t* L) {
   L->x_perm = take((Tz * k + Tz) * H * 2);
   L->h = take(Tz * (k + ns) * I * 2);
   L->y = take(Tz * (k + ns) * H * 4);
-  L->partial = take(fused_partial_bytes(256));   // stream-K fix-up slots of the fused kernel (grid <= 256 CTAs)
+  L->partial = take(T <= kFusedMaxT ? fused_partial_bytes(256) : 256);   // stream-K fix-up slots of the fused kernel (grid <= 256 CTAs); unused above its T limit
   L->total = o;
 }
 
@@ -129,15 +132,43 @@ void make_host_stage(const eldr_moe_shape_t* s, int T, size_t base, HostStage* S
   S->total = o;
 }
 
+// Per-DEVICE state: cudaFuncSetAttribute is a per-device setting and the SM count / co-residency of the persistent
+// grid are properties of the device the call runs on, so everything cached here is keyed by the device ordinal.
+constexpr int kMaxDevices = 64;
+enum { kAttrFused = 0, kAttrRouteBig, kAttrUmma, kAttrPair, kAttrStream, kAttrRouteSims, kAttrGateLogits, kAttrGateRoute,
+       kAttrRouteOnly, kAttrCount };
+struct DevState {
+  std::atomic<int> sms{0};
+  std::atomic<int> fused_ok{-1};          // -1 unknown, 0 the persistent grid cannot be co-resident, 1 it can
+  std::atomic<int> coop_pdl_ok{-1};       // -1 unknown, 1 cooperative + programmatic launch compose on this driver, 0 they do not
+  std::atomic<bool> attr[kAttrCount];
+  DevState() { for (auto& a : attr) a.store(false); }
+};
+DevState g_dev[kMaxDevices];
+
+int current_device() {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) dev = 0;
+  return dev;
+}
 int num_sms() {
-  static int n = 0;
+  DevState& d = g_dev[current_device()];
+  int n = d.sms.load(std::memory_order_relaxed);
   if (n == 0) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
+    cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, current_device());
     if (n <= 0) n = 148;
+    d.sms.store(n, std::memory_order_relaxed);
   }
   return n;
+}
+// cudaFuncAttributeMaxDynamicSharedMemorySize, once per (device, kernel family)
+template <typename F>
+bool once_per_device(int which, F&& set) {
+  DevState& d = g_dev[current_device()];
+  if (d.attr[which].load(std::memory_order_acquire)) return true;
+  if (!set()) return false;
+  d.attr[which].store(true, std::memory_order_release);
+  return true;
 }
 
 // ---------------------------------------------------------------------------- TMA descriptors
@@ -162,34 +193,53 @@ encode_tiled_fn get_encode_fn() {
 // bf16 [rows, cols] row-major, box = box_rows x 64 columns (128 bytes), SWIZZLE_128B, OOB reads give zeros.
 // Descriptors are pure functions of (ptr, rows, cols, box_rows); a small cache avoids re-encoding the
 // static weight descriptors every step.
-struct TmapKey { const void* p; uint64_t rows, cols; uint32_t box_rows, kind; };
-struct TmapSlot { TmapKey k; CUtensorMap m; bool used; };
+// The cache is a 4-way set-associative table of 1024 slots hashed on (device, pointer, shape): a 48-layer stack holds
+// 96 weight descriptors plus the activations' (the 64-slot round-robin list of round 1 cycled and missed on every
+// lookup there).  Within a set the oldest entry is replaced.
+struct TmapKey { const void* p; uint64_t rows, cols; uint32_t box_rows, kind; int dev; };
+struct TmapSlot { TmapKey k; CUtensorMap m; uint64_t stamp; bool used; };
+constexpr int kTmSets = 256, kTmWays = 4;
 std::mutex g_tm_mu;
-TmapSlot g_tm_cache[64];
-int g_tm_next = 0;
+TmapSlot g_tm_cache[kTmSets * kTmWays];
+uint64_t g_tm_clock = 0;
 
+inline bool tm_same(const TmapKey& a, const TmapKey& b) {
+  return a.p == b.p && a.rows == b.rows && a.cols == b.cols && a.box_rows == b.box_rows && a.kind == b.kind && a.dev == b.dev;
+}
+inline int tm_set(const TmapKey& k) {
+  uint64_t h = reinterpret_cast<uintptr_t>(k.p) * 0x9E3779B97F4A7C15ull;
+  h ^= (k.rows * 0xC2B2AE3D27D4EB4Full) ^ (k.cols << 17) ^ ((uint64_t)k.box_rows << 7) ^ ((uint64_t)k.kind << 3) ^ (uint64_t)k.dev;
+  h ^= h >> 29;
+  return (int)(h % kTmSets);
+}
 bool tmap_lookup(const TmapKey& k, CUtensorMap* out) {
   std::lock_guard<std::mutex> lk(g_tm_mu);
-  for (auto& s : g_tm_cache)
-    if (s.used && s.k.p == k.p && s.k.rows == k.rows && s.k.cols == k.cols && s.k.box_rows == k.box_rows &&
-        s.k.kind == k.kind) {
-      *out = s.m;
+  TmapSlot* set = g_tm_cache + tm_set(k) * kTmWays;
+  for (int w = 0; w < kTmWays; ++w)
+    if (set[w].used && tm_same(set[w].k, k)) {
+      set[w].stamp = ++g_tm_clock;
+      *out = set[w].m;
       return true;
     }
   return false;
 }
 void tmap_store(const TmapKey& k, const CUtensorMap& m) {
   std::lock_guard<std::mutex> lk(g_tm_mu);
-  TmapSlot& s = g_tm_cache[g_tm_next];
-  g_tm_next = (g_tm_next + 1) % 64;
-  s.k = k;
-  s.m = m;
-  s.used = true;
+  TmapSlot* set = g_tm_cache + tm_set(k) * kTmWays;
+  int victim = 0;
+  for (int w = 0; w < kTmWays; ++w) {
+    if (!set[w].used) { victim = w; break; }
+    if (set[w].stamp < set[victim].stamp) victim = w;
+  }
+  set[victim].k = k;
+  set[victim].m = m;
+  set[victim].stamp = ++g_tm_clock;
+  set[victim].used = true;
 }
 
 // bf16 [rows, cols] row-major, box = box_rows x 64 columns (128 bytes), SWIZZLE_128B, OOB reads give zeros.
 bool make_tmap(CUtensorMap* out, const void* ptr, uint64_t rows, uint64_t cols, uint32_t box_rows) {
-  const TmapKey key{ptr, rows, cols, box_rows, 2};
+  const TmapKey key{ptr, rows, cols, box_rows, 2, current_device()};
   if (tmap_lookup(key, out)) return true;
   encode_tiled_fn fn = get_encode_fn();
   if (!fn) { snprintf(g_err, sizeof(g_err), "cuTensorMapEncodeTiled entry point not found"); return false; }
@@ -208,7 +258,7 @@ bool make_tmap(CUtensorMap* out, const void* ptr, uint64_t rows, uint64_t cols, 
 // w13 [n_exp, 2I, H] viewed as 5-D (col, row-in-16, branch{w1,w3}, 16-row group, expert) so that ONE box of
 // (64 cols, 16 rows, 2 branches, 4 groups) lands in shared memory as 4 x [16 rows of w1 | same 16 rows of w3].
 bool make_tmap_w13_5d(CUtensorMap* out, const void* ptr, uint64_t n_exp, uint64_t I, uint64_t H) {
-  const TmapKey key{ptr, n_exp * 2 * I, H, 16, 5};
+  const TmapKey key{ptr, n_exp * 2 * I, H, 16, 5, current_device()};
   if (tmap_lookup(key, out)) return true;
   encode_tiled_fn fn = get_encode_fn();
   if (!fn) { snprintf(g_err, sizeof(g_err), "cuTensorMapEncodeTiled entry point not found"); return false; }
@@ -238,7 +288,7 @@ cudaError_t launch_dep(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
-  cfg.numAttrs = (g_pdl && !g_prof_on) ? 1 : 0;
+  cfg.numAttrs = (g_pdl.load() && !g_prof_on) ? 1 : 0;
   return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
 }
 
@@ -258,7 +308,45 @@ cudaError_t launch_dep_pair(void (*kernel)(KArgs...), dim3 grid, dim3 block, siz
   attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[1].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
-  cfg.numAttrs = (g_pdl && !g_prof_on) ? 2 : 1;
+  cfg.numAttrs = (g_pdl.load() && !g_prof_on) ? 2 : 1;
+  return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
+// The fused step: cooperative launch (all CTAs co-resident or the launch fails) plus, when allowed, the
+// programmatic-dependent-launch attribute.  Whether the two attributes compose is found out once per device: if the
+// first launch with both is rejected as an invalid configuration, the kernel is launched cooperatively without PDL
+// from then on.
+template <typename... KArgs, typename... Args>
+cudaError_t launch_fused(void (*kernel)(KArgs...), DevState& dv, dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[2];
+  attr[0].id = cudaLaunchAttributeCooperative;
+  attr[0].val.cooperative = 1;
+  attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[1].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  const bool want_pdl = g_pdl.load() && !g_prof_on;
+  if (!g_coop.load()) {
+    // ELDR_OPT_COOPERATIVE = 0: plain launch (+ PDL).  For a GPU this process has to itself: nothing else can hold an
+    // SM, the occupancy check above has shown that the grid fits, and consecutive steps overlap their launch latency.
+    cfg.attrs = attr + 1;
+    cfg.numAttrs = want_pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+  }
+  int both = dv.coop_pdl_ok.load(std::memory_order_relaxed);
+  if (want_pdl && both != 0) {
+    cfg.numAttrs = 2;
+    const cudaError_t e = cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+    if (e == cudaSuccess || both == 1) { dv.coop_pdl_ok.store(1, std::memory_order_relaxed); return e; }
+    if (e != cudaErrorInvalidValue && e != cudaErrorNotSupported && e != cudaErrorInvalidConfiguration) return e;
+    cudaGetLastError();
+    dv.coop_pdl_ok.store(0, std::memory_order_relaxed);
+  }
+  cfg.numAttrs = 1;
   return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
 }
 
@@ -272,7 +360,7 @@ int32_t launch_gate_logits(const eldr_moe_shape_t* s, int T, const eldr_bf16* x,
                            const float* gate_bias, float* z, cudaStream_t st) {
   const size_t smem = (size_t)kGateTok * s->hidden * 2;
   if (smem > 200 * 1024) return ELDR_ERR_UNSUPPORTED;
-  if (smem > 48 * 1024 && !set_smem(gate_logits_kernel, smem)) return ELDR_ERR_CUDA;
+  if (smem > 48 * 1024 && !once_per_device(kAttrGateLogits, [] { return set_smem(gate_logits_kernel, 200 * 1024); })) return ELDR_ERR_CUDA;
   dim3 grid((s->n_experts + kGateExp - 1) / kGateExp, (T + kGateTok - 1) / kGateTok);
   gate_logits_kernel<<<grid, 256, smem, st>>>(x, gate_w, gate_bias, z, T, s->hidden, s->n_experts);
   return launch_ok("gate_logits_kernel") ? ELDR_OK : ELDR_ERR_CUDA;
@@ -350,6 +438,10 @@ int32_t eldr_moe_set_option(int32_t key, int32_t value) {
   }
   if (key == ELDR_OPT_DP_MIN_ROUNDS && value >= 1 && value <= (1 << 20)) {
     g_dp_min_rounds = value;
+    return ELDR_OK;
+  }
+  if (key == ELDR_OPT_COOPERATIVE && (value == 0 || value == 1)) {
+    g_coop = value;
     return ELDR_OK;
   }
   if (key == ELDR_OPT_SK_SPLIT_PCT && value >= 0 && value <= 100) {
@@ -459,8 +551,10 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
   // ------------------------------------------------------------------ whole step in one persistent launch
   // AUTO: shared experts receive every token, so from ~224 tokens their activation tiles are as wide as the weight
   // tiles and the staged path (rows gathered once, plain TMA boxes) is faster: config-5 shape at T = 256 280 -> 257 us
-  const bool want_fused = g_step_path == ELDR_STEP_FUSED || (g_step_path == ELDR_STEP_AUTO && !(ns > 0 && T >= 224));
-  if (want_fused && g_ffn_path == ELDR_FFN_TCGEN05 && H % 64 == 0 && I % 64 == 0 &&
+  const int step_path = g_step_path.load();
+  const bool want_fused = step_path == ELDR_STEP_FUSED || (step_path == ELDR_STEP_AUTO && !(ns > 0 && T >= 224));
+  const int ffn_path = g_ffn_path.load();
+  if (want_fused && ffn_path == ELDR_FFN_TCGEN05 && H % 64 == 0 && I % 64 == 0 &&
       T <= kFusedMaxT && num_sms() <= 256) {
     FusedArgs fa;
     fa.x = x; fa.gate_w = gate_w; fa.gate_bias = gate_bias;
@@ -483,9 +577,9 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
     const size_t min_area = (size_t)3 * (kUmmaWBytes + kNPCap * 128) > (size_t)gate_tok * H * 2
                                 ? (size_t)3 * (kUmmaWBytes + kNPCap * 128) : (size_t)gate_tok * H * 2;
     fa.stage_area = fixed < smem_max ? (int)((smem_max - fixed) / 1024 * 1024) : 0;
-    fa.ring_bytes = g_ring_kb * 1024;
-    fa.dp_min_rounds = g_dp_min_rounds;
-    fa.sk_split_pct = g_sk_split_pct;
+    fa.ring_bytes = g_ring_kb.load() * 1024;
+    fa.dp_min_rounds = g_dp_min_rounds.load();
+    fa.sk_split_pct = g_sk_split_pct.load();
     const size_t smem = fixed + fa.stage_area;
     if ((size_t)fa.stage_area >= min_area) {
       CUtensorMap tm_w13, tm_sw13, tm_w2, tm_sw2, tm_x, tm_h;
@@ -500,19 +594,46 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
         tm_sw13 = tm_w13;
         tm_sw2 = tm_w2;
       }
-      static bool fused_attr_set = false;
-      if (!fused_attr_set) {
-        if (!set_smem(moe_fused_kernel<8>, 227 * 1024) || !set_smem(moe_fused_kernel<16>, 227 * 1024) ||
-            !set_smem(moe_fused_kernel<32>, 227 * 1024)) return ELDR_ERR_CUDA;
-        fused_attr_set = true;
-      }
-      prof_begin();
-      prof_mark(0, st);
+      if (!once_per_device(kAttrFused, [] {
+            return set_smem(moe_fused_kernel<8>, 227 * 1024) && set_smem(moe_fused_kernel<16>, 227 * 1024) &&
+                   set_smem(moe_fused_kernel<32>, 227 * 1024);
+          })) return ELDR_ERR_CUDA;
       auto kern = gate_tok == 8 ? moe_fused_kernel<8> : (gate_tok == 16 ? moe_fused_kernel<16> : moe_fused_kernel<32>);
-      launch_dep(kern, dim3(num_sms()), dim3(kFusedThreads), smem, st, tm_w13, tm_sw13, tm_w2, tm_sw2, tm_x, tm_h, fa);
-      if (!launch_ok("moe_fused_kernel")) return ELDR_ERR_CUDA;
-      prof_mark(ELDR_PROFILE_SLOTS, st);
-      return ELDR_OK;
+      // The persistent grid's CTAs wait on one another (tile flags, tagged ids, h / y flags): they must all be
+      // resident.  (1) Once per device: the occupancy calculator must grant one CTA of this size on every SM, else the
+      // call takes the staged path (no grid-wide waits there).  (2) Every launch is a COOPERATIVE launch: the driver
+      // starts the grid only when all of its CTAs can be co-resident -- also next to kernels of other streams or
+      // under an SM partition (MPS, green contexts) -- and fails the launch otherwise instead of letting resident CTAs
+      // spin on CTAs that have no SM.
+      DevState& dv = g_dev[current_device()];
+      int fused_ok = dv.fused_ok.load(std::memory_order_relaxed);
+      if (fused_ok < 0) {
+        int per_sm = 0;
+        if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kFusedThreads, 227 * 1024), "occupancy(moe_fused_kernel)"))
+          return ELDR_ERR_CUDA;
+        int coop = 0;
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, current_device());
+        fused_ok = (per_sm >= 1 && coop) ? 1 : 0;
+        dv.fused_ok.store(fused_ok, std::memory_order_relaxed);
+      }
+      if (fused_ok == 1) {
+        prof_begin();
+        prof_mark(0, st);
+        const cudaError_t le = launch_fused(kern, dv, dim3(num_sms()), dim3(kFusedThreads), smem, st, tm_w13, tm_sw13, tm_w2, tm_sw2, tm_x, tm_h, fa);
+        if (le == cudaErrorCooperativeLaunchTooLarge) {
+          // the device cannot hold the grid right now (partitioned SMs): not an error of the call -- staged path
+          cudaGetLastError();
+          if (g_step_path.load() == ELDR_STEP_FUSED) { snprintf(g_err, sizeof(g_err), "moe_fused_kernel: grid cannot be co-resident"); return ELDR_ERR_UNSUPPORTED; }
+        } else {
+          ++g_launches;
+          if (!cuda_ok(le, "moe_fused_kernel") || !cuda_ok(cudaGetLastError(), "moe_fused_kernel")) return ELDR_ERR_CUDA;
+          prof_mark(ELDR_PROFILE_SLOTS, st);
+          return ELDR_OK;
+        }
+      } else if (g_step_path.load() == ELDR_STEP_FUSED) {
+        snprintf(g_err, sizeof(g_err), "moe_fused_kernel: one CTA per SM is not available on this device");
+        return ELDR_ERR_UNSUPPORTED;
+      }
     }
   }
 
@@ -544,12 +665,10 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
     RouteBigArgs rb{ra, reinterpret_cast<int32_t*>(ws + L.cnt + align_up((size_t)E * 4, 256)), force_routing ? 1 : 0};
     const int n_chunks = (T + kRouteChunk - 1) / kRouteChunk;
     const size_t big_smem = route_big_smem_bytes(E);
-    static bool route_big_attr_set = false;
-    if (!route_big_attr_set) {
-      if (!set_smem(route_count_kernel, route_big_smem_bytes(kMaxExperts)) ||
-          !set_smem(route_scatter_kernel, route_big_smem_bytes(kMaxExperts))) return ELDR_ERR_CUDA;
-      route_big_attr_set = true;
-    }
+    if (!once_per_device(kAttrRouteBig, [] {
+          return set_smem(route_count_kernel, route_big_smem_bytes(kMaxExperts)) &&
+                 set_smem(route_scatter_kernel, route_big_smem_bytes(kMaxExperts));
+        })) return ELDR_ERR_CUDA;
     prof_mark(1, st);
     route_count_kernel<<<n_chunks, kRouteBigThreads, big_smem, st>>>(rb);
     if (!launch_ok("route_count_kernel")) return ELDR_ERR_CUDA;
@@ -564,13 +683,13 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
     size_t smem = (size_t)kGateTok * H * 2;
     if (route_smem > smem) smem = route_smem;
     if (smem > 200 * 1024) return ELDR_ERR_UNSUPPORTED;
-    if (smem > 48 * 1024 && !set_smem(gate_topk_route_kernel, smem)) return ELDR_ERR_CUDA;
+    if (smem > 48 * 1024 && !once_per_device(kAttrGateRoute, [] { return set_smem(gate_topk_route_kernel, 200 * 1024); })) return ELDR_ERR_CUDA;
     dim3 grid((E + kGateExp - 1) / kGateExp, (T + kGateTok - 1) / kGateTok);
     prof_mark(0, st);
     gate_topk_route_kernel<<<grid, 256, smem, st>>>(ga);
     if (!launch_ok("gate_topk_route_kernel")) return ELDR_ERR_CUDA;
   } else {
-    if (route_smem > 48 * 1024 && !set_smem(route_only_kernel, route_smem)) return ELDR_ERR_CUDA;
+    if (route_smem > 48 * 1024 && !once_per_device(kAttrRouteOnly, [] { return set_smem(route_only_kernel, 200 * 1024); })) return ELDR_ERR_CUDA;
     prof_mark(1, st);
     route_only_kernel<<<1, 1024, route_smem, st>>>(ra);
     if (!launch_ok("route_only_kernel")) return ELDR_ERR_CUDA;
@@ -591,7 +710,7 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
   const int sms = num_sms();
   int g13 = max_work * f13.tiles_per_expert; if (g13 > sms) g13 = sms;
   int g2 = max_work * f2.tiles_per_expert; if (g2 > sms) g2 = sms;
-  if (H % 64 == 0 && I % 64 == 0 && g_ffn_path == ELDR_FFN_TCGEN05) {
+  if (H % 64 == 0 && I % 64 == 0 && ffn_path == ELDR_FFN_TCGEN05) {
     // tcgen05 + TMEM path: weights are the M=128 operand, the expert's tokens the N operand
     CUtensorMap tm_w13, tm_sw13, tm_x16, tm_x64, tm_w2, tm_sw2, tm_h16, tm_h64;
     if (!make_tmap_w13_5d(&tm_w13, w13, E, I, H)) return ELDR_ERR_CUDA;
@@ -613,27 +732,24 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
     cfg.np = T <= 64 ? 64 : (T <= kDecodeMaxT ? 128 : 256);
     cfg.stages = T <= 64 ? 8 : (T <= kDecodeMaxT ? 6 : 4);
     const size_t smem = (size_t)cfg.stages * (kUmmaWBytes + cfg.np * 128) + 1024 + 256;
-    static bool umma_attr_set = false;
-    if (!umma_attr_set) {
-      const size_t mx = 8 * (kUmmaWBytes + 64 * 128) + 1024 + 256;
-      if (!set_smem(ffn_umma_kernel<0>, mx) || !set_smem(ffn_umma_kernel<1>, mx)) return ELDR_ERR_CUDA;
-      umma_attr_set = true;
-    }
+    if (!once_per_device(kAttrUmma, [] {
+          const size_t mx = 8 * (kUmmaWBytes + 64 * 128) + 1024 + 256;
+          return set_smem(ffn_umma_kernel<0>, mx) && set_smem(ffn_umma_kernel<1>, mx);
+        })) return ELDR_ERR_CUDA;
     f13.tiles_per_expert = I / 64;
     // auto: from 256 tokens per expert on average (half of the experts then need a second 256-token pass and the pass-
     // level unit list pays): T = 4096 on the Qwen shape 0.605 vs 0.632 ms; below it single-CTA tiles win (T = 3072:
     // 0.462 vs 0.528 ms, T = 3584: 0.510 vs 0.524 ms)
-    const bool pair_pays = g_ffn_pair == 2 || (g_ffn_pair == 1 && (size_t)T * k >= (size_t)256 * E);
+    const int ffn_pair = g_ffn_pair.load();
+    const bool pair_pays = ffn_pair == 2 || (ffn_pair == 1 && (size_t)T * k >= (size_t)256 * E);
     if (T > kDecodeMaxT && pair_pays && I % 128 == 0 && H % 256 == 0 && sms >= 2) {
       // prefill-shaped: M = 256 tiles over SM pairs (ffn_umma2.cuh), six 32 KiB stages per CTA
       const int stages = 6;
       const size_t smem2 = (size_t)stages * kPairStageBytes + 1024 + 256 + (size_t)(2 * max_work + 2) * 4 + 16;
-      static bool pair_attr_set = false;
-      if (!pair_attr_set) {
-        const size_t mx2 = (size_t)stages * kPairStageBytes + 1024 + 256 + (size_t)(2 * (256 + 64) + 4) * 4 + 16;
-        if (!set_smem(ffn_umma2_kernel<0>, mx2) || !set_smem(ffn_umma2_kernel<1>, mx2)) return ELDR_ERR_CUDA;
-        pair_attr_set = true;
-      }
+      if (!once_per_device(kAttrPair, [stages] {
+            const size_t mx2 = (size_t)stages * kPairStageBytes + 1024 + 256 + (size_t)(2 * (256 + 64) + 4) * 4 + 16;
+            return set_smem(ffn_umma2_kernel<0>, mx2) && set_smem(ffn_umma2_kernel<1>, mx2);
+          })) return ELDR_ERR_CUDA;
       const int grid2 = sms & ~1;
       prof_mark(3, st);
       launch_dep_pair(ffn_umma2_kernel<0>, dim3(grid2), dim3(kUmmaThreads), smem2, st, tm_w13, tm_sw13, tm_x16, tm_x64, f13, stages, max_work + 1);
@@ -663,12 +779,9 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
     }
     if (!make_tmap(&tm_x, x_perm, (uint64_t)x_rows, H, kFfnXBox)) return ELDR_ERR_CUDA;
     if (!make_tmap(&tm_h, hbuf, (uint64_t)out_rows, I, kFfnXBox)) return ELDR_ERR_CUDA;
-    static bool attr_set = false;
-    if (!attr_set) {
-      if (!set_smem(ffn_stream_kernel<0>, kFfnSmemBytes) || !set_smem(ffn_stream_kernel<1>, kFfnSmemBytes))
-        return ELDR_ERR_CUDA;
-      attr_set = true;
-    }
+    if (!once_per_device(kAttrStream, [] {
+          return set_smem(ffn_stream_kernel<0>, kFfnSmemBytes) && set_smem(ffn_stream_kernel<1>, kFfnSmemBytes);
+        })) return ELDR_ERR_CUDA;
     prof_mark(3, st);
     launch_dep(ffn_stream_kernel<0>, dim3(g13), dim3(kFfnThreads), kFfnSmemBytes, st, tm_w13, tm_sw13, tm_x, f13);
     if (!launch_ok("ffn_stream_kernel<w13>")) return ELDR_ERR_CUDA;
@@ -826,11 +939,7 @@ int32_t eldr_route_decide(const eldr_moe_shape_t* s, int32_t R, int32_t K, const
   if (R == 0) return ELDR_OK;
   if (!sig_req || !idf || !layer_mask || !centroids || !loads || !worker || !sims) return ELDR_ERR_INVALID_ARG;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  static bool route_attr_set = false;
-  if (!route_attr_set) {
-    if (!set_smem(route_sims_kernel, kRouteStageCells * 4)) return ELDR_ERR_CUDA;
-    route_attr_set = true;
-  }
+  if (!once_per_device(kAttrRouteSims, [] { return set_smem(route_sims_kernel, kRouteStageCells * 4); })) return ELDR_ERR_CUDA;
   route_sims_kernel<<<dim3(R, (K + 7) / 8 < 16 ? (K + 7) / 8 : 16), 256, kRouteStageCells * 4, st>>>(sig_req, idf, layer_mask, centroids, sims, s->n_layers, s->n_experts, K);
   if (!launch_ok("route_sims_kernel")) return ELDR_ERR_CUDA;
   route_pick_kernel<<<1, kRoutePickThreads, 0, st>>>(sims, loads, worker, R, K, tau);

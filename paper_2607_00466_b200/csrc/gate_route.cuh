@@ -158,8 +158,11 @@ __device__ __forceinline__ void warp_topk(const float* __restrict__ zrow, int E,
 
 // ------------------------------------------------------------------------ a3: signature increments
 // int32 request cell: atomic add.  int8 block cell: CUDA has no 8-bit atomics -> 32-bit atomic add of
-// 1 << 8*(byte in word) on the aligned word; no carry can cross because a cell never exceeds the KV
-// block size (<= 127; ids are distinct per token).  Integer adds commute => bit-exact in any order.
+// 1 << 8*(byte in word) on the aligned word.  Under the contract a cell never exceeds the KV block size
+// (<= 127; ids are distinct per token).  A caller that keeps accumulating into a block it never resets would
+// otherwise carry into the NEIGHBOURING expert's cell: the cell saturates at 127 instead (reading in DESIGN.md 2;
+// the add is undone when the cell already held 127 -- transient values stay below 256 because at most a block's
+// worth of adds to one cell can be in flight).  Integer adds commute => bit-exact in any order.
 __device__ __forceinline__ void sig_add(int32_t* sig_req, int8_t* sig_block, int req, int blk, int L,
                                         int layer, int E, int e) {
   if (sig_req != nullptr && req >= 0)
@@ -167,7 +170,9 @@ __device__ __forceinline__ void sig_add(int32_t* sig_req, int8_t* sig_block, int
   if (sig_block != nullptr && blk >= 0) {
     const size_t idx = ((size_t)blk * L + layer) * E + e;
     unsigned int* word = reinterpret_cast<unsigned int*>(sig_block + (idx & ~(size_t)3));
-    atomicAdd(word, 1u << (8u * (unsigned)(idx & 3)));
+    const unsigned int shift = 8u * (unsigned)(idx & 3), inc = 1u << shift;
+    const unsigned int old = atomicAdd(word, inc);
+    if (((old >> shift) & 0xffu) >= 127u) atomicSub(word, inc);
   }
 }
 

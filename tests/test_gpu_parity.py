@@ -771,3 +771,69 @@ def test_prefill_shaped_forced_routing_and_determinism(gpu, oracle):
         outs.append(dl.run(xg, None, force_routing=1).clone())
         torch.cuda.synchronize()
     assert torch.equal(outs[0], outs[1])
+
+
+# ------------------------------------------------------------------------------------ boundary hardening
+def test_int8_block_cells_saturate_at_127_on_gpu(gpu, oracle):
+    """127/128 boundary of an int8 block cell (DESIGN.md 2 reading "int8 cells saturate"): 130 accumulations into one
+    row -- through eldr_signature_accumulate and through the fused step's in-kernel increments -- stop at 127 and never
+    carry into the neighbouring expert's cell (the cells share a 32-bit word on the GPU); equals the oracle."""
+    import torch
+    shape = synth.MoEShape(hidden=64, inter=64, n_experts=8, top_k=2, n_layers=1, kv_block_size=16)
+    E = shape.n_experts
+    ids = np.tile(np.array([[3, 5], [4, 5]], np.int32), (65, 1))            # cells 3, 4: 65 each; cell 5: 130
+    T = ids.shape[0]
+    req = np.zeros(T, np.int32)
+    blk = np.zeros(T, np.int32)
+    sig_req = torch.zeros((1, 1, E), dtype=torch.int32, device="cuda")
+    sig_blk = torch.zeros((1, 1, E), dtype=torch.int8, device="cuda")
+    gpu.eldr_signature_accumulate(shape, 0, torch.from_numpy(ids).cuda(), torch.from_numpy(req).cuda(),
+                                  torch.from_numpy(blk).cuda(), sig_req, sig_blk)
+    o_req = np.zeros((1, 1, E), np.int32)
+    o_blk = np.zeros((1, 1, E), np.int8)
+    oracle.signature_accumulate(shape, 0, ids, req, blk, o_req, o_blk)
+    assert np.array_equal(sig_blk.cpu().numpy(), o_blk) and np.array_equal(sig_req.cpu().numpy(), o_req)
+    assert sig_blk.cpu().numpy()[0, 0].tolist() == [0, 0, 0, 65, 65, 127, 0, 0]
+    # the fused step's own increments: the same decode batch recorded 130 times into the same 4 block rows
+    lw = synth.make_layer_weights(shape, 3, w_std=0.05, gate_std=0.3)
+    dl = gpu.DecodeLayer(shape, lw, max_T=4)
+    x = gpu.bf16_from_bits(synth.make_hidden(4, shape.hidden, 3))
+    d_blk = torch.arange(4, dtype=torch.int32, device="cuda")
+    sig_blk2 = torch.zeros((4, 1, E), dtype=torch.int8, device="cuda")
+    for _ in range(130):
+        dl.run(x, None, token_req=None, token_block=d_blk, sig_req=None, sig_block=sig_blk2)
+    torch.cuda.synchronize()
+    assert gpu.eldr_moe_last_launch_count() == 1
+    got = sig_blk2.cpu().numpy()[:, 0]
+    ids_g = dl.ids[:4].cpu().numpy()
+    want = np.zeros((4, E), np.int8)
+    for t in range(4):
+        want[t, ids_g[t]] = 127
+    assert np.array_equal(got, want)
+
+
+def test_two_layers_on_two_streams_match_serial_results(gpu, oracle):
+    """Two DecodeLayers (own workspaces) enqueued from two streams at the same time.  The fused step is a persistent
+    grid whose CTAs wait on one another; it is launched cooperatively, so two such grids can never be half-resident
+    together -- the second waits for the first (or the launch fails cleanly): results are the serial ones bit for
+    bit, never a spin-cap trap."""
+    import torch
+    shape = synth.SHAPE_QWEN
+    lw = synth.make_layer_weights(shape, synth.WEIGHT_SEED)
+    dls = [gpu.DecodeLayer(shape, lw, max_T=64) for _ in range(2)]
+    cases = []
+    for u in (16, 96):
+        xb, bias = synth.union_case(shape, 64, u, synth.accepted_union_seed(64, u))
+        cases.append((gpu.bf16_from_bits(xb), torch.from_numpy(bias).cuda()))
+    ref = [dls[i].run(*cases[i]).clone() for i in range(2)]
+    torch.cuda.synchronize()
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    outs = [[], []]
+    for rep in range(20):
+        for i in range(2):
+            with torch.cuda.stream(streams[i]):
+                outs[i].append(dls[i].run(*cases[i]).clone())
+    torch.cuda.synchronize()
+    for i in range(2):
+        for o in outs[i]:
+            assert torch.equal(o.view(torch.int16), ref[i].view(torch.int16))

@@ -323,3 +323,20 @@ def test_signature_prefix_sharing_equals_cold_prefill_and_reset(oracle):
     assert not sig_block[b].any()
     other = wl.req_blocks[2]
     assert sig_block[other].any()
+
+
+def test_int8_block_cells_saturate_at_127(oracle):
+    """DESIGN.md 2 reading "int8 cells saturate": 130 tokens written into ONE block row (outside PAPER.md:255's
+    contract of <= block-size tokens per block) leave the cell at 127, its neighbours untouched, and the int32
+    request row at the true count -- pinned against numpy's clip."""
+    shape = synth.MoEShape(hidden=8, inter=8, n_experts=8, top_k=2, n_layers=1, kv_block_size=16)
+    T = 130
+    ids = np.tile(np.array([[3, 5]], np.int32), (T, 1))
+    req = np.zeros(T, np.int32)
+    blk = np.zeros(T, np.int32)
+    sig_req = np.zeros((1, 1, 8), np.int32)
+    sig_blk = np.zeros((1, 1, 8), np.int8)
+    oracle.signature_accumulate(shape, 0, ids, req, blk, sig_req, sig_blk)
+    want = np.clip(np.bincount(ids.ravel(), minlength=8), 0, 127)
+    assert sig_blk[0, 0].tolist() == want.tolist() == [0, 0, 0, 127, 0, 127, 0, 0]
+    assert sig_req[0, 0].tolist() == [0, 0, 0, 130, 0, 130, 0, 0]
