@@ -51,12 +51,13 @@ def lib_path() -> str:
     return _build.LIB
 
 
-def load(build_if_missing: bool = False):
-    """dlopen the CUDA library.  Raises if it is not built (no fallback)."""
+def load(build_if_missing: bool = False, path: Optional[str] = None):
+    """dlopen the CUDA library.  Raises if it is not built (no fallback).  `path`: another build of the same library
+    (the -DELDR_TRACE one of `bench.py --timeline`); must be given on the first load of the process."""
     global _lib
     if _lib is not None:
         return _lib
-    path = _build.LIB
+    path = path or _build.LIB
     if not os.path.exists(path):
         if build_if_missing:
             _build.build()

@@ -18,27 +18,34 @@ def _headers():
     return sorted(glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(CSRC, "*.h")))
 
 
-def _stale() -> bool:
-    if not os.path.exists(LIB):
+def _stale(lib: str = None) -> bool:
+    lib = lib or LIB
+    if not os.path.exists(lib):
         return True
-    t = os.path.getmtime(LIB)
+    t = os.path.getmtime(lib)
     deps = [os.path.join(CSRC, f) for f in SOURCES] + _headers() + [os.path.join(_ROOT, "include", "eldr_moe.h")]
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and not _stale():
-        return LIB
+TRACE_LIB = os.path.join(CSRC, "libeldr_moe_trace.so")
+
+
+def build(force: bool = False, verbose: bool = False, trace: bool = False) -> str:
+    """trace=True builds a SECOND library, libeldr_moe_trace.so, with -DELDR_TRACE: the fused kernel then stamps
+    %globaltimer at its milestones (`bench.py --timeline`).  The measured library carries no trace code."""
+    lib = TRACE_LIB if trace else LIB
+    if not force and not _stale(lib):
+        return lib
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
            "-Xcompiler", "-fPIC", "-shared", "-I", os.path.join(_ROOT, "include"), "-I", CSRC,
-           "-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
-    cmd[1:1] = os.environ.get("ELDR_EXTRA_NVCC_FLAGS", "").split()
+           "-o", lib] + [os.path.join(CSRC, s) for s in SOURCES]
+    cmd[1:1] = os.environ.get("ELDR_EXTRA_NVCC_FLAGS", "").split() + (["-DELDR_TRACE"] if trace else [])
     if verbose:
         cmd.insert(1, "-Xptxas")
         cmd.insert(2, "-v")
     subprocess.check_call(cmd)
-    return LIB
+    return lib
 
 
 if __name__ == "__main__":

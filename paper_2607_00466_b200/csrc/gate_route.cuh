@@ -176,6 +176,30 @@ __device__ __forceinline__ void sig_add(int32_t* sig_req, int8_t* sig_block, int
   }
 }
 
+// The same increment in two halves, for a caller that must not wait for the atomic's round trip (the fused step's
+// top-k owners sit on the serial prelude): begin() issues both adds and keeps the int8 word's OLD value in flight;
+// finish(), called when the step's work is done, undoes the add if the cell was already saturated.
+struct SigPending {
+  unsigned int* word;
+  unsigned int old, shift;
+};
+__device__ __forceinline__ SigPending sig_add_begin(int32_t* sig_req, int8_t* sig_block, int req, int blk, int L,
+                                                    int layer, int E, int e) {
+  SigPending p{nullptr, 0u, 0u};
+  if (sig_req != nullptr && req >= 0)
+    atomicAdd(sig_req + ((size_t)req * L + layer) * E + e, 1);
+  if (sig_block != nullptr && blk >= 0) {
+    const size_t idx = ((size_t)blk * L + layer) * E + e;
+    p.word = reinterpret_cast<unsigned int*>(sig_block + (idx & ~(size_t)3));
+    p.shift = 8u * (unsigned)(idx & 3);
+    p.old = atomicAdd(p.word, 1u << p.shift);
+  }
+  return p;
+}
+__device__ __forceinline__ void sig_add_finish(const SigPending& p) {
+  if (p.word != nullptr && ((p.old >> p.shift) & 0xffu) >= 127u) atomicSub(p.word, 1u << p.shift);
+}
+
 struct TopkArgs {
   const float* z;            // [T,E]
   int32_t* ids;              // [T,k]

@@ -786,9 +786,6 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
 
   // ------------------------------------------------------------- prologue (overlaps the previous kernel's tail)
   if (tid == 0) FSTAMP2(8);
-#ifdef ELDR_TRACE
-  const unsigned long long t_entry_ = gtime();
-#endif
   if (tid == 0) {
     for (int s = 0; s < kMaxStages; ++s) { mbar_init(full_bar(s), 2); mbar_init(empty_bar(s), 1); }
     for (int b = 0; b < 2; ++b) { mbar_init(tfull_bar(b), 1); mbar_init(tempty_bar(b), 4); }
@@ -821,9 +818,6 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
   if (tid == 0) FSTAMP(1);
 
   const uint32_t epoch = __ldcg(a.sync + kSyncGen) + 1u;
-#ifdef ELDR_TRACE
-  if (tid == 0) atomicMax(&g_trace[(3000 + (epoch & 63)) * 16 + 0], ~t_entry_);     // earliest CTA entry of this step
-#endif
   if (cta == 0 && tid == 0) {
     // this step's tile counters (the previous grid has completed: pdl_wait above)
     a.sync[kSyncTileCnt] = 0u;
@@ -833,6 +827,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
   }
 
   // ------------------------------------------------------------------------------ G + K: gate and top-k
+  SigPending sig_pend{nullptr, 0u, 0u};     // this lane's signature increment of the step, saturation check deferred to the end
   if (!a.force_routing) {
     const int n_et = (E + kGateExp - 1) / kGateExp, n_gr = (T + kGateTok - 1) / kGateTok;
     const int n_tiles = n_et * ((T + GT - 1) / GT);
@@ -862,8 +857,9 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
           a.tk.ids[(size_t)t * k + lane] = id;
           a.tk.w[(size_t)t * k + lane] = w;
           st_relaxed_u64(a.wtag + (size_t)t * kMaxTopK + lane, ((unsigned long long)epoch << 32) | __float_as_uint(w));
-          sig_add(a.tk.sig_req, a.tk.sig_block, a.tk.token_req ? a.tk.token_req[t] : -1,
-                  a.tk.token_block ? a.tk.token_block[t] : -1, a.tk.L, a.tk.layer, E, id);
+          sig_add_finish(sig_pend);          // (a second group of this owner: T <= 256 never has one)
+          sig_pend = sig_add_begin(a.tk.sig_req, a.tk.sig_block, a.tk.token_req ? a.tk.token_req[t] : -1,
+                                   a.tk.token_block ? a.tk.token_block[t] : -1, a.tk.L, a.tk.layer, E, id);
         }
       }
     }
@@ -1288,52 +1284,12 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
   // combined: barrier + combine 3.4 us after the last tile).  Polls are one 4-byte load per slot and sleep 250 ns in
   // between: warps that polled from the moment their role ended, all lanes, every 100 ns, hot-spotted the flags' L2
   // lines and cost every step 40 us (measured).
-#ifdef ELDR_OLD_TAIL
-  if (tid == 0) FSTAMP(8);
-  __syncthreads();
-  if (tid == 0) flag_release(a.sync + kSyncDone + cta, epoch);
-  if (warp == 0) warp_wait_flags(a.sync + kSyncDone, G, epoch, lane);
-  __syncthreads();
-  {
-    const int q_per_row = H >> 2;
-    for (int idx = cta * kFusedThreads + tid; idx < T * q_per_row; idx += G * kFusedThreads) {
-      const int t = idx / q_per_row, c4 = idx - t * q_per_row;
-      int pos[kMaxTopK];
-      float wt[kMaxTopK];
-      float4 v[kMaxTopK];
-#pragma unroll
-      for (int j = 0; j < kMaxTopK; ++j)
-        if (j < k) { pos[j] = sm.pos_of_pair[t * k + j]; wt[j] = __ldcg(a.tk.w + t * k + j); }
-#pragma unroll
-      for (int j = 0; j < kMaxTopK; ++j)
-        if (j < k) v[j] = __ldcg(reinterpret_cast<const float4*>(a.ybuf + (size_t)pos[j] * H + (size_t)c4 * 4));
-      float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll
-      for (int j = 0; j < kMaxTopK; ++j)
-        if (j < k) {
-          acc.x = fmaf(wt[j], v[j].x, acc.x); acc.y = fmaf(wt[j], v[j].y, acc.y);
-          acc.z = fmaf(wt[j], v[j].z, acc.z); acc.w = fmaf(wt[j], v[j].w, acc.w);
-        }
-      for (int s = 0; s < ns; ++s) {
-        const float4 sv = __ldcg(reinterpret_cast<const float4*>(a.ybuf + ((size_t)T * k + (size_t)s * T + t) * H + (size_t)c4 * 4));
-        acc.x += sv.x; acc.y += sv.y; acc.z += sv.z; acc.w += sv.w;
-      }
-      uint2 o;
-      o.x = (uint32_t)f32_to_bf16_rn(acc.x) | ((uint32_t)f32_to_bf16_rn(acc.y) << 16);
-      o.y = (uint32_t)f32_to_bf16_rn(acc.z) | ((uint32_t)f32_to_bf16_rn(acc.w) << 16);
-      *reinterpret_cast<uint2*>(a.out + (size_t)t * H + (size_t)c4 * 4) = o;
-    }
-  }
-  if (tid == 0) FSTAMP(10);
-  if (cta == 0 && tid == 0) a.sync[kSyncGen] = epoch;
-  tc_fence_before();
-  __syncthreads();
-#else
   if (tid == 0) FSTAMP(8);
   __syncthreads();
   if (k <= 8) fused_combine<8>(a, sm, ydone, epoch, n_work, tilesB, cta, G, warp, lane);
   else fused_combine<kMaxTopK>(a, sm, ydone, epoch, n_work, tilesB, cta, G, warp, lane);
   if (tid == 0) FSTAMP(10);
+  sig_add_finish(sig_pend);
 
   tc_fence_before();
   __syncthreads();
@@ -1346,13 +1302,9 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     // every step 30 us (measured).
     if (atomicAdd(a.sync + kSyncExit, 1u) == (uint32_t)G - 1u) a.sync[kSyncGen] = epoch;
   }
-#endif
   if (warp == 6) {
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_base), "r"(tmem_cols) : "memory");
   }
-#ifdef ELDR_TRACE
-  if (tid == 0) atomicMax(&g_trace[(3000 + (epoch & 63)) * 16 + 1], gtime());        // latest CTA exit of this step
-#endif
 }
 
 }  // namespace eldr
