@@ -120,6 +120,30 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* shape, int32_t layer, int3
                               int32_t* sig_req, int8_t* sig_block,
                               void* workspace, size_t workspace_bytes, eldr_stream_t stream);
 
+/* The same step with MXFP4 expert weights (section 6 Testbed: "GPT-OSS-120B (128
+ * experts, top-4, mxfp4)").  The paper only names the format; readings (oracle/mxfp4.py): OCP MX v1.0 --
+ * element = FP4 E2M1 code (sign, 2 exponent bits bias 1, 1 mantissa bit: magnitudes 0, .5, 1, 1.5, 2, 3, 4, 6), two
+ * codes per byte with element 2i in the LOW nibble; one E8M0 scale byte per 32 consecutive elements of the
+ * contraction (innermost) axis, value = e2m1(code) * 2^(scale - 127).  Scale bytes must lie in 3..250 (every decoded
+ * value is then exactly a bf16 number; 255 = NaN is outside the contract).
+ *   w13_codes [E,2I,H/2] uint8, w13_scales [E,2I,H/32] uint8 (rows 0..I-1 = w1, I..2I-1 = w3);
+ *   w2_codes  [E,H,I/2]  uint8, w2_scales  [E,H,I/32]  uint8.  All device pointers, 16-byte aligned.
+ * Operation: eldr_moe_decode_layer on the DECODED weights -- activations stay bf16 and are not quantised, products
+ * accumulate in fp32 -- so the same oracle and tolerances apply.  Only the packed bytes are read from HBM
+ * ((|U|)*3*H*I*(1/2 + 1/32) bytes per step); they are decoded to bf16 in shared memory on the way to the tensor cores.
+ * Every other argument as eldr_moe_decode_layer.  Restrictions: T <= 1024, n_shared == 0, H % 64 == 0, I % 64 == 0
+ * (else ELDR_ERR_UNSUPPORTED).  Five launches (gate+top-k+signature+routing, gather, w1/w3, w2, combine). */
+int32_t eldr_moe_decode_layer_mxfp4(const eldr_moe_shape_t* shape, int32_t layer, int32_t T,
+                                    const eldr_bf16* x, const float* gate_w, const float* gate_bias,
+                                    const uint8_t* w13_codes, const uint8_t* w13_scales,
+                                    const uint8_t* w2_codes, const uint8_t* w2_scales,
+                                    eldr_bf16* out,
+                                    int32_t* topk_ids, float* topk_w, int32_t force_routing,
+                                    int32_t* active_experts, int32_t* n_active,
+                                    const int32_t* token_req, const int32_t* token_block,
+                                    int32_t* sig_req, int8_t* sig_block,
+                                    void* workspace, size_t workspace_bytes, eldr_stream_t stream);
+
 /* Same step with the per-step inputs and results in HOST memory (pinned for async copies): copies h_x and
  * the token maps to the device, runs eldr_moe_decode_layer, copies out / ids / weights / n_active back and
  * synchronises `stream` before returning.  Weights, gate, signature tables and workspace stay on the device.

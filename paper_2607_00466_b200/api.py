@@ -18,7 +18,7 @@ from . import build as _build
 _lib = None
 
 EXPORTS = [
-    "eldr_moe_gate_topk", "eldr_moe_decode_layer", "eldr_moe_decode_layer_host",
+    "eldr_moe_gate_topk", "eldr_moe_decode_layer", "eldr_moe_decode_layer_host", "eldr_moe_decode_layer_mxfp4",
     "eldr_signature_accumulate", "eldr_signature_reset_blocks", "eldr_signature_readout", "eldr_route_decide",
     "eldr_moe_workspace_bytes", "eldr_moe_workspace_bytes_host", "eldr_moe_workspace_layout",
     "eldr_moe_last_launch_count", "eldr_status_string", "eldr_last_cuda_error",
@@ -175,6 +175,22 @@ def eldr_moe_decode_layer(shape, layer: int, x, gate_w, gate_bias, w13, w2, shar
         _stream()), "eldr_moe_decode_layer")
 
 
+def eldr_moe_decode_layer_mxfp4(shape, layer: int, x, gate_w, gate_bias, w13_codes, w13_scales, w2_codes, w2_scales, out,
+                                topk_ids, topk_w, force_routing: int, active_experts, n_active,
+                                token_req=None, token_block=None, sig_req=None, sig_block=None, workspace=None):
+    s = make_shape(shape)
+    T = x.shape[0]
+    _check(load().eldr_moe_decode_layer_mxfp4(
+        C.byref(s), C.c_int32(layer), C.c_int32(T), _ptr(x, torch.bfloat16), _ptr(gate_w, torch.float32),
+        _ptr(gate_bias, torch.float32), _ptr(w13_codes, torch.uint8), _ptr(w13_scales, torch.uint8),
+        _ptr(w2_codes, torch.uint8), _ptr(w2_scales, torch.uint8), _ptr(out, torch.bfloat16),
+        _ptr(topk_ids, torch.int32), _ptr(topk_w, torch.float32), C.c_int32(force_routing),
+        _ptr(active_experts, torch.int32), _ptr(n_active, torch.int32),
+        _ptr(token_req, torch.int32), _ptr(token_block, torch.int32), _ptr(sig_req, torch.int32),
+        _ptr(sig_block, torch.int8), _ptr(workspace), C.c_size_t(workspace.numel() * workspace.element_size()),
+        _stream()), "eldr_moe_decode_layer_mxfp4")
+
+
 def eldr_moe_decode_layer_host(shape, layer: int, h_x, gate_w, gate_bias, w13, w2, shared_w13, shared_w2,
                                h_out, h_topk_ids, h_topk_w, h_n_active, h_token_req=None, h_token_block=None,
                                sig_req=None, sig_block=None, workspace=None):
@@ -266,3 +282,33 @@ class DecodeLayer:
         off = getattr(L, name)
         n = int(np.prod(spec[1])) * torch.empty((), dtype=spec[0]).element_size()
         return self.workspace[off: off + n].view(spec[0]).view(spec[1])
+
+
+class MxDecodeLayer:
+    """Holder of one MXFP4 layer's device tensors + workspace (plumbing; no arithmetic).  `w13` / `w2` are
+    (codes uint8 [E,rows,K/2], scales uint8 [E,rows,K/32]) numpy pairs."""
+
+    def __init__(self, shape, gate_w, w13, w2, max_T: int, device="cuda"):
+        self.shape = shape
+        self.gate_w = torch.from_numpy(gate_w).to(device)
+        self.w13_codes, self.w13_scales = (torch.from_numpy(np.ascontiguousarray(a)).to(device) for a in w13)
+        self.w2_codes, self.w2_scales = (torch.from_numpy(np.ascontiguousarray(a)).to(device) for a in w2)
+        self.max_T = max_T
+        self.workspace = torch.empty(eldr_moe_workspace_bytes(shape, max_T), dtype=torch.uint8, device=device)
+        E, k, H = shape.n_experts, shape.top_k, shape.hidden
+        self.out = torch.empty((max_T, H), dtype=torch.bfloat16, device=device)
+        self.ids = torch.empty((max_T, k), dtype=torch.int32, device=device)
+        self.w = torch.empty((max_T, k), dtype=torch.float32, device=device)
+        self.active = torch.empty((E,), dtype=torch.int32, device=device)
+        self.n_active = torch.zeros((1,), dtype=torch.int32, device=device)
+
+    def run(self, x, gate_bias=None, layer=0, force_routing=0, token_req=None, token_block=None,
+            sig_req=None, sig_block=None):
+        T = x.shape[0]
+        eldr_moe_decode_layer_mxfp4(self.shape, layer, x, self.gate_w, gate_bias, self.w13_codes, self.w13_scales,
+                                    self.w2_codes, self.w2_scales, self.out[:T], self.ids[:T], self.w[:T],
+                                    force_routing, self.active, self.n_active, token_req, token_block,
+                                    sig_req, sig_block, self.workspace)
+        return self.out[:T]
+
+    ws_view = DecodeLayer.ws_view

@@ -13,6 +13,7 @@
 #include "ffn_stream.cuh"
 #include "ffn_umma.cuh"
 #include "ffn_umma2.cuh"
+#include "ffn_mx.cuh"
 #include "gate_route.cuh"
 #include "gate_prefill.cuh"
 #include "moe_fused.cuh"
@@ -136,7 +137,7 @@ void make_host_stage(const eldr_moe_shape_t* s, int T, size_t base, HostStage* S
 // grid are properties of the device the call runs on, so everything cached here is keyed by the device ordinal.
 constexpr int kMaxDevices = 64;
 enum { kAttrFused = 0, kAttrRouteBig, kAttrUmma, kAttrPair, kAttrStream, kAttrRouteSims, kAttrGateLogits, kAttrGateRoute,
-       kAttrRouteOnly, kAttrCount };
+       kAttrRouteOnly, kAttrMx, kAttrCount };
 struct DevState {
   std::atomic<int> sms{0};
   std::atomic<int> fused_ok{-1};          // -1 unknown, 0 the persistent grid cannot be co-resident, 1 it can
@@ -251,6 +252,24 @@ bool make_tmap(CUtensorMap* out, const void* ptr, uint64_t rows, uint64_t cols, 
                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) { snprintf(g_err, sizeof(g_err), "cuTensorMapEncodeTiled failed: %d", (int)r); return false; }
+  tmap_store(key, *out);
+  return true;
+}
+
+// uint8 [rows, row_bytes] row-major, box = box_rows x 128 bytes, SWIZZLE_128B (packed MXFP4 codes: 256 codes per row per box)
+bool make_tmap_u8(CUtensorMap* out, const void* ptr, uint64_t rows, uint64_t row_bytes, uint32_t box_rows) {
+  const TmapKey key{ptr, rows, row_bytes, box_rows, 8, current_device()};
+  if (tmap_lookup(key, out)) return true;
+  encode_tiled_fn fn = get_encode_fn();
+  if (!fn) { snprintf(g_err, sizeof(g_err), "cuTensorMapEncodeTiled entry point not found"); return false; }
+  cuuint64_t gdim[2] = {row_bytes, rows};
+  cuuint64_t gstride[1] = {row_bytes};
+  cuuint32_t box[2] = {128, box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(ptr), gdim, gstride, box, estr,
+                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) { snprintf(g_err, sizeof(g_err), "cuTensorMapEncodeTiled(u8) failed: %d", (int)r); return false; }
   tmap_store(key, *out);
   return true;
 }
@@ -801,6 +820,114 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
   prof_mark(5, st);
   launch_dep(k <= 8 ? combine_kernel<8> : combine_kernel<kMaxTopK>, dim3((T * (H / 4) + 255) / 256), dim3(256), 0, st,
              ybuf, topk_w, pair_pos, out, T, H, k, ns);
+  if (!launch_ok("combine_kernel")) return ELDR_ERR_CUDA;
+  prof_mark(ELDR_PROFILE_SLOTS, st);
+  return ELDR_OK;
+}
+
+int32_t eldr_moe_decode_layer_mxfp4(const eldr_moe_shape_t* s, int32_t layer, int32_t T, const eldr_bf16* x,
+                                    const float* gate_w, const float* gate_bias, const uint8_t* w13_codes,
+                                    const uint8_t* w13_scales, const uint8_t* w2_codes, const uint8_t* w2_scales,
+                                    eldr_bf16* out, int32_t* topk_ids, float* topk_w, int32_t force_routing,
+                                    int32_t* active_experts, int32_t* n_active, const int32_t* token_req,
+                                    const int32_t* token_block, int32_t* sig_req, int8_t* sig_block,
+                                    void* workspace, size_t workspace_bytes, eldr_stream_t stream) {
+  g_launches = 0;
+  int32_t rc = check_shape(s);
+  if (rc != ELDR_OK) return rc;
+  if (T < 0 || layer < 0 || layer >= s->n_layers) return ELDR_ERR_INVALID_ARG;
+  if (T == 0) return ELDR_OK;
+  if (!x || !w13_codes || !w13_scales || !w2_codes || !w2_scales || !out || !topk_ids || !topk_w || !active_experts ||
+      !n_active || !workspace) return ELDR_ERR_INVALID_ARG;
+  if (!force_routing && !gate_w) return ELDR_ERR_INVALID_ARG;
+  if (!aligned16(x) || !aligned16(gate_w) || !aligned16(w13_codes) || !aligned16(w13_scales) || !aligned16(w2_codes) ||
+      !aligned16(w2_scales) || !aligned16(out) || !aligned16(workspace) || !aligned16(sig_block)) return ELDR_ERR_INVALID_ARG;
+  // decode-shaped calls, no shared experts, whole 64-element k-chunks (two 32-element scale blocks each)
+  if (T > kDecodeMaxT || s->n_shared != 0 || s->hidden % 64 || s->inter % 64) return ELDR_ERR_UNSUPPORTED;
+  eldr_moe_ws_layout_t L;
+  make_layout(s, T, &L);
+  if (workspace_bytes < L.total) return ELDR_ERR_WORKSPACE_SMALL;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  uint8_t* ws = static_cast<uint8_t*>(workspace);
+  const int H = s->hidden, I = s->inter, E = s->n_experts, k = s->top_k;
+  float* z = reinterpret_cast<float*>(ws + L.z);
+  int32_t* perm = reinterpret_cast<int32_t*>(ws + L.perm);
+  int32_t* pair_pos = reinterpret_cast<int32_t*>(ws + L.pair_pos);
+  int4* work = reinterpret_cast<int4*>(ws + L.work);
+  int32_t* n_work = reinterpret_cast<int32_t*>(ws + L.n_work);
+  uint16_t* x_perm = reinterpret_cast<uint16_t*>(ws + L.x_perm);
+  uint16_t* hbuf = reinterpret_cast<uint16_t*>(ws + L.h);
+  float* ybuf = reinterpret_cast<float*>(ws + L.y);
+  prof_begin();
+  RouteArgs ra;
+  ra.tk = TopkArgs{z, topk_ids, topk_w, token_req, token_block, sig_req, sig_block, T, E, k, s->n_layers, layer, s->renormalize};
+  ra.force_routing = force_routing ? 1 : 0;
+  ra.n_shared = 0;
+  ra.H = H;
+  ra.cnt = reinterpret_cast<int32_t*>(ws + L.cnt);
+  ra.off = reinterpret_cast<int32_t*>(ws + L.off);
+  ra.perm = perm; ra.pair_pos = pair_pos; ra.work = work; ra.n_work = n_work;
+  ra.active = active_experts; ra.n_active = n_active;
+  const int W = (T + 31) / 32;
+  const size_t route_smem = (size_t)E * W * 8 + (size_t)(2 * E + 1) * 4;
+  if (!force_routing) {
+    GateRouteArgs ga;
+    ga.x = x; ga.gate_w = gate_w; ga.gate_bias = gate_bias; ga.r = ra;
+    ga.sync = reinterpret_cast<uint32_t*>(ws + L.sync + align_up(fused_sync_words(E, 0, I, H) * 4, 256));
+    size_t smem = (size_t)kGateTok * H * 2;
+    if (route_smem > smem) smem = route_smem;
+    if (smem > 200 * 1024) return ELDR_ERR_UNSUPPORTED;
+    if (smem > 48 * 1024 && !once_per_device(kAttrGateRoute, [] { return set_smem(gate_topk_route_kernel, 200 * 1024); })) return ELDR_ERR_CUDA;
+    dim3 grid((E + kGateExp - 1) / kGateExp, (T + kGateTok - 1) / kGateTok);
+    prof_mark(0, st);
+    gate_topk_route_kernel<<<grid, 256, smem, st>>>(ga);
+    if (!launch_ok("gate_topk_route_kernel")) return ELDR_ERR_CUDA;
+  } else {
+    if (route_smem > 48 * 1024 && !once_per_device(kAttrRouteOnly, [] { return set_smem(route_only_kernel, 200 * 1024); })) return ELDR_ERR_CUDA;
+    prof_mark(1, st);
+    route_only_kernel<<<1, 1024, route_smem, st>>>(ra);
+    if (!launch_ok("route_only_kernel")) return ELDR_ERR_CUDA;
+  }
+  const int x_rows = T * k;
+  prof_mark(2, st);
+  launch_dep(gather_x_kernel, dim3((x_rows + 7) / 8), dim3(256), 0, st, x, perm, x_perm, T, H, k, x_rows);
+  if (!launch_ok("gather_x_kernel")) return ELDR_ERR_CUDA;
+
+  const int max_work = E < T * k ? E : T * k;
+  MxArgs m13, m2;
+  m13.f = FfnArgs{work, n_work, E, H, 2 * I, I, H, I / 64, hbuf, nullptr};
+  m2.f = FfnArgs{work, n_work, E, I, H, I, H, (H + 127) / 128, nullptr, ybuf};
+  m13.scales = w13_scales;
+  m2.scales = w2_scales;
+  m13.np = m2.np = T <= 64 ? 64 : 128;
+  m13.stages = m2.stages = 3;
+  m13.raw_stages = m2.raw_stages = 5;
+  m13.act_stages = m2.act_stages = T <= 64 ? 8 : 4;
+  const size_t smem = mx_smem_bytes(m13.np, m13.stages, m13.raw_stages, m13.act_stages);
+  if (!once_per_device(kAttrMx, [] {
+        const size_t a_ = mx_smem_bytes(64, 3, 5, 8), b_ = mx_smem_bytes(128, 3, 5, 4);
+        const size_t mx = a_ > b_ ? a_ : b_;
+        return set_smem(ffn_mx_kernel<0>, mx) && set_smem(ffn_mx_kernel<1>, mx);
+      })) return ELDR_ERR_CUDA;
+  CUtensorMap tm_c13, tm_c2, tm_x16, tm_x64, tm_h16, tm_h64;
+  if (!make_tmap_u8(&tm_c13, w13_codes, (uint64_t)E * 2 * I, (uint64_t)H / 2, 64)) return ELDR_ERR_CUDA;
+  if (!make_tmap_u8(&tm_c2, w2_codes, (uint64_t)E * H, (uint64_t)I / 2, 128)) return ELDR_ERR_CUDA;
+  if (!make_tmap(&tm_x16, x_perm, (uint64_t)x_rows, H, 16)) return ELDR_ERR_CUDA;
+  if (!make_tmap(&tm_x64, x_perm, (uint64_t)x_rows, H, 64)) return ELDR_ERR_CUDA;
+  if (!make_tmap(&tm_h16, hbuf, (uint64_t)x_rows, I, 16)) return ELDR_ERR_CUDA;
+  if (!make_tmap(&tm_h64, hbuf, (uint64_t)x_rows, I, 64)) return ELDR_ERR_CUDA;
+  const int sms = num_sms();
+  int g13 = max_work * m13.f.tiles_per_expert; if (g13 > sms) g13 = sms;
+  int g2 = max_work * m2.f.tiles_per_expert; if (g2 > sms) g2 = sms;
+  prof_mark(3, st);
+  launch_dep(ffn_mx_kernel<0>, dim3(g13), dim3(kMxThreads), smem, st, tm_c13, tm_x16, tm_x64, m13);
+  if (!launch_ok("ffn_mx_kernel<w13>")) return ELDR_ERR_CUDA;
+  prof_mark(4, st);
+  launch_dep(ffn_mx_kernel<1>, dim3(g2), dim3(kMxThreads), smem, st, tm_c2, tm_h16, tm_h64, m2);
+  if (!launch_ok("ffn_mx_kernel<w2>")) return ELDR_ERR_CUDA;
+  prof_mark(5, st);
+  launch_dep(k <= 8 ? combine_kernel<8> : combine_kernel<kMaxTopK>, dim3((T * (H / 4) + 255) / 256), dim3(256), 0, st,
+             ybuf, topk_w, pair_pos, out, T, H, k, 0);
   if (!launch_ok("combine_kernel")) return ELDR_ERR_CUDA;
   prof_mark(ELDR_PROFILE_SLOTS, st);
   return ELDR_OK;
