@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- the one measurement entry point: MoE-layer decode step time and achieved HBM bandwidth.
 
-  python bench.py [--config 2|3|4|5|prefill|route|mxfp4] [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+  python bench.py [--config 2|3|4|5|prefill|route|mxfp4|fit] [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
   python bench.py --timeline T:U[,U...]          in-kernel timeline of the fused step (markdown; -DELDR_TRACE build)
 
 A "step" is ONE layer-step = one eldr_moe_decode_layer call: gate GEMV -> softmax top-k + signature accumulation ->
@@ -19,7 +19,8 @@ the paper's models and prompts.
              single-cluster vs mixed batches; per-layer time, 48-layer stack time, realised unions.
   --config 5 27 layers x (64 routed top-6 + 2 shared experts), I = 1408, T = 256; plus the prefill-shaped signature
              accumulation (32 requests, prompts 512-4096, 16-token KV blocks).
-  --config prefill / route / mxfp4: the SURVEY.md 8(f) rows (prefill-shaped layer, routing decision, MXFP4 experts).
+  --config prefill / route / mxfp4 / fit: the SURVEY.md 8(f) rows (prefill-shaped layer, routing decision, MXFP4 experts,
+             offline fit -- the last one is host code and needs no GPU).
 N > 1: independent replicas, one per GPU (the path does not shard: SURVEY.md 8(e)), launched by torchrun.
 """
 from __future__ import annotations
@@ -760,13 +761,58 @@ def run_mxfp4(args):
                       "clocks": sampler.summary()}), flush=True)
 
 
+def run_fit(args):
+    """the offline fit at the paper's scale ("under 10 s on CPU"; 1,000 calibration
+    requests per cell): IDF -> greedy layer mask -> Eq. 2 signatures -> Hungarian-balanced K-means (K = 8).
+    Host code (the paper's is too); the oracle's K-means step (scipy Hungarian on duplicated slots) is timed beside it."""
+    from paper_2607_00466_b200 import api
+    api.load()
+    N, L, E, K, P = 1000, 48, 128, 8, 2000
+    g = np.random.default_rng(33)
+    informative = g.permutation(L)[: L // 2]
+    proto = np.full((8, L, E), 0.05)
+    for d in range(8):
+        for l in informative:
+            proto[d, l, g.permutation(E)[:4]] += 3.0
+    proto[:, :, 0] += 2.0
+    dom = g.integers(0, 8, size=N)
+    counts = np.empty((N, L, E), np.int32)
+    dec = np.empty((N, L, E))
+    for r in range(N):
+        p = proto[dom[r]] / proto[dom[r]].sum(axis=1, keepdims=True)
+        for l in range(L):
+            counts[r, l] = g.multinomial(64, p[l] if l in informative else np.full(E, 1.0 / E))
+        dec[r] = np.clip(p * 4 + 0.05 * g.random((L, E)), 0, 1)
+    pairs = g.integers(0, N, size=(P, 2)).astype(np.int32)
+    init = g.permutation(N)[:K].astype(np.int32)
+    t = {}
+    t0 = time.perf_counter(); idf = api.eldr_fit_idf(counts); t["idf_s"] = time.perf_counter() - t0
+    t0 = time.perf_counter(); order, cum, ns, mask = api.eldr_fit_layer_mask(counts, idf, dec, pairs); t["layer_mask_s"] = time.perf_counter() - t0
+    x = (counts * idf[None])[:, np.nonzero(mask)[0], :].reshape(N, -1)
+    sig = x / np.linalg.norm(x, axis=1, keepdims=True)
+    t0 = time.perf_counter(); cent, assign, steps, total = api.eldr_fit_kmeans_balanced(sig, K, init, 50); t["kmeans_s"] = time.perf_counter() - t0
+    sizes = np.bincount(assign, minlength=K).tolist()
+    purity = float(np.mean([np.bincount(dom[assign == k], minlength=8).max() / max(1, (assign == k).sum()) for k in range(K)]))
+    cpu = None
+    if not args.no_cpu_baseline:
+        from oracle import fit as ofit
+        t0 = time.perf_counter(); o_cent, o_assign, o_steps, o_total = ofit.kmeans_balanced(sig, K, init, 50); dt = time.perf_counter() - t0
+        cpu = {"value": round(dt, 3), "unit": "s", "cores": 1, "kind": "oracle", "sample": "the balanced K-means step only (same signatures, same seeds)",
+               "assignment_equal": bool(np.array_equal(assign, o_assign)), "steps": o_steps, "total_cost_diff": abs(total - o_total)}
+    print(json.dumps({"metric": "offline_fit_seconds", "value": round(sum(t.values()), 3), "unit": "s", "higher_is_better": False, "dtype": "f64",
+                      "data": "synthetic", "config": {"workload": "SURVEY.md 8(f) row 4: 1000 calibration requests, L=48, E=128, K=8 workers, 2000 pairs (host code)"},
+                      "stages_s": {k_: round(v, 4) for k_, v in t.items()}, "kept_layers": int(ns), "rho_at_peak": round(float(cum[ns - 1]), 4),
+                      "rho_all_layers": round(float(cum[-1]), 4), "kmeans_steps": steps, "cluster_sizes": sizes, "cluster_purity": round(purity, 3),
+                      "cpu_baseline": cpu, "paper_context": "balanced K-means re-fit under 10 s on CPU (PAPER.md:163)"}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="2", choices=["2", "3", "4", "5", "prefill", "route", "mxfp4"])
+    ap.add_argument("--config", default="2", choices=["2", "3", "4", "5", "prefill", "route", "mxfp4", "fit"])
     ap.add_argument("--unions", default="", help="config 2: subset of the union sizes, e.g. 16,128")
     ap.add_argument("--prefill-T", default="2048,4096,8192,16384")
     ap.add_argument("--timeline", default="", help="T:U[,U...]  e.g. 64:16,128 -- print the fused kernel's in-kernel timeline (markdown)")
@@ -795,6 +841,8 @@ def main():
         return run_prefill(args)
     if args.config == "mxfp4":
         return run_mxfp4(args)
+    if args.config == "fit":
+        return run_fit(args)
     run_ours(args, rank, local_rank, world)
 
 

@@ -193,6 +193,37 @@ int32_t eldr_route_decide(const eldr_moe_shape_t* shape, int32_t R, int32_t K, c
                           const float* idf, const uint8_t* layer_mask, const float* centroids, int32_t* loads,
                           float tau, int32_t* worker, float* sims, eldr_stream_t stream);
 
+/* ---- Offline fit.  HOST functions: every pointer is host memory, fp64, synchronous, no CUDA
+ * call -- the paper fits on the CPU before serving ("under 10 s on CPU").  Readings where the paper is
+ * silent: DESIGN.md 9d (the random calibration pairs and the initial centroids are inputs; average ranks for ties;
+ * cos-dist of a zero vector = 1; greedy ties -> lowest layer; N* = first maximum; centroid = renormalised mean, an
+ * empty centroid keeps its value).
+ *
+ * eldr_fit_idf: h_idf[l,e] = log((N+1) / (df(l,e)+1)), df = requests with h_counts[r,l,e] > 0.
+ *   h_counts [N,L,E] int32 in (per-request prefill counts c_r(l,e));  h_idf [L,E] double out.
+ * eldr_fit_layer_mask (Eq. 1 at :183): greedy layer selection on rho = Spearman(cos-dist of the signatures
+ *   restricted to the mask, cos-dist of the decode patterns) over the given request pairs.
+ *   h_decode_p [N,L,E] double in (decode-time activation probabilities p_i(l,e)); h_pairs [P,2] int32 in;
+ *   h_order [L] int32 out (layers in the order they were appended); h_cum_rho [L] double out (rho of each prefix);
+ *   h_n_star [1] out (prefix length at which rho peaks); h_mask [L] uint8 out (1 = kept: the first N* of the order).
+ * eldr_fit_balanced_assign: the assignment of N points to K centroids minimising the total cost with at
+ *   most `cap` points per centroid (K*cap >= N).  h_cost [N,K] double in; h_assign [N] int32 out; h_total [1] out or NULL.
+ * eldr_fit_kmeans_balanced: Hungarian-balanced spherical K-means, cap = ceil(N/K), cost = 1 - cosine.
+ *   h_sig [N,d] double in (unit rows: Eq. 2 signatures); h_init_idx [K] int32 in (requests whose signatures seed the
+ *   centroids); at most max_iter assignment steps, stops when the assignment repeats;
+ *   h_centroids [K,d] double out (unit rows); h_assign [N] int32 out; h_steps [1], h_total [1] out (assignment steps
+ *   run; total cosine distance of the final assignment to the centroids it was computed against).
+ * Errors: ELDR_ERR_INVALID_ARG for null pointers, non-positive sizes, K*cap < N, indices out of range. */
+int32_t eldr_fit_idf(const int32_t* h_counts, int32_t N, int32_t L, int32_t E, double* h_idf);
+int32_t eldr_fit_layer_mask(const int32_t* h_counts, const double* h_idf, const double* h_decode_p,
+                            int32_t N, int32_t L, int32_t E, const int32_t* h_pairs, int32_t P,
+                            int32_t* h_order, double* h_cum_rho, int32_t* h_n_star, uint8_t* h_mask);
+int32_t eldr_fit_balanced_assign(const double* h_cost, int32_t N, int32_t K, int32_t cap,
+                                 int32_t* h_assign, double* h_total);
+int32_t eldr_fit_kmeans_balanced(const double* h_sig, int32_t N, int32_t d, int32_t K,
+                                 const int32_t* h_init_idx, int32_t max_iter,
+                                 double* h_centroids, int32_t* h_assign, int32_t* h_steps, double* h_total);
+
 size_t  eldr_moe_workspace_bytes(const eldr_moe_shape_t* shape, int32_t max_T);
 size_t  eldr_moe_workspace_bytes_host(const eldr_moe_shape_t* shape, int32_t max_T);
 int32_t eldr_moe_workspace_layout(const eldr_moe_shape_t* shape, int32_t T, eldr_moe_ws_layout_t* layout);

@@ -23,6 +23,7 @@ EXPORTS = [
     "eldr_moe_workspace_bytes", "eldr_moe_workspace_bytes_host", "eldr_moe_workspace_layout",
     "eldr_moe_last_launch_count", "eldr_status_string", "eldr_last_cuda_error",
     "eldr_moe_profile_enable", "eldr_moe_profile_read", "eldr_moe_set_option",
+    "eldr_fit_idf", "eldr_fit_layer_mask", "eldr_fit_balanced_assign", "eldr_fit_kmeans_balanced",
 ]
 OPT_FFN_PATH, FFN_MMA_SYNC, FFN_TCGEN05 = 0, 0, 1
 OPT_PDL = 1
@@ -282,6 +283,55 @@ class DecodeLayer:
         off = getattr(L, name)
         n = int(np.prod(spec[1])) * torch.empty((), dtype=spec[0]).element_size()
         return self.workspace[off: off + n].view(spec[0]).view(spec[1])
+
+
+# ---- offline fit (host functions of the library: numpy arrays in, numpy arrays out; marshalling only) ----------------
+def _np(a, dtype):
+    a = np.ascontiguousarray(a, dtype=dtype)
+    return a, a.ctypes.data_as(C.c_void_p)
+
+
+def eldr_fit_idf(counts: np.ndarray) -> np.ndarray:
+    counts, pc = _np(counts, np.int32)
+    N, L, E = counts.shape
+    idf = np.empty((L, E), np.float64)
+    _check(load().eldr_fit_idf(pc, C.c_int32(N), C.c_int32(L), C.c_int32(E), idf.ctypes.data_as(C.c_void_p)), "eldr_fit_idf")
+    return idf
+
+
+def eldr_fit_layer_mask(counts, idf, decode_p, pairs):
+    counts, pc = _np(counts, np.int32)
+    idf, pi = _np(idf, np.float64)
+    decode_p, pd = _np(decode_p, np.float64)
+    pairs, pp = _np(pairs, np.int32)
+    N, L, E = counts.shape
+    order, cum = np.empty(L, np.int32), np.empty(L, np.float64)
+    n_star, mask = np.zeros(1, np.int32), np.empty(L, np.uint8)
+    _check(load().eldr_fit_layer_mask(pc, pi, pd, C.c_int32(N), C.c_int32(L), C.c_int32(E), pp, C.c_int32(len(pairs)),
+                                      order.ctypes.data_as(C.c_void_p), cum.ctypes.data_as(C.c_void_p),
+                                      n_star.ctypes.data_as(C.c_void_p), mask.ctypes.data_as(C.c_void_p)), "eldr_fit_layer_mask")
+    return order, cum, int(n_star[0]), mask
+
+
+def eldr_fit_balanced_assign(cost, cap: int):
+    cost, pc = _np(cost, np.float64)
+    N, K = cost.shape
+    assign, total = np.empty(N, np.int32), np.zeros(1, np.float64)
+    _check(load().eldr_fit_balanced_assign(pc, C.c_int32(N), C.c_int32(K), C.c_int32(cap), assign.ctypes.data_as(C.c_void_p),
+                                           total.ctypes.data_as(C.c_void_p)), "eldr_fit_balanced_assign")
+    return assign, float(total[0])
+
+
+def eldr_fit_kmeans_balanced(sig, K: int, init_idx, max_iter: int = 50):
+    sig, ps = _np(sig, np.float64)
+    init_idx, pi = _np(init_idx, np.int32)
+    N, d = sig.shape
+    cent, assign = np.empty((K, d), np.float64), np.empty(N, np.int32)
+    steps, total = np.zeros(1, np.int32), np.zeros(1, np.float64)
+    _check(load().eldr_fit_kmeans_balanced(ps, C.c_int32(N), C.c_int32(d), C.c_int32(K), pi, C.c_int32(max_iter),
+                                           cent.ctypes.data_as(C.c_void_p), assign.ctypes.data_as(C.c_void_p),
+                                           steps.ctypes.data_as(C.c_void_p), total.ctypes.data_as(C.c_void_p)), "eldr_fit_kmeans_balanced")
+    return cent, assign, int(steps[0]), float(total[0])
 
 
 class MxDecodeLayer:

@@ -14,6 +14,7 @@
 #include "ffn_umma.cuh"
 #include "ffn_umma2.cuh"
 #include "ffn_mx.cuh"
+#include "fit_host.cuh"
 #include "gate_route.cuh"
 #include "gate_prefill.cuh"
 #include "moe_fused.cuh"
@@ -1071,6 +1072,41 @@ int32_t eldr_route_decide(const eldr_moe_shape_t* s, int32_t R, int32_t K, const
   if (!launch_ok("route_sims_kernel")) return ELDR_ERR_CUDA;
   route_pick_kernel<<<1, kRoutePickThreads, 0, st>>>(sims, loads, worker, R, K, tau);
   return launch_ok("route_pick_kernel") ? ELDR_OK : ELDR_ERR_CUDA;
+}
+
+// ------------------------------------------------------------------------------- offline fit (host)
+int32_t eldr_fit_idf(const int32_t* h_counts, int32_t N, int32_t L, int32_t E, double* h_idf) {
+  if (!h_counts || !h_idf || N < 1 || L < 1 || E < 1) return ELDR_ERR_INVALID_ARG;
+  eldr_fit::idf_table(h_counts, N, L, E, h_idf);
+  return ELDR_OK;
+}
+
+int32_t eldr_fit_layer_mask(const int32_t* h_counts, const double* h_idf, const double* h_decode_p, int32_t N, int32_t L,
+                            int32_t E, const int32_t* h_pairs, int32_t P, int32_t* h_order, double* h_cum_rho,
+                            int32_t* h_n_star, uint8_t* h_mask) {
+  if (!h_counts || !h_idf || !h_decode_p || !h_pairs || !h_order || !h_cum_rho || !h_n_star || !h_mask) return ELDR_ERR_INVALID_ARG;
+  if (N < 2 || L < 1 || E < 1 || P < 2) return ELDR_ERR_INVALID_ARG;
+  for (int p = 0; p < 2 * P; ++p)
+    if (h_pairs[p] < 0 || h_pairs[p] >= N) return ELDR_ERR_INVALID_ARG;
+  eldr_fit::greedy_layer_mask(h_counts, h_idf, h_decode_p, N, L, E, h_pairs, P, h_order, h_cum_rho, h_n_star, h_mask);
+  return ELDR_OK;
+}
+
+int32_t eldr_fit_balanced_assign(const double* h_cost, int32_t N, int32_t K, int32_t cap, int32_t* h_assign, double* h_total) {
+  if (!h_cost || !h_assign || N < 1 || K < 1 || cap < 1 || (long long)K * cap < N) return ELDR_ERR_INVALID_ARG;
+  const double t = eldr_fit::balanced_assign(h_cost, N, K, cap, h_assign);
+  if (h_total) *h_total = t;
+  return ELDR_OK;
+}
+
+int32_t eldr_fit_kmeans_balanced(const double* h_sig, int32_t N, int32_t d, int32_t K, const int32_t* h_init_idx,
+                                 int32_t max_iter, double* h_centroids, int32_t* h_assign, int32_t* h_steps, double* h_total) {
+  if (!h_sig || !h_init_idx || !h_centroids || !h_assign || !h_steps || !h_total) return ELDR_ERR_INVALID_ARG;
+  if (N < 1 || d < 1 || K < 1 || K > N || max_iter < 1) return ELDR_ERR_INVALID_ARG;
+  for (int k = 0; k < K; ++k)
+    if (h_init_idx[k] < 0 || h_init_idx[k] >= N) return ELDR_ERR_INVALID_ARG;
+  eldr_fit::kmeans_balanced(h_sig, N, d, K, h_init_idx, max_iter, h_centroids, h_assign, h_steps, h_total);
+  return ELDR_OK;
 }
 
 }  // extern "C"
