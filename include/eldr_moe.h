@@ -166,6 +166,16 @@ int32_t eldr_signature_accumulate(const eldr_moe_shape_t* shape, int32_t layer, 
                                   const int32_t* token_block, int32_t* sig_req, int8_t* sig_block,
                                   eldr_stream_t stream);
 
+/* The same for n_layers consecutive layers in ONE launch (prefill-shaped capture: a prefill forward yields the picks of
+ * every layer; "in a single GPU pass", Table 1's scatter at PAPER.md:308 is the context figure).
+ *   topk_ids [n_layers, T, k] int32 (layer-major); rows layer0 .. layer0+n_layers-1 of the signature tensors are updated.
+ * Increments of a 256-token chunk are combined in shared memory before they reach the tables; results are identical
+ * to n_layers calls of eldr_signature_accumulate (integer adds commute; int8 cells saturate at 127). */
+int32_t eldr_signature_accumulate_layers(const eldr_moe_shape_t* shape, int32_t layer0, int32_t n_layers, int32_t T,
+                                         const int32_t* topk_ids, const int32_t* token_req,
+                                         const int32_t* token_block, int32_t* sig_req, int8_t* sig_block,
+                                         eldr_stream_t stream);
+
 /* PAPER.md:253 "a reused block resets its signature": zero the L*E cells of each listed row (ids < 0 skipped). */
 int32_t eldr_signature_reset_blocks(const eldr_moe_shape_t* shape, const int32_t* block_ids, int32_t n,
                                     int8_t* sig_block, eldr_stream_t stream);

@@ -19,7 +19,7 @@ _lib = None
 
 EXPORTS = [
     "eldr_moe_gate_topk", "eldr_moe_decode_layer", "eldr_moe_decode_layer_host", "eldr_moe_decode_layer_mxfp4",
-    "eldr_signature_accumulate", "eldr_signature_reset_blocks", "eldr_signature_readout", "eldr_route_decide",
+    "eldr_signature_accumulate", "eldr_signature_accumulate_layers", "eldr_signature_reset_blocks", "eldr_signature_readout", "eldr_route_decide",
     "eldr_moe_workspace_bytes", "eldr_moe_workspace_bytes_host", "eldr_moe_workspace_layout",
     "eldr_moe_last_launch_count", "eldr_status_string", "eldr_last_cuda_error",
     "eldr_moe_profile_enable", "eldr_moe_profile_read", "eldr_moe_set_option",
@@ -216,6 +216,16 @@ def eldr_signature_accumulate(shape, layer: int, topk_ids, token_req, token_bloc
         C.byref(s), C.c_int32(layer), C.c_int32(T), _ptr(topk_ids, torch.int32), _ptr(token_req, torch.int32),
         _ptr(token_block, torch.int32), _ptr(sig_req, torch.int32), _ptr(sig_block, torch.int8), _stream()),
         "eldr_signature_accumulate")
+
+
+def eldr_signature_accumulate_layers(shape, topk_ids, token_req, token_block, sig_req, sig_block, layer0: int = 0):
+    """topk_ids [n_layers, T, k]: all layers of a prefill-shaped capture in one launch."""
+    s = make_shape(shape)
+    n_layers, T = topk_ids.shape[0], topk_ids.shape[1]
+    _check(load().eldr_signature_accumulate_layers(
+        C.byref(s), C.c_int32(layer0), C.c_int32(n_layers), C.c_int32(T), _ptr(topk_ids, torch.int32),
+        _ptr(token_req, torch.int32), _ptr(token_block, torch.int32), _ptr(sig_req, torch.int32),
+        _ptr(sig_block, torch.int8), _stream()), "eldr_signature_accumulate_layers")
 
 
 def eldr_signature_reset_blocks(shape, block_ids, sig_block):

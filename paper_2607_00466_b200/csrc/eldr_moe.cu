@@ -138,7 +138,7 @@ void make_host_stage(const eldr_moe_shape_t* s, int T, size_t base, HostStage* S
 // grid are properties of the device the call runs on, so everything cached here is keyed by the device ordinal.
 constexpr int kMaxDevices = 64;
 enum { kAttrFused = 0, kAttrRouteBig, kAttrUmma, kAttrPair, kAttrStream, kAttrRouteSims, kAttrGateLogits, kAttrGateRoute,
-       kAttrRouteOnly, kAttrMx, kAttrCount };
+       kAttrRouteOnly, kAttrMx, kAttrSigLayers, kAttrCount };
 struct DevState {
   std::atomic<int> sms{0};
   std::atomic<int> fused_ok{-1};          // -1 unknown, 0 the persistent grid cannot be co-resident, 1 it can
@@ -1028,6 +1028,23 @@ int32_t eldr_signature_accumulate(const eldr_moe_shape_t* s, int32_t layer, int3
   return launch_ok("sig_accumulate_kernel") ? ELDR_OK : ELDR_ERR_CUDA;
 }
 
+int32_t eldr_signature_accumulate_layers(const eldr_moe_shape_t* s, int32_t layer0, int32_t n_layers, int32_t T,
+                                         const int32_t* topk_ids, const int32_t* token_req, const int32_t* token_block,
+                                         int32_t* sig_req, int8_t* sig_block, eldr_stream_t stream) {
+  g_launches = 0;
+  int32_t rc = check_shape(s);
+  if (rc != ELDR_OK) return rc;
+  if (T < 0 || n_layers < 0 || layer0 < 0 || layer0 + n_layers > s->n_layers) return ELDR_ERR_INVALID_ARG;
+  if (T == 0 || n_layers == 0) return ELDR_OK;
+  if (!topk_ids || !aligned16(sig_block)) return ELDR_ERR_INVALID_ARG;
+  const int E = s->n_experts;
+  const size_t smem = (size_t)E * 4 + (size_t)(kSigChunk + 4) * ((E + 3) / 4) * 4;
+  if (smem > 48 * 1024 && !once_per_device(kAttrSigLayers, [] { return set_smem(sig_accumulate_layers_kernel, 100 * 1024); })) return ELDR_ERR_CUDA;
+  sig_accumulate_layers_kernel<<<dim3((T + kSigChunk - 1) / kSigChunk, n_layers), 256, smem, static_cast<cudaStream_t>(stream)>>>(
+      topk_ids, token_req, token_block, sig_req, sig_block, T, E, s->top_k, s->n_layers, layer0);
+  return launch_ok("sig_accumulate_layers_kernel") ? ELDR_OK : ELDR_ERR_CUDA;
+}
+
 int32_t eldr_signature_reset_blocks(const eldr_moe_shape_t* s, const int32_t* block_ids, int32_t n,
                                     int8_t* sig_block, eldr_stream_t stream) {
   g_launches = 0;
@@ -1050,7 +1067,9 @@ int32_t eldr_signature_readout(const eldr_moe_shape_t* s, const int32_t* block_i
   if (n_req == 0) return ELDR_OK;
   if (!block_ids || !req_off || !sig_block || !sig_out) return ELDR_ERR_INVALID_ARG;
   const int cells = s->n_layers * s->n_experts;
-  dim3 grid((cells + 255) / 256 < 64 ? (cells + 255) / 256 : 64, n_req);
+  const int per_thread = (cells % 16 == 0) ? 16 : 1;
+  const int want = (cells / per_thread + 255) / 256;
+  dim3 grid(want < 64 ? (want > 0 ? want : 1) : 64, n_req);
   sig_readout_kernel<<<grid, 256, 0, static_cast<cudaStream_t>(stream)>>>(block_ids, req_off, sig_block, sig_out,
                                                                        cells);
   return launch_ok("sig_readout_kernel") ? ELDR_OK : ELDR_ERR_CUDA;

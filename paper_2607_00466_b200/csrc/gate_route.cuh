@@ -508,6 +508,89 @@ __global__ void __launch_bounds__(256) sig_accumulate_kernel(const int32_t* __re
   sig_add(sig_req, sig_block, token_req ? token_req[t] : -1, token_block ? token_block[t] : -1, L, layer, E, e);
 }
 
+// All layers of a prefill-shaped call in ONE launch ("Each forward accumulates the new tokens' expert picks
+// into the matching rows in a single GPU pass"): grid (token chunks of 256, layers).  A chunk's increments are first
+// combined in shared memory -- the request histogram when all 256 tokens belong to one request (the prefill case), the
+// KV-block rows per run of equal block ids (a new run at least every 64 tokens, so a byte cell cannot overflow) -- and
+// only the non-zero cells / words go to global memory: ~10x fewer global atomics than one per pick.  Decode-shaped
+// chunks (every token its own request) take the direct path for the request table.  Same saturating int8 semantics.
+constexpr int kSigChunk = 256;
+__global__ void __launch_bounds__(256) sig_accumulate_layers_kernel(const int32_t* __restrict__ ids_all,
+                                                                    const int32_t* __restrict__ token_req,
+                                                                    const int32_t* __restrict__ token_block,
+                                                                    int32_t* sig_req, int8_t* sig_block, int T, int E,
+                                                                    int k, int L, int layer0) {
+  extern __shared__ __align__(16) uint8_t sig_smem[];
+  const int EW = (E + 3) >> 2;                                  // 32-bit words per block row
+  int32_t* rhist = reinterpret_cast<int32_t*>(sig_smem);        // [E]
+  uint32_t* bhist = reinterpret_cast<uint32_t*>(rhist + E);     // [kSigChunk + 4][EW] packed byte counts per run
+  __shared__ int s_slot_of[kSigChunk];
+  __shared__ int s_run_blk[kSigChunk + 4];
+  __shared__ int s_warp_tot[8];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int t0 = blockIdx.x * kSigChunk, layer = layer0 + blockIdx.y;
+  const int n_tok = min(kSigChunk, T - t0);
+  const int32_t* ids = ids_all + (size_t)blockIdx.y * T * k;
+  const int t = t0 + tid;
+  const int my_req = (tid < n_tok && token_req) ? token_req[t] : -1;
+  const int my_blk = (tid < n_tok && token_block) ? token_block[t] : -1;
+  const int req0 = token_req ? token_req[t0] : -1;
+  const bool uniform = __syncthreads_and(tid >= n_tok || my_req == req0) && sig_req != nullptr && req0 >= 0;
+  // runs of equal block ids -> slots (block scan of the run heads)
+  int prev_blk = -2;
+  if (tid > 0 && tid < n_tok && token_block) prev_blk = token_block[t - 1];
+  const int head = (tid < n_tok) && (tid == 0 || my_blk != prev_blk || (tid & 63) == 0);
+  const uint32_t hb = __ballot_sync(0xffffffffu, head);
+  if (lane == 0) s_warp_tot[warp] = __popc(hb);
+  for (int i = tid; i < E; i += 256) rhist[i] = 0;
+  for (int i = tid; i < (kSigChunk + 4) * EW; i += 256) bhist[i] = 0u;
+  __syncthreads();
+  int base = 0, n_runs = 0;
+#pragma unroll
+  for (int w = 0; w < 8; ++w) { if (w < warp) base += s_warp_tot[w]; n_runs += s_warp_tot[w]; }
+  const int slot = base + __popc(hb & ((2u << lane) - 1u)) - 1;
+  if (tid < n_tok) s_slot_of[tid] = slot;
+  if (head) s_run_blk[slot] = my_blk;
+  __syncthreads();
+  const bool do_blk = sig_block != nullptr;
+  for (int p = tid; p < n_tok * k; p += 256) {
+    const int tl = p / k;
+    const int e = ids[(size_t)t0 * k + p];
+    if (e < 0 || e >= E) continue;
+    const int rq = token_req ? token_req[t0 + tl] : -1;
+    if (uniform) atomicAdd(&rhist[e], 1);
+    else if (sig_req != nullptr && rq >= 0) atomicAdd(sig_req + ((size_t)rq * L + layer) * E + e, 1);
+    if (do_blk && s_run_blk[s_slot_of[tl]] >= 0) atomicAdd(&bhist[s_slot_of[tl] * EW + (e >> 2)], 1u << (8 * (e & 3)));
+  }
+  __syncthreads();
+  if (uniform)
+    for (int e = tid; e < E; e += 256)
+      if (rhist[e]) atomicAdd(sig_req + ((size_t)req0 * L + layer) * E + e, rhist[e]);
+  if (do_blk) {
+    const bool word_ok = (E & 3) == 0;            // rows are whole 32-bit words (and 4-byte aligned: L*E*blk multiple of 4)
+    for (int i = tid; i < n_runs * EW; i += 256) {
+      const uint32_t add = bhist[i];
+      if (!add) continue;
+      const int r = i / EW, wd = i - r * EW;
+      const size_t cell0 = ((size_t)s_run_blk[r] * L + layer) * E + (size_t)wd * 4;
+      if (word_ok) {
+        unsigned int* word = reinterpret_cast<unsigned int*>(sig_block + cell0);
+        const unsigned int old = atomicAdd(word, add);
+        unsigned int undo = 0u;
+#pragma unroll
+        for (int b = 0; b < 4; ++b) {
+          const unsigned int ob = (old >> (8 * b)) & 0xffu, c = (add >> (8 * b)) & 0xffu;
+          if (c && ob + c > 127u) undo |= (ob + c - max(ob, 127u)) << (8 * b);
+        }
+        if (undo) atomicSub(word, undo);
+      } else {
+        for (int b = 0; b < 4 && wd * 4 + b < E; ++b)
+          for (unsigned int c = (add >> (8 * b)) & 0xffu; c > 0; --c) sig_add(nullptr, sig_block, -1, s_run_blk[r], L, layer, E, wd * 4 + b);
+      }
+    }
+  }
+}
+
 __global__ void __launch_bounds__(256) sig_reset_kernel(const int32_t* __restrict__ block_ids, int8_t* sig_block,
                                                         int row_bytes) {
   const int b = block_ids[blockIdx.x];
@@ -526,6 +609,32 @@ __global__ void __launch_bounds__(256) sig_readout_kernel(const int32_t* __restr
                                                           int32_t* __restrict__ sig_out, int row_cells) {
   const int r = blockIdx.y;
   const int b0 = req_off[r], b1 = req_off[r + 1];
+  if ((row_cells & 15) == 0) {
+    // 16 cells per thread: one 16-byte load per block row, four rows in flight (a request sums 32-256 rows)
+    for (int c16 = blockIdx.x * 256 + threadIdx.x; c16 < (row_cells >> 4); c16 += gridDim.x * 256) {
+      int acc[16];
+#pragma unroll
+      for (int j = 0; j < 16; ++j) acc[j] = 0;
+      for (int i = b0; i < b1; i += 4) {
+        uint4 v[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int b = (i + u < b1) ? block_ids[i + u] : -1;
+          v[u] = b >= 0 ? ld_nc_v4(sig_block + (size_t)b * row_cells + (size_t)c16 * 16) : make_uint4(0u, 0u, 0u, 0u);
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const uint32_t wv[4] = {v[u].x, v[u].y, v[u].z, v[u].w};
+#pragma unroll
+          for (int j = 0; j < 16; ++j) acc[j] += (int)(int8_t)((wv[j >> 2] >> (8 * (j & 3))) & 0xffu);
+        }
+      }
+      int4* dst = reinterpret_cast<int4*>(sig_out + (size_t)r * row_cells + (size_t)c16 * 16);
+#pragma unroll
+      for (int q = 0; q < 4; ++q) dst[q] = make_int4(acc[4 * q], acc[4 * q + 1], acc[4 * q + 2], acc[4 * q + 3]);
+    }
+    return;
+  }
   for (int c = blockIdx.x * 256 + threadIdx.x; c < row_cells; c += gridDim.x * 256) {
     int acc = 0;
     for (int i = b0; i < b1; ++i) {

@@ -837,3 +837,48 @@ def test_two_layers_on_two_streams_match_serial_results(gpu, oracle):
     for i in range(2):
         for o in outs[i]:
             assert torch.equal(o.view(torch.int16), ref[i].view(torch.int16))
+
+
+@pytest.mark.parametrize("E,k,T,shaped", [(64, 6, 3000, "prefill"), (64, 6, 700, "decode"), (10, 3, 530, "prefill"), (130, 4, 257, "mixed")])
+def test_signature_accumulate_layers_one_launch(gpu, oracle, E, k, T, shaped):
+    """eldr_signature_accumulate_layers (all layers in one launch, chunk-level combining in shared memory) equals the
+    oracle's serial loop bit for bit: prefill-shaped maps (long runs of one request, 16-token KV blocks, non-contiguous
+    block ids, padding tokens), decode-shaped maps (every token its own request and block), E not a multiple of 4
+    (byte path), and a block that receives more than 127 picks of one expert (saturation)."""
+    import torch
+    L = 5
+    shape = synth.MoEShape(hidden=64, inter=64, n_experts=E, top_k=k, n_layers=L + 2, kv_block_size=16)
+    rng = np.random.default_rng(E * 1000 + T)
+    ids = np.stack([np.stack([rng.choice(E, size=k, replace=False) for _ in range(T)]) for _ in range(L)]).astype(np.int32)
+    if shaped == "prefill":
+        lens = []
+        while sum(lens) < T:
+            lens.append(int(rng.integers(100, 900)))
+        token_req = np.repeat(np.arange(len(lens)), lens)[:T].astype(np.int32)
+        blk_perm = rng.permutation(T // 16 + 40).astype(np.int32)
+        token_block = blk_perm[np.arange(T) // 16]
+        token_req[::97] = -1
+        token_block[5::131] = -1
+    elif shaped == "decode":
+        token_req = rng.permutation(T).astype(np.int32)
+        token_block = rng.permutation(T).astype(np.int32)
+    else:
+        token_req = (np.arange(T) // 40).astype(np.int32)
+        token_block = np.zeros(T, np.int32)              # one block takes every token: its cells saturate
+        ids[:, :, 0] = 7
+        ids[:, :, 1:] = np.stack([np.stack([rng.choice(np.arange(8, E), size=k - 1, replace=False) for _ in range(T)]) for _ in range(L)])
+    n_req, n_blk = int(token_req.max()) + 1, int(token_block.max()) + 1
+    sig_req = torch.zeros((n_req, L + 2, E), dtype=torch.int32, device="cuda")
+    sig_blk = torch.zeros((n_blk, L + 2, E), dtype=torch.int8, device="cuda")
+    gpu.eldr_signature_accumulate_layers(shape, torch.from_numpy(ids).cuda(), torch.from_numpy(token_req).cuda(),
+                                         torch.from_numpy(token_block).cuda(), sig_req, sig_blk, layer0=1)
+    torch.cuda.synchronize()
+    assert gpu.eldr_moe_last_launch_count() == 1
+    o_req = np.zeros((n_req, L + 2, E), np.int32)
+    o_blk = np.zeros((n_blk, L + 2, E), np.int8)
+    for l in range(L):
+        oracle.signature_accumulate(shape, 1 + l, ids[l], token_req, token_block, o_req, o_blk)
+    assert np.array_equal(sig_req.cpu().numpy(), o_req)
+    assert np.array_equal(sig_blk.cpu().numpy(), o_blk)
+    if shaped == "mixed":
+        assert o_blk[0, 1, 7] == 127 and o_blk[0, 0].max() == 0
