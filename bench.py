@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- the one measurement entry point: MoE-layer decode step time and achieved HBM bandwidth.
 
-  python bench.py [--config 2|3|4|5|prefill|route|mxfp4|fit] [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+  python bench.py [--config 2|3|4|5|prefill|route|mxfp4|fit|gemv] [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
   python bench.py --timeline T:U[,U...]          in-kernel timeline of the fused step (markdown; -DELDR_TRACE build)
 
 A "step" is ONE layer-step = one eldr_moe_decode_layer call: gate GEMV -> softmax top-k + signature accumulation ->
@@ -761,6 +761,65 @@ def run_mxfp4(args):
                       "clocks": sampler.summary()}), flush=True)
 
 
+def run_gemv(args):
+    """north_star: "Tensor cores ... only where tokens-per-expert fill a tile, with a CUDA-core GEMV path otherwise".  The
+    comparison that decides the default: FFN kernel times (CUDA events around each launch of the staged step) of the
+    tcgen05 swap-AB kernels and of the CUDA-core GEMV kernels (ELDR_OPT_FFN_PATH) at 1..8 tokens per expert, Qwen3-shaped
+    layer, plus the fused step.  Forced routing: T tokens share one set of experts so that m = T exactly."""
+    import torch
+    from paper_2607_00466_b200 import api, synth
+    api.load()
+    shape = synth.SHAPE_QWEN
+    lw = synth.make_layer_weights(shape, synth.WEIGHT_SEED)
+    dl = api.DecodeLayer(shape, lw, max_T=128)
+    copies = [(dl.w13, dl.w2)] + [(dl.w13.clone(), dl.w2.clone()) for _ in range(N_COPIES - 1)]
+    rows = []
+    for m, n_exp in ((1, 8), (1, 32), (2, 32), (4, 32), (8, 32), (8, 128)):
+        # m tokens per expert on n_exp experts: T = m * n_exp / k tokens, token t takes experts (t // m) * k .. + k - 1
+        k = shape.top_k
+        T = m * n_exp // k
+        ids = np.stack([((t // m) * k + np.arange(k)) % shape.n_experts for t in range(T)]).astype(np.int32)
+        x = api.bf16_from_bits(synth.make_hidden(T, shape.hidden, 300 + T))
+        row = {"tokens_per_expert": m, "experts": n_exp, "T": T}
+        for name, step_path, ffn in (("tcgen05_staged", api.STEP_STAGED, api.FFN_TCGEN05), ("gemv_staged", api.STEP_STAGED, api.FFN_GEMV),
+                                     ("fused", api.STEP_FUSED, api.FFN_TCGEN05)):
+            api.eldr_moe_set_option(api.OPT_STEP_PATH, step_path)
+            api.eldr_moe_set_option(api.OPT_FFN_PATH, ffn)
+            n = [0]
+
+            def step():
+                dl.w13, dl.w2 = copies[n[0] % N_COPIES]
+                n[0] += 1
+                dl.ids[:T].copy_(torch.from_numpy(ids))
+                dl.w[:T].fill_(1.0 / k)
+                dl.run(x, None, force_routing=1)
+            for _ in range(5):
+                step()
+            outs = dl.out[:T].clone()
+            api.eldr_moe_profile_enable(True)
+            acc = {}
+            for _ in range(args.steps):
+                step()
+                for kk, v in api.eldr_moe_profile_read().items():
+                    acc[kk] = acc.get(kk, 0.0) + v * 1e3 / args.steps
+            api.eldr_moe_profile_enable(False)
+            assert int(dl.n_active.item()) == n_exp
+            if name == "fused":
+                row["fused_step_us"] = round(acc["gate"], 2)
+            else:
+                row[name + "_w13_us"], row[name + "_w2_us"] = round(acc["ffn13"], 2), round(acc["ffn2"], 2)
+                row[name + "_w13_GBps"] = round(n_exp * 2 * shape.hidden * shape.inter * 2 / acc["ffn13"] / 1e3)
+            row.setdefault("_ref", outs)
+            assert (outs.float() - row["_ref"].float()).abs().max().item() <= 2e-2 * row["_ref"].float().abs().max().item() + 1e-6
+        row.pop("_ref")
+        rows.append(row)
+    api.eldr_moe_set_option(api.OPT_STEP_PATH, api.STEP_AUTO)
+    api.eldr_moe_set_option(api.OPT_FFN_PATH, api.FFN_TCGEN05)
+    print(json.dumps({"metric": "ffn_kernel_us_gemv_vs_tcgen05", "unit": "us", "value": rows[0]["gemv_staged_w13_us"], "higher_is_better": False,
+                      "config": {"workload": "Qwen3-30B-A3B-shaped layer, forced routing, m tokens per expert on n experts; per-launch CUDA events"},
+                      "rows": rows}), flush=True)
+
+
 def run_fit(args):
     """the offline fit at the paper's scale ("under 10 s on CPU"; 1,000 calibration
     requests per cell): IDF -> greedy layer mask -> Eq. 2 signatures -> Hungarian-balanced K-means (K = 8).
@@ -812,7 +871,7 @@ def main():
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="2", choices=["2", "3", "4", "5", "prefill", "route", "mxfp4", "fit"])
+    ap.add_argument("--config", default="2", choices=["2", "3", "4", "5", "prefill", "route", "mxfp4", "fit", "gemv"])
     ap.add_argument("--unions", default="", help="config 2: subset of the union sizes, e.g. 16,128")
     ap.add_argument("--prefill-T", default="2048,4096,8192,16384")
     ap.add_argument("--timeline", default="", help="T:U[,U...]  e.g. 64:16,128 -- print the fused kernel's in-kernel timeline (markdown)")
@@ -843,6 +902,8 @@ def main():
         return run_mxfp4(args)
     if args.config == "fit":
         return run_fit(args)
+    if args.config == "gemv":
+        return run_gemv(args)
     run_ours(args, rank, local_rank, world)
 
 

@@ -239,7 +239,8 @@ size_t  eldr_moe_workspace_bytes_host(const eldr_moe_shape_t* shape, int32_t max
 int32_t eldr_moe_workspace_layout(const eldr_moe_shape_t* shape, int32_t T, eldr_moe_ws_layout_t* layout);
 
 /* Process-wide tuning knobs (defaults are the fast settings; used by tests and profiles to compare paths).
- *   ELDR_OPT_FFN_PATH: ELDR_FFN_TCGEN05 (default; tcgen05.mma + TMEM) or ELDR_FFN_MMA_SYNC (legacy mma.sync). */
+ *   ELDR_OPT_FFN_PATH: ELDR_FFN_TCGEN05 (default; tcgen05.mma + TMEM), ELDR_FFN_MMA_SYNC (legacy mma.sync) or ELDR_FFN_GEMV
+ *   (CUDA-core GEMV, 8 tokens per pass: the comparison path for tiny tokens-per-expert counts; staged launches). */
 #define ELDR_OPT_FFN_PATH 0
 #define ELDR_OPT_PDL      1   /* 1 (default): programmatic dependent launch between the step's kernels; 0: plain */
 #define ELDR_OPT_STEP_PATH 2  /* ELDR_STEP_FUSED: the whole step in ONE persistent launch (T <= 256, H,I % 64 == 0);
@@ -271,6 +272,7 @@ int32_t eldr_moe_workspace_layout(const eldr_moe_shape_t* shape, int32_t T, eldr
 #define ELDR_STEP_AUTO    2
 #define ELDR_FFN_MMA_SYNC 0
 #define ELDR_FFN_TCGEN05  1
+#define ELDR_FFN_GEMV     2
 int32_t eldr_moe_set_option(int32_t key, int32_t value);
 
 /* Per-kernel device timing of eldr_moe_decode_layer (measurement aid, off by default, per host thread).

@@ -25,7 +25,7 @@ EXPORTS = [
     "eldr_moe_profile_enable", "eldr_moe_profile_read", "eldr_moe_set_option",
     "eldr_fit_idf", "eldr_fit_layer_mask", "eldr_fit_balanced_assign", "eldr_fit_kmeans_balanced",
 ]
-OPT_FFN_PATH, FFN_MMA_SYNC, FFN_TCGEN05 = 0, 0, 1
+OPT_FFN_PATH, FFN_MMA_SYNC, FFN_TCGEN05, FFN_GEMV = 0, 0, 1, 2
 OPT_PDL = 1
 OPT_STEP_PATH, STEP_STAGED, STEP_FUSED, STEP_AUTO = 2, 0, 1, 2
 OPT_RING_KB = 3

@@ -14,6 +14,7 @@
 #include "ffn_umma.cuh"
 #include "ffn_umma2.cuh"
 #include "ffn_mx.cuh"
+#include "ffn_gemv.cuh"
 #include "fit_host.cuh"
 #include "gate_route.cuh"
 #include "gate_prefill.cuh"
@@ -138,7 +139,7 @@ void make_host_stage(const eldr_moe_shape_t* s, int T, size_t base, HostStage* S
 // grid are properties of the device the call runs on, so everything cached here is keyed by the device ordinal.
 constexpr int kMaxDevices = 64;
 enum { kAttrFused = 0, kAttrRouteBig, kAttrUmma, kAttrPair, kAttrStream, kAttrRouteSims, kAttrGateLogits, kAttrGateRoute,
-       kAttrRouteOnly, kAttrMx, kAttrSigLayers, kAttrCount };
+       kAttrRouteOnly, kAttrMx, kAttrSigLayers, kAttrGemv, kAttrCount };
 struct DevState {
   std::atomic<int> sms{0};
   std::atomic<int> fused_ok{-1};          // -1 unknown, 0 the persistent grid cannot be co-resident, 1 it can
@@ -436,7 +437,7 @@ const char* eldr_status_string(int32_t st) {
 const char* eldr_last_cuda_error(void) { return g_err; }
 
 int32_t eldr_moe_set_option(int32_t key, int32_t value) {
-  if (key == ELDR_OPT_FFN_PATH && (value == ELDR_FFN_MMA_SYNC || value == ELDR_FFN_TCGEN05)) {
+  if (key == ELDR_OPT_FFN_PATH && (value == ELDR_FFN_MMA_SYNC || value == ELDR_FFN_TCGEN05 || value == ELDR_FFN_GEMV)) {
     g_ffn_path = value;
     return ELDR_OK;
   }
@@ -730,7 +731,22 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
   const int sms = num_sms();
   int g13 = max_work * f13.tiles_per_expert; if (g13 > sms) g13 = sms;
   int g2 = max_work * f2.tiles_per_expert; if (g2 > sms) g2 = sms;
-  if (H % 64 == 0 && I % 64 == 0 && ffn_path == ELDR_FFN_TCGEN05) {
+  if (ffn_path == ELDR_FFN_GEMV) {
+    // CUDA-core GEMV path (comparison path for tiny tokens-per-expert counts: profiles/r2_gemv_vs_tcgen05.md)
+    const size_t smem13 = (size_t)kGemvTok * H * 2, smem2 = (size_t)kGemvTok * I * 2;
+    if (smem13 > 200 * 1024 || smem2 > 200 * 1024) return ELDR_ERR_UNSUPPORTED;
+    if ((smem13 > 48 * 1024 || smem2 > 48 * 1024) && !once_per_device(kAttrGemv, [] {
+          return set_smem(ffn_gemv_kernel<0>, 200 * 1024) && set_smem(ffn_gemv_kernel<1>, 200 * 1024);
+        })) return ELDR_ERR_CUDA;
+    f13.tiles_per_expert = (I + 63) / 64;
+    g13 = max_work * f13.tiles_per_expert; if (g13 > sms) g13 = sms;
+    prof_mark(3, st);
+    launch_dep(ffn_gemv_kernel<0>, dim3(g13), dim3(kGemvThreads), smem13, st, w13, shared_w13, x_perm, f13);
+    if (!launch_ok("ffn_gemv_kernel<w13>")) return ELDR_ERR_CUDA;
+    prof_mark(4, st);
+    launch_dep(ffn_gemv_kernel<1>, dim3(g2), dim3(kGemvThreads), smem2, st, w2, shared_w2, hbuf, f2);
+    if (!launch_ok("ffn_gemv_kernel<w2>")) return ELDR_ERR_CUDA;
+  } else if (H % 64 == 0 && I % 64 == 0 && ffn_path == ELDR_FFN_TCGEN05) {
     // tcgen05 + TMEM path: weights are the M=128 operand, the expert's tokens the N operand
     CUtensorMap tm_w13, tm_sw13, tm_x16, tm_x64, tm_w2, tm_sw2, tm_h16, tm_h64;
     if (!make_tmap_w13_5d(&tm_w13, w13, E, I, H)) return ELDR_ERR_CUDA;

@@ -429,9 +429,9 @@ def test_host_buffer_entry_point_matches_device_entry_point(gpu):
     assert int(h_na.item()) == int(dl.n_active.item())
 
 
-@pytest.mark.parametrize("step_path,ffn_path,pdl", [(1, 1, 0), (0, 1, 1), (0, 0, 1), (0, 1, 0), (0, 0, 0), (1, 1, 1)])
+@pytest.mark.parametrize("step_path,ffn_path,pdl", [(1, 1, 0), (0, 1, 1), (0, 0, 1), (0, 1, 0), (0, 0, 0), (1, 1, 1), (0, 2, 1), (2, 2, 0)])
 def test_alternate_paths_match_oracle(gpu, oracle, step_path, ffn_path, pdl):
-    """The selectable paths (one persistent launch vs one launch per stage, legacy mma.sync FFN, launches without
+    """The selectable paths (one persistent launch vs one launch per stage, legacy mma.sync FFN, CUDA-core GEMV FFN, launches without
     programmatic dependent launch) must pass the same parity gates, including multi-pass experts (m > 64) and
     shared experts.  Consecutive cases reuse the same workspace memory, so this also checks that the epoch flags
     of one path never confuse the other."""
