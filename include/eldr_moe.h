@@ -263,6 +263,12 @@ int32_t eldr_moe_workspace_layout(const eldr_moe_shape_t* shape, int32_t T, eldr
                                  green-context SM partitions; a grid that cannot fit returns to the staged path).  Measured on
                                  B200 the driver does not overlap a cooperative launch with its predecessor (PDL has no effect):
                                  +2.5 us per step.  0 = plain launch + PDL, for a GPU the process has to itself */
+#define ELDR_OPT_HEAD_FIRST 8 /* fused step, static (stream-K) ranges: 0 (default) = ascending order, a split tile is finished by the
+                                 owner of its first stage; 1 = a CTA first computes and parks the head of the tile its range
+                                 ends in, then finishes the tile its range starts in with the previous CTA's parked head, then
+                                 streams its whole tiles (every range ends without a fix-up).  Measured on B200: 1 is SLOWER
+                                 (|U| = 16: 66.6 vs 61.2 us, 32: 82.2 vs 76.4) -- the early fix-up waits for a partner whose
+                                 head piece is longer than ours while the ring is still filling */
 #define ELDR_OPT_FFN_PAIR 5   /* prefill-shaped calls (T > 1024, I % 128 == 0, H % 256 == 0): the expert FFN as tcgen05
                                  cta_group::2 tiles (M = 256 over an SM pair, ffn_umma2.cuh).  1 (default): when the call
                                  has >= 256 tokens per expert on average (T*k >= 256*E); 2: always; 0: never (one CTA

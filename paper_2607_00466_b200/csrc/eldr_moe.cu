@@ -36,6 +36,7 @@ std::atomic<int> g_ring_kb{208};
 std::atomic<int> g_dp_min_rounds{4};
 std::atomic<int> g_sk_split_pct{0};
 std::atomic<int> g_coop{1};
+std::atomic<int> g_head_first{0};
 
 thread_local char g_err[256] = "";
 thread_local int g_launches = 0;
@@ -461,6 +462,10 @@ int32_t eldr_moe_set_option(int32_t key, int32_t value) {
     g_dp_min_rounds = value;
     return ELDR_OK;
   }
+  if (key == ELDR_OPT_HEAD_FIRST && (value == 0 || value == 1)) {
+    g_head_first = value;
+    return ELDR_OK;
+  }
   if (key == ELDR_OPT_COOPERATIVE && (value == 0 || value == 1)) {
     g_coop = value;
     return ELDR_OK;
@@ -601,6 +606,7 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
     fa.ring_bytes = g_ring_kb.load() * 1024;
     fa.dp_min_rounds = g_dp_min_rounds.load();
     fa.sk_split_pct = g_sk_split_pct.load();
+    fa.head_first = g_head_first.load();
     const size_t smem = fixed + fa.stage_area;
     if ((size_t)fa.stage_area >= min_area) {
       CUtensorMap tm_w13, tm_sw13, tm_w2, tm_sw2, tm_x, tm_h;

@@ -108,6 +108,7 @@ struct FusedArgs {
   int ring_bytes;              // cap on the bytes the ring keeps in flight (<= stage_area)
   int dp_min_rounds;           // hybrid schedule: data-parallel part only if a phase has at least this many tile rounds
   int sk_split_pct;            // small unions (whole phase stream-K): share of the accumulator passes in the first expert group
+  int head_first;              // static ranges: head piece first and parked, split tiles finished by the owner of their last stage
 };
 
 #ifdef ELDR_TRACE
@@ -571,14 +572,17 @@ struct Piece {
 struct PieceWalker {
   int tpe, kit;          // row tiles per (entry, pass); k-chunks per tile
   long long g, hi, P;    // remainder part: current / end stage of this CTA, total stages
+  long long hi_walk;     // end of the ascending walk (the head piece, emitted first, is cut off)
+  bool head_first, head_pending;
   int ent;               // cursor into cumpass
   const int32_t* cumpass;
   int tile0;             // remainder part: first tile (R0)
   int dp_tile, dp_end, G;
   bool dp;
   __device__ __forceinline__ void init(int sp, int tilesA, int tilesB, int kitA, int kitB, int total_pass,
-                                       const int32_t* cp, int cta, int G_, int min_rounds, int split_pct) {
+                                       const int32_t* cp, int cta, int G_, int min_rounds, int split_pct, bool head_first_) {
     const int ph = sp >> 1;
+    head_first = head_first_;
     tpe = ph == 0 ? tilesA : tilesB;
     kit = ph == 0 ? kitA : kitB;
     G = G_;
@@ -609,6 +613,8 @@ struct PieceWalker {
     }
     g = P * cta / G;
     hi = P * (cta + 1) / G;
+    hi_walk = hi;
+    head_pending = head_first && !dp;
   }
   // data-parallel part: `claimed` is the tile this CTA drew from the phase's counter (ascending per CTA), or
   // anything >= dp_end / negative when the part is exhausted.  Remainder part: `claimed` is ignored.
@@ -619,11 +625,37 @@ struct PieceWalker {
       p.k0 = 0;
       p.k1 = kit;
     } else {
-      if (g >= hi) return false;
+      // Static range [g, hi) of the stage sequence, ascending by default.  Optional piece order (head_first,
+      // ELDR_OPT_HEAD_FIRST): the HEAD of the tile the range ends in comes first and is parked at once; then the tail of
+      // the tile the range starts in -- finished here with the previous CTA's parked head -- then the whole tiles, so
+      // that no range ends on a fix-up.  (Per-CTA traces show the CTAs whose range ends in a short head piece raising
+      // their last h flags ~6 us after the others; but with the fix-ups moved to the start of the sub-phase the step
+      // got 5 us SLOWER at |U| = 16 / 32 -- kept as a parity-tested option, off by default.)
+      if (head_pending) {
+        head_pending = false;
+        if (g < hi) {
+          const long long t_last = (hi - 1) / kit;
+          if (hi % kit != 0 && t_last != g / kit) {
+            p.tile = tile0 + (int)t_last;
+            p.k0 = 0;
+            p.k1 = (int)(hi - t_last * kit);
+            hi_walk = t_last * kit;
+            ent = 0;
+            const int cpi_h = p.tile / tpe;
+            p.rt = p.tile - cpi_h * tpe;
+            int e2 = 0;
+            while (cumpass[e2 + 1] <= cpi_h) ++e2;
+            p.ent = e2;
+            p.pass = cpi_h - cumpass[e2];
+            return true;
+          }
+        }
+      }
+      if (g >= hi_walk) return false;
       const int lt = (int)(g / kit);                 // tile index inside the remainder
       p.tile = tile0 + lt;
       p.k0 = (int)(g - (long long)lt * kit);
-      p.k1 = (int)min((long long)kit, p.k0 + (hi - g));
+      p.k1 = (int)min((long long)kit, p.k0 + (hi_walk - g));
       g += p.k1 - p.k0;
     }
     const int cpi = p.tile / tpe;
@@ -950,7 +982,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
       for (int sp = 0; sp < 4; ++sp) {
         const int ph = sp >> 1;
         PieceWalker pw;
-        pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds, a.sk_split_pct);
+        pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds, a.sk_split_pct, a.head_first != 0);
         Piece p;
         auto stream_piece = [&]() {
           const int4 wk = sm.work[p.ent];
@@ -1020,7 +1052,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     for (int sp = 0; sp < 4; ++sp) {
       const int ph = sp >> 1;
       PieceWalker pw;
-      pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds, a.sk_split_pct);
+      pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds, a.sk_split_pct, a.head_first != 0);
       Piece p;
       int ready_ent = -1;
       while (consumer_next(pw, p, cn)) {
@@ -1093,7 +1125,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     bool first = true;
     for (int sp = 0; sp < 4; ++sp) {
       PieceWalker pw;
-      pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds, a.sk_split_pct);
+      pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds, a.sk_split_pct, a.head_first != 0);
       Piece p;
       while (consumer_next(pw, p, cn)) {
         const int4 wk = sm.work[p.ent];
@@ -1127,7 +1159,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     for (int sp = 0; sp < 4; ++sp) {
       const int ph = sp >> 1;
       PieceWalker pw;
-      pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds, a.sk_split_pct);
+      pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds, a.sk_split_pct, a.head_first != 0);
       const long long P = pw.P;
       Piece p;
       while (consumer_next(pw, p, cn)) {
@@ -1143,32 +1175,53 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
         int n_partner = 0;
         float4 pf0[4], pf1[4];                                  // two chunks of the first partner in flight
         bool pf_valid = false;
-        if (p.k0 == 0 && p.k1 < pw.kit) {
-          const long long tile_end = ((long long)(p.tile - pw.tile0) + 1) * pw.kit;
-          long long covered = (long long)(p.tile - pw.tile0) * pw.kit + p.k1;
-          int j = cta + 1;
-          while (covered < tile_end && j < G) {
-            const long long hj = P * (j + 1) / G;
-            if (hj > covered) {                              // CTA j owns a non-empty piece of this tile
-              if (lane == 0) {
-                uint32_t spins = 0;
+        // Which piece of a split tile finishes it: the owner of its LAST stage (head_first: the partners are the
+        // PRECEDING CTAs, which parked their head pieces at the very start of the sub-phase) or, in the round-1 order,
+        // the owner of its first stage (partners = the following CTAs, which reach the tile first).
+        const bool hf = a.head_first != 0;
+        const int dir = hf ? -1 : 1;
+        const bool finisher = hf ? (p.k1 == pw.kit) : (p.k0 == 0);
+        if (finisher && (hf ? p.k0 > 0 : p.k1 < pw.kit)) {
+          auto wait_partner = [&](int j) {
+            if (lane == 0) {
+              uint32_t spins = 0;
 #ifdef ELDR_TRACE
-                const unsigned long long tp0_ = gtime();
+              const unsigned long long tp0_ = gtime();
 #endif
-                while (flag_acquire(pready + sp * 256 + j) != epoch) { __nanosleep(40); if (++spins > (1u << 24)) __trap(); }
+              while (flag_acquire(pready + sp * 256 + j) != epoch) { __nanosleep(40); if (++spins > (1u << 24)) __trap(); }
 #ifdef ELDR_TRACE
-                if (tid == 0) FADD3(12 + sp, gtime() - tp0_);
+              if (tid == 0) FADD3(12 + sp, gtime() - tp0_);
 #endif
-              }
-              covered = min(hj, tile_end);
-              n_partner = j - cta;
             }
-            ++j;
+          };
+          if (!hf) {
+            const long long tile_end = ((long long)(p.tile - pw.tile0) + 1) * pw.kit;
+            long long covered = (long long)(p.tile - pw.tile0) * pw.kit + p.k1;
+            int j = cta + 1;
+            while (covered < tile_end && j < G) {
+              const long long hj = P * (j + 1) / G;
+              if (hj > covered) {                              // CTA j owns a non-empty piece of this tile
+                wait_partner(j);
+                covered = min(hj, tile_end);
+                n_partner = j - cta;
+              }
+              ++j;
+            }
+          } else {
+            const long long tile_start = (long long)(p.tile - pw.tile0) * pw.kit;
+            for (int j = cta - 1; j >= 0; --j) {
+              const long long lj = P * j / G, hj = P * (j + 1) / G;
+              if (hj <= lj) continue;                          // empty range: parked nothing
+              if (hj <= tile_start) break;
+              wait_partner(j);
+              n_partner = cta - j;
+              if (lj <= tile_start) break;
+            }
           }
           __syncwarp();
-          pf_valid = n_partner >= 1 && (P * (cta + 2) / G > P * (cta + 1) / G);
+          pf_valid = n_partner >= 1 && (P * (cta + dir + 1) / G > P * (cta + dir) / G);
         }
-        const float* pf_src = a.partial + ((size_t)(sp * G + cta + 1) * 128 + row) * kNPCap;
+        const float* pf_src = a.partial + ((size_t)(sp * G + cta + dir) * 128 + row) * kNPCap;
         auto pf_load = [&](float4 (&dst)[4], int c0) {
           if (pf_valid && c0 < n_here) {
 #pragma unroll
@@ -1182,8 +1235,8 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
         tc_fence_after();
         if (tid == 0 && ph == 0) FSTAMP(2);
         const uint32_t t_addr = tmem_base + buf * kNPCap + ((uint32_t)(qtr * 32) << 16);
-        if (p.k0 > 0) {
-          // ---- not the head of this tile: park the raw accumulators for the head owner
+        if (!finisher) {
+          // ---- not the finisher of this tile: park the raw accumulators for it
           float* dstp = a.partial + ((size_t)(sp * G + cta) * 128 + row) * kNPCap;
           for (int c0 = 0; c0 < n_here; c0 += 16) {
             float v[16];
@@ -1199,7 +1252,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
           asm volatile("bar.sync 1, 128;" ::: "memory");
           if (tid == 0) flag_release(pready + sp * 256 + cta, epoch);
         } else {
-          // ---- head (or only) owner: add the parked partials of the following CTAs in ascending order
+          // ---- finisher (or only owner): add the partners' parked partials, nearest CTA first (a fixed order)
           auto chunk = [&](int c0, float4 (&pfx)[4]) {
             float v[16];
             tmem_ld16(t_addr + c0, v);
@@ -1212,9 +1265,9 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
             }
             for (int j = pf_valid ? 2 : 1; j <= n_partner; ++j) {
               // CTAs with an empty range parked nothing; their slot is skipped by the same test as above
-              const long long lj = P * (cta + j) / G, hj = P * (cta + j + 1) / G;
+              const long long lj = P * (cta + dir * j) / G, hj = P * (cta + dir * j + 1) / G;
               if (hj <= lj) continue;
-              const float* srcp = a.partial + ((size_t)(sp * G + cta + j) * 128 + row) * kNPCap + c0;
+              const float* srcp = a.partial + ((size_t)(sp * G + cta + dir * j) * 128 + row) * kNPCap + c0;
 #pragma unroll
               for (int q = 0; q < 4; ++q) {
                 const float4 pv = __ldcg(reinterpret_cast<const float4*>(srcp + 4 * q));

@@ -601,6 +601,24 @@ def test_schedule_variants_match_oracle_and_each_other(gpu, oracle, qwen_layer, 
         gpu.eldr_moe_set_option(gpu.OPT_DP_MIN_ROUNDS, 4)
 
 
+def test_head_first_piece_order_matches_oracle(gpu, oracle, qwen_layer):
+    """ELDR_OPT_HEAD_FIRST = 1 (head pieces parked first, split tiles finished by the owner of their last stage): same
+    parity gates, run-to-run bit-identical; on the small-union cases (every tile split) and a large one."""
+    import torch
+    shape, lw, dl = qwen_layer
+    gpu.eldr_moe_set_option(gpu.OPT_HEAD_FIRST, 1)
+    try:
+        for T, u in ((64, 16), (8, 32), (64, 96)):
+            xb, bias = synth.union_case(shape, T, u, synth.accepted_union_seed(T, u))
+            r = run_case(gpu, oracle, shape, lw, xb, bias, layer_obj=dl)
+            assert gpu.eldr_moe_last_launch_count() == 1 and r["n_active"] == u
+            first = dl.run(gpu.bf16_from_bits(xb), torch.from_numpy(bias).cuda()).clone()
+            again = dl.run(gpu.bf16_from_bits(xb), torch.from_numpy(bias).cuda())
+            assert torch.equal(again.view(torch.int16), first.view(torch.int16))
+    finally:
+        gpu.eldr_moe_set_option(gpu.OPT_HEAD_FIRST, 0)
+
+
 def test_invalid_option_values_are_rejected(gpu):
     for key, value in ((gpu.OPT_DP_MIN_ROUNDS, 0), (gpu.OPT_RING_KB, 16), (99, 1)):
         with pytest.raises(RuntimeError):
