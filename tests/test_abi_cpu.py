@@ -115,10 +115,15 @@ def test_tuning_options_validate_their_values(lib):
     ELDR_ERR_INVALID_ARG, valid ones take effect without a GPU (they are read at the next call)."""
     api, so = lib
     set_opt = so.eldr_moe_set_option
-    for key, good, bad in [(api.OPT_FFN_PATH, [api.FFN_MMA_SYNC, api.FFN_TCGEN05], [-1, 2]),
+    for key, good, bad in [(api.OPT_FFN_PATH, [api.FFN_MMA_SYNC, api.FFN_GEMV, api.FFN_TCGEN05], [-1, 3]),
                            (api.OPT_PDL, [0, 1], [2]),
                            (api.OPT_STEP_PATH, [api.STEP_STAGED, api.STEP_FUSED, api.STEP_AUTO], [3]),
-                           (api.OPT_FFN_PAIR, [0, 2, 1], [-1, 3])]:
+                           (api.OPT_FFN_PAIR, [0, 2, 1], [-1, 3]),
+                           (api.OPT_RING_KB, [32, 208], [31, 209]),
+                           (api.OPT_DP_MIN_ROUNDS, [1, 4], [0]),
+                           (api.OPT_SK_SPLIT_PCT, [60, 0], [-1, 101]),
+                           (api.OPT_COOPERATIVE, [0, 1], [-1, 2]),
+                           (api.OPT_HEAD_FIRST, [1, 0], [2])]:
         for v in bad:
             assert set_opt(C.c_int32(key), C.c_int32(v)) == -1
         for v in good:                      # the last one is the default
