@@ -269,6 +269,10 @@ int32_t eldr_moe_workspace_layout(const eldr_moe_shape_t* shape, int32_t T, eldr
                                  streams its whole tiles (every range ends without a fix-up).  Measured on B200: 1 is SLOWER
                                  (|U| = 16: 66.6 vs 61.2 us, 32: 82.2 vs 76.4) -- the early fix-up waits for a partner whose
                                  head piece is longer than ours while the ring is still filling */
+#define ELDR_OPT_XS_MIN_NP 9  /* fused step: when some expert receives at least this many tokens (padded to 16) the w1/w3 phase reads
+                                 its activations from an expert-sorted copy of x written inside the step (16 rows per TMA
+                                 instruction) instead of gathering token rows from x (4 rows per instruction) for every stage;
+                                 16..144, 144 = never (one accumulator pass holds at most 128 columns).  Default 48 */
 #define ELDR_OPT_FFN_PAIR 5   /* prefill-shaped calls (T > 1024, I % 128 == 0, H % 256 == 0): the expert FFN as tcgen05
                                  cta_group::2 tiles (M = 256 over an SM pair, ffn_umma2.cuh).  1 (default): when the call
                                  has >= 256 tokens per expert on average (T*k >= 256*E); 2: always; 0: never (one CTA

@@ -34,6 +34,7 @@ OPT_FFN_PAIR = 5
 OPT_SK_SPLIT_PCT = 6
 OPT_COOPERATIVE = 7
 OPT_HEAD_FIRST = 8
+OPT_XS_MIN_NP = 9
 PROFILE_SLOTS = ("gate", "route", "gather", "ffn13", "ffn2", "combine")
 
 

@@ -37,6 +37,7 @@ std::atomic<int> g_dp_min_rounds{4};
 std::atomic<int> g_sk_split_pct{0};
 std::atomic<int> g_coop{1};
 std::atomic<int> g_head_first{0};
+std::atomic<int> g_xs_min_np{48};
 
 thread_local char g_err[256] = "";
 thread_local int g_launches = 0;
@@ -462,6 +463,10 @@ int32_t eldr_moe_set_option(int32_t key, int32_t value) {
     g_dp_min_rounds = value;
     return ELDR_OK;
   }
+  if (key == ELDR_OPT_XS_MIN_NP && value >= 16 && value <= 144) {
+    g_xs_min_np = value;
+    return ELDR_OK;
+  }
   if (key == ELDR_OPT_HEAD_FIRST && (value == 0 || value == 1)) {
     g_head_first = value;
     return ELDR_OK;
@@ -607,10 +612,13 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
     fa.dp_min_rounds = g_dp_min_rounds.load();
     fa.sk_split_pct = g_sk_split_pct.load();
     fa.head_first = g_head_first.load();
+    fa.xs_min_np = g_xs_min_np.load();
+    fa.xs = x_perm;
     const size_t smem = fixed + fa.stage_area;
     if ((size_t)fa.stage_area >= min_area) {
-      CUtensorMap tm_w13, tm_sw13, tm_w2, tm_sw2, tm_x, tm_h;
+      CUtensorMap tm_w13, tm_sw13, tm_w2, tm_sw2, tm_x, tm_xs, tm_h;
       if (!make_tmap(&tm_x, x, (uint64_t)T, H, 1)) return ELDR_ERR_CUDA;                       // gather4: 1-row box
+      if (!make_tmap(&tm_xs, x_perm, (uint64_t)T * k + (ns ? T : 0), H, 16)) return ELDR_ERR_CUDA;   // wide batches: expert-sorted copy
       if (!make_tmap(&tm_h, hbuf, (uint64_t)T * (k + ns), I, 16)) return ELDR_ERR_CUDA;
       if (!make_tmap_w13_5d(&tm_w13, w13, E, I, H)) return ELDR_ERR_CUDA;
       if (!make_tmap(&tm_w2, w2, (uint64_t)E * H, I, 128)) return ELDR_ERR_CUDA;
@@ -646,7 +654,7 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
       if (fused_ok == 1) {
         prof_begin();
         prof_mark(0, st);
-        const cudaError_t le = launch_fused(kern, dv, dim3(num_sms()), dim3(kFusedThreads), smem, st, tm_w13, tm_sw13, tm_w2, tm_sw2, tm_x, tm_h, fa);
+        const cudaError_t le = launch_fused(kern, dv, dim3(num_sms()), dim3(kFusedThreads), smem, st, tm_w13, tm_sw13, tm_w2, tm_sw2, tm_x, tm_xs, tm_h, fa);
         if (le == cudaErrorCooperativeLaunchTooLarge) {
           // the device cannot hold the grid right now (partitioned SMs): not an error of the call -- staged path
           cudaGetLastError();

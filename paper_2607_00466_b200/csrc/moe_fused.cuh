@@ -53,8 +53,8 @@ constexpr int kSyncGen = 0;
 constexpr int kSyncCntReady = 1;                // CTA 0 zeroed this step's tile counters
 constexpr int kSyncTileCnt = 2;                 // [2] next unclaimed data-parallel tile of phase A / B
 constexpr int kSyncExit = 4;                    // CTAs that have left the step (zeroed by CTA 0 with the tile counters; the last one bumps the generation)
-constexpr int kSyncDone = 32;                   // [256]     (unused since the flag-driven combine; kept for layout stability)
-constexpr int kSyncGroup = kSyncDone + 256;     // [32]      per token group "ids/weights written"
+constexpr int kSyncXReady = 32;                 // [256]     per CTA "my rows of the expert-sorted copy of x are written"
+constexpr int kSyncGroup = kSyncXReady + 256;     // [32]      per token group "ids/weights written"
 constexpr int kSyncTile = kSyncGroup + 32;      // [32][32]  gate logit tile written
 constexpr int kSyncPartial = kSyncTile + 1024;  // [4][256]  per (sub-phase, CTA) "partial accumulators parked"
 constexpr int kSyncHReady = kSyncPartial + 1024; // [(E+ns)*2*tilesA] per phase-A tile "h tile written", then
@@ -101,6 +101,7 @@ struct FusedArgs {
   unsigned long long* idt;     // [T][4] tagged top-k ids (inside the sync region)
   unsigned long long* wtag;    // [T][16] tagged top-k weights (inside the sync region)
   float* partial;              // [4][gridDim.x][128][kNPCap] fp32 scratch of the stream-K fix-up
+  uint16_t* xs;                // [T*k (+T), H] bf16: x rows in expert-sorted position order (wide batches only)
   uint16_t* hbuf;              // [T*(k+ns), I] bf16
   float* ybuf;                 // [T*(k+ns), H] fp32
   uint16_t* out;               // [T,H] bf16
@@ -108,6 +109,7 @@ struct FusedArgs {
   int ring_bytes;              // cap on the bytes the ring keeps in flight (<= stage_area)
   int dp_min_rounds;           // hybrid schedule: data-parallel part only if a phase has at least this many tile rounds
   int sk_split_pct;            // small unions (whole phase stream-K): share of the accumulator passes in the first expert group
+  int xs_min_np;               // experts with this many token columns or more (np, padded to 16): phase A reads the sorted copy of x
   int head_first;              // static ranges: head piece first and parked, split tiles finished by the owner of their last stage
 };
 
@@ -777,8 +779,8 @@ template <int GT>
 __global__ void __launch_bounds__(kFusedThreads, 1)
 moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_constant__ CUtensorMap tm_sw13,
                  const __grid_constant__ CUtensorMap tm_w2, const __grid_constant__ CUtensorMap tm_sw2,
-                 const __grid_constant__ CUtensorMap tm_x, const __grid_constant__ CUtensorMap tm_h,
-                 const FusedArgs a) {
+                 const __grid_constant__ CUtensorMap tm_x, const __grid_constant__ CUtensorMap tm_xs,
+                 const __grid_constant__ CUtensorMap tm_h, const FusedArgs a) {
   extern __shared__ uint8_t smem_dyn[];
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int G = gridDim.x, cta = blockIdx.x;
@@ -827,6 +829,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     tma_prefetch_desc(&tm_w13);
     tma_prefetch_desc(&tm_w2);
     tma_prefetch_desc(&tm_x);
+    tma_prefetch_desc(&tm_xs);
     tma_prefetch_desc(&tm_h);
   }
   constexpr uint32_t tmem_cols = 2 * kNPCap;
@@ -931,6 +934,33 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
   // ------------------------------------------------------------------------------------------ F: expert FFN
   const int n_work = sm.meta[0];
   const int NP = sm.meta[1], S = sm.meta[2], total_pass = sm.meta[3];
+  // Wide batches (some expert has xs_min_np token columns or more): phase A reads its activations from an
+  // expert-sorted copy of x, sixteen rows per TMA instruction, instead of gathering the token rows four per
+  // instruction from x for every stage -- at 64-128 tokens per expert the gather instructions, not the bytes, bound
+  // phase A (measured: T = 256, |U| = 32: 110.6 -> 99.0 us with plain boxes).  CTA c copies rows c, c + G, ... (one
+  // warp per 4-KiB row) while its weights producer fills the ring, then raises its flag; the activation producers
+  // wait for all G flags once.  Narrow batches keep the gather: few instructions per stage and no extra hand-over.
+  const bool use_xs = NP >= a.xs_min_np;
+  if (use_xs && warp != 4) {
+    const int n_rows = T * k + (ns ? T : 0);
+    const int w7 = warp < 4 ? warp : warp - 1;
+    const int vec = H >> 3;                                     // 16-byte chunks per row
+    for (int pos = cta + G * w7; pos < n_rows; pos += G * 7) {
+      const uint4* src = reinterpret_cast<const uint4*>(a.x + (size_t)sm.tok_of_pos[pos] * H);
+      uint4* dst = reinterpret_cast<uint4*>(a.xs + (size_t)pos * H);
+      for (int c0 = lane; c0 < vec; c0 += 256) {
+        uint4 v[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) v[j] = (c0 + 32 * j < vec) ? __ldcg(src + c0 + 32 * j) : make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll
+        for (int j = 0; j < 8; ++j)
+          if (c0 + 32 * j < vec) dst[c0 + 32 * j] = v[j];
+      }
+    }
+    fence_proxy_async_all();                                    // generic stores, read by other SMs' TMA loads
+    asm volatile("bar.sync 2, 224;" ::: "memory");
+    if (tid == 0) flag_release(a.sync + kSyncXReady + cta, epoch);
+  }
   const uint32_t stage_bytes = kUmmaWBytes + NP * 128;
   const int tilesA = I / 64, tilesB = (H + 127) / 128;
   const int kitA = H / 64, kitB = I / 64;
@@ -1046,6 +1076,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     }
     __syncwarp();
     uint32_t it = 0, cn = 0;
+    bool xs_ready = false;
 #ifdef ELDR_TRACE
     unsigned long long stall = 0, nb = 0;
 #endif
@@ -1057,6 +1088,12 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
       int ready_ent = -1;
       while (consumer_next(pw, p, cn)) {
         const int4 wk = sm.work[p.ent];
+        if (ph == 0 && use_xs && !xs_ready) {
+          warp_wait_flags(a.sync + kSyncXReady, G, epoch, lane);
+          fence_proxy_async_all();
+          __syncwarp();
+          xs_ready = true;
+        }
         if (ph == 1 && p.ent != ready_ent) {
           // every h tile of this expert must have landed (written by generic stores of other CTAs, read here by
           // the async proxy: acquire, then a proxy fence)
@@ -1084,7 +1121,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
         const int n_pad = (n_here + 15) & ~15;
         // phase A: this lane's four gather rows (padding rows repeat the last valid row; their columns are ignored)
         int r0 = 0, r1 = 0, r2 = 0, r3 = 0;
-        if (ph == 0 && 4 * lane < n_pad) {
+        if (ph == 0 && !use_xs && 4 * lane < n_pad) {
           const uint16_t* tp = sm.tok_of_pos + wk.y + n0;
           r0 = tp[min(4 * lane, n_here - 1)];
           r1 = tp[min(4 * lane + 1, n_here - 1)];
@@ -1101,7 +1138,11 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
           __syncwarp();
           const uint32_t dst = sm.stage_base + s * stage_bytes + kUmmaWBytes;
           if (ph == 0) {
-            if (4 * lane < n_pad) tma_gather4(dst + lane * 512, &tm_x, kc * 64, r0, r1, r2, r3, full_bar(s), xpol);
+            if (use_xs) {
+              if (16 * lane < n_pad) tma_load_2d(dst + lane * 2048, &tm_xs, kc * 64, wk.y + n0 + 16 * lane, full_bar(s), xpol);
+            } else if (4 * lane < n_pad) {
+              tma_gather4(dst + lane * 512, &tm_x, kc * 64, r0, r1, r2, r3, full_bar(s), xpol);
+            }
           } else {
             if (16 * lane < n_pad) tma_load_2d(dst + lane * 2048, &tm_h, kc * 64, wk.z + n0 + 16 * lane, full_bar(s), xpol);
           }
@@ -1173,7 +1214,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
         // own accumulator: under a saturated memory system every dependent L2 round trip costs more than a microsecond.
         if (tid == 0 && ph == 0) FSTAMP2(3);
         int n_partner = 0;
-        float4 pf0[4], pf1[4];                                  // two chunks of the first partner in flight
+        float4 pf0[4], pf1[4], pf2[4], pf3[4];                  // four chunks of the first partner in flight
         bool pf_valid = false;
         // Which piece of a split tile finishes it: the owner of its LAST stage (head_first: the partners are the
         // PRECEDING CTAs, which parked their head pieces at the very start of the sub-phase) or, in the round-1 order,
@@ -1221,29 +1262,33 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
           __syncwarp();
           pf_valid = n_partner >= 1 && (P * (cta + dir + 1) / G > P * (cta + dir) / G);
         }
-        const float* pf_src = a.partial + ((size_t)(sp * G + cta + dir) * 128 + row) * kNPCap;
+        // parked partials: [slot][column / 4][row] float4 -- the 32 lanes of a warp (consecutive rows) touch 512
+        // contiguous bytes per access
+        const float4* pf_src = reinterpret_cast<const float4*>(a.partial) + (size_t)(sp * G + cta + dir) * 128 * (kNPCap / 4) + row;
         auto pf_load = [&](float4 (&dst)[4], int c0) {
           if (pf_valid && c0 < n_here) {
 #pragma unroll
-            for (int q = 0; q < 4; ++q) dst[q] = __ldcg(reinterpret_cast<const float4*>(pf_src + c0 + 4 * q));
+            for (int q = 0; q < 4; ++q) dst[q] = __ldcg(pf_src + (size_t)(c0 / 4 + q) * 128);
           }
         };
         if (tid == 0 && ph == 0) FSTAMP2(2);
         pf_load(pf0, 0);
         pf_load(pf1, 16);
+        pf_load(pf2, 32);
+        pf_load(pf3, 48);
         mbar_wait(tfull_bar(buf), (piece_no >> 1) & 1);
         tc_fence_after();
         if (tid == 0 && ph == 0) FSTAMP(2);
         const uint32_t t_addr = tmem_base + buf * kNPCap + ((uint32_t)(qtr * 32) << 16);
         if (!finisher) {
           // ---- not the finisher of this tile: park the raw accumulators for it
-          float* dstp = a.partial + ((size_t)(sp * G + cta) * 128 + row) * kNPCap;
+          float4* dstp = reinterpret_cast<float4*>(a.partial) + (size_t)(sp * G + cta) * 128 * (kNPCap / 4) + row;
           for (int c0 = 0; c0 < n_here; c0 += 16) {
             float v[16];
             tmem_ld16(t_addr + c0, v);
 #pragma unroll
             for (int q = 0; q < 4; ++q)
-              *reinterpret_cast<float4*>(dstp + c0 + 4 * q) = make_float4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
+              dstp[(size_t)(c0 / 4 + q) * 128] = make_float4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
           }
           tc_fence_before();
           __syncwarp();
@@ -1261,16 +1306,16 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
               for (int q = 0; q < 4; ++q) {
                 v[4 * q] += pfx[q].x; v[4 * q + 1] += pfx[q].y; v[4 * q + 2] += pfx[q].z; v[4 * q + 3] += pfx[q].w;
               }
-              pf_load(pfx, c0 + 32);                           // refill this buffer two chunks ahead
+              pf_load(pfx, c0 + 64);                           // refill this buffer four chunks ahead
             }
             for (int j = pf_valid ? 2 : 1; j <= n_partner; ++j) {
               // CTAs with an empty range parked nothing; their slot is skipped by the same test as above
               const long long lj = P * (cta + dir * j) / G, hj = P * (cta + dir * j + 1) / G;
               if (hj <= lj) continue;
-              const float* srcp = a.partial + ((size_t)(sp * G + cta + dir * j) * 128 + row) * kNPCap + c0;
+              const float4* srcp = reinterpret_cast<const float4*>(a.partial) + (size_t)(sp * G + cta + dir * j) * 128 * (kNPCap / 4) + row;
 #pragma unroll
               for (int q = 0; q < 4; ++q) {
-                const float4 pv = __ldcg(reinterpret_cast<const float4*>(srcp + 4 * q));
+                const float4 pv = __ldcg(srcp + (size_t)(c0 / 4 + q) * 128);
                 v[4 * q] += pv.x; v[4 * q + 1] += pv.y; v[4 * q + 2] += pv.z; v[4 * q + 3] += pv.w;
               }
             }
@@ -1300,10 +1345,12 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
               }
             }
           };
-          for (int c0 = 0; c0 < n_here; c0 += 32) {
+          for (int c0 = 0; c0 < n_here; c0 += 64) {
             chunk(c0, pf0);
             if (tid == 0 && ph == 0 && c0 == 0) FSTAMP(3);
             if (c0 + 16 < n_here) chunk(c0 + 16, pf1);
+            if (c0 + 32 < n_here) chunk(c0 + 32, pf2);
+            if (c0 + 48 < n_here) chunk(c0 + 48, pf3);
           }
           tc_fence_before();
           __syncwarp();
