@@ -126,7 +126,9 @@ __device__ __forceinline__ unsigned long long gtime() {
 #define FTIMED(acc, stmt) do { const long long c0_ = clock64(); stmt; acc += clock64() - c0_; } while (0)
 #define FSTAMP3(id) do { g_trace[((blockIdx.x + 1024) & 4095) * 16 + (id)] = gtime(); } while (0)
 #define FADD3(id, v) do { g_trace[((blockIdx.x + 1024) & 4095) * 16 + (id)] += (unsigned long long)(v); } while (0)
+#define FADD4(id, v) do { g_trace[((blockIdx.x + 3072) & 4095) * 16 + (id)] += (unsigned long long)(v); } while (0)
 #else
+#define FADD4(id, v) do {} while (0)
 #define FSTAMP3(id) do {} while (0)
 #define FADD3(id, v) do {} while (0)
 #define FSTAMP2(id) do {} while (0)
@@ -1276,8 +1278,14 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
         pf_load(pf1, 16);
         pf_load(pf2, 32);
         pf_load(pf3, 48);
+#ifdef ELDR_TRACE
+        const long long ce0_ = clock64();
+#endif
         mbar_wait(tfull_bar(buf), (piece_no >> 1) & 1);
         tc_fence_after();
+#ifdef ELDR_TRACE
+        const long long ce1_ = clock64();
+#endif
         if (tid == 0 && ph == 0) FSTAMP(2);
         const uint32_t t_addr = tmem_base + buf * kNPCap + ((uint32_t)(qtr * 32) << 16);
         if (!finisher) {
@@ -1293,9 +1301,15 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive(tempty_bar(buf));
+#ifdef ELDR_TRACE
+          const long long ce2_ = clock64();
+#endif
           __threadfence();
           asm volatile("bar.sync 1, 128;" ::: "memory");
           if (tid == 0) flag_release(pready + sp * 256 + cta, epoch);
+#ifdef ELDR_TRACE
+          if (tid == 0) { const int b_ = ph * 8; FADD4(b_ + 0, 1); FADD4(b_ + 1, ce1_ - ce0_); FADD4(b_ + 2, ce2_ - ce1_); FADD4(b_ + 3, clock64() - ce2_); }
+#endif
         } else {
           // ---- finisher (or only owner): add the partners' parked partials, nearest CTA first (a fixed order)
           auto chunk = [&](int c0, float4 (&pfx)[4]) {
@@ -1321,18 +1335,28 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
             }
             if (ph == 0) {
               // lanes 0-15: g for i = rt*64 + 16*qtr + lane; lanes 16-31: u for the same i
+              // (three straight-line passes -- exchange, SiLU * u, predicated stores: with the bounds test around
+              // the whole body every element was its own branch region, shuffle -> ex2 -> rcp -> store in series,
+              // ~0.8 us per 16-column chunk)
               const bool lo = lane < 16;
               const int i = p.rt * 64 + 16 * qtr + (lane & 15);
+              float gv[8], uv[8];
 #pragma unroll
               for (int kk = 0; kk < 8; ++kk) {
                 const float send = lo ? v[8 + kk] : v[kk];
                 const float recv = __shfl_xor_sync(0xffffffffu, send, 16);
-                const float gv = lo ? v[kk] : recv;
-                const float uv = lo ? recv : v[8 + kk];
-                const int tok = n0 + c0 + (lo ? kk : 8 + kk);
-                if (tok < wk.w)
-                  a.hbuf[(size_t)(wk.z + tok) * I + i] = f32_to_bf16_rn(__fdividef(gv, 1.0f + __expf(-gv)) * uv);
+                gv[kk] = lo ? v[kk] : recv;
+                uv[kk] = lo ? recv : v[8 + kk];
               }
+              uint16_t hv[8];
+#pragma unroll
+              for (int kk = 0; kk < 8; ++kk) hv[kk] = f32_to_bf16_rn(__fdividef(gv[kk], 1.0f + __expf(-gv[kk])) * uv[kk]);
+              const int tok0 = n0 + c0 + (lo ? 0 : 8);
+              uint16_t* hp = a.hbuf + (size_t)(wk.z + tok0) * I + i;
+              const int n_rem = wk.w - tok0;
+#pragma unroll
+              for (int kk = 0; kk < 8; ++kk)
+                if (kk < n_rem) hp[(size_t)kk * I] = hv[kk];
             } else {
               const int r = p.rt * 128 + row;
               if (r < H) {
@@ -1356,6 +1380,9 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
           __syncwarp();
           if (lane == 0) mbar_arrive(tempty_bar(buf));
           if (tid == 0 && ph == 0) FSTAMP(4);
+#ifdef ELDR_TRACE
+          const long long ce2_ = clock64();
+#endif
           if (ph == 0) {
             // publish "h tile written": each writer orders its stores before later async-proxy (TMA) reads, the
             // four epilogue warps meet, one thread releases (cumulative)
@@ -1367,6 +1394,9 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
             asm volatile("bar.sync 1, 128;" ::: "memory");
             if (tid == 0) flag_release(ydone + p.tile, epoch);
           }
+#ifdef ELDR_TRACE
+          if (tid == 0) { const int b_ = ph * 8 + 4; FADD4(b_ + 0, 1); FADD4(b_ + 1, ce1_ - ce0_); FADD4(b_ + 2, ce2_ - ce1_); FADD4(b_ + 3, clock64() - ce2_); }
+#endif
         }
         ++piece_no;
       }
