@@ -97,6 +97,23 @@ int32_t eldr_moe_gate_topk(const eldr_moe_shape_t* shape, int32_t layer, int32_t
                            int32_t* sig_req, int8_t* sig_block,
                            void* workspace, size_t workspace_bytes, eldr_stream_t stream);
 
+/* eldr_moe_gate_topk for callers that may not allocate (CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): same operation, same outputs, NO workspace argument and no allocation of any kind inside the call (no
+ * cudaMalloc / cudaFree, no allocating library routine).  The logits z [T,E] fp32 live in a file-scope
+ * `static __device__` array of ELDR_STATIC_SCRATCH_BYTES bytes inside the library; every GPU that loads the library
+ * holds that array until the process exits.
+ *   Limit: T * n_experts * 4 <= ELDR_STATIC_SCRATCH_BYTES (1 MiB: T <= 2048 at E = 128); beyond it the call returns
+ *   ELDR_ERR_WORKSPACE_SMALL (eldr_last_cuda_error() says by how much) and launches nothing.
+ *   All calls on a device share the one array and it keeps the last call's logits; the call overwrites every element
+ *   it later reads, so nothing needs clearing -- but two calls that OVERLAP on the GPU (different streams, or graphs
+ *   replayed concurrently) race on it: serialise them.  Other arguments exactly as eldr_moe_gate_topk. */
+#define ELDR_STATIC_SCRATCH_BYTES (1u << 20)
+int32_t eldr_moe_gate_topk_static(const eldr_moe_shape_t* shape, int32_t layer, int32_t T,
+                                  const eldr_bf16* x, const float* gate_w, const float* gate_bias,
+                                  int32_t* topk_ids, float* topk_w,
+                                  const int32_t* token_req, const int32_t* token_block,
+                                  int32_t* sig_req, int8_t* sig_block, eldr_stream_t stream);
+
 /* One decode step of one MoE layer: gate -> top-k (+signature) -> token->expert permutation with union
  * compaction -> grouped SwiGLU FFN streaming each ACTIVE expert's weights once -> weighted combine.
  *   w13 [E,2I,H] bf16: rows 0..I-1 = w1 (SiLU branch), rows I..2I-1 = w3;  w2 [E,H,I] bf16;

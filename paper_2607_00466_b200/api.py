@@ -18,7 +18,7 @@ from . import build as _build
 _lib = None
 
 EXPORTS = [
-    "eldr_moe_gate_topk", "eldr_moe_decode_layer", "eldr_moe_decode_layer_host", "eldr_moe_decode_layer_mxfp4",
+    "eldr_moe_gate_topk", "eldr_moe_gate_topk_static", "eldr_moe_decode_layer", "eldr_moe_decode_layer_host", "eldr_moe_decode_layer_mxfp4",
     "eldr_signature_accumulate", "eldr_signature_accumulate_layers", "eldr_signature_reset_blocks", "eldr_signature_readout", "eldr_route_decide",
     "eldr_moe_workspace_bytes", "eldr_moe_workspace_bytes_host", "eldr_moe_workspace_layout",
     "eldr_moe_last_launch_count", "eldr_status_string", "eldr_last_cuda_error",
@@ -160,6 +160,21 @@ def eldr_moe_gate_topk(shape, layer: int, x, gate_w, gate_bias, topk_ids, topk_w
         _ptr(token_req, torch.int32), _ptr(token_block, torch.int32), _ptr(sig_req, torch.int32),
         _ptr(sig_block, torch.int8), _ptr(workspace), C.c_size_t(workspace.numel() * workspace.element_size()),
         _stream()), "eldr_moe_gate_topk")
+
+
+STATIC_SCRATCH_BYTES = 1 << 20
+
+
+def eldr_moe_gate_topk_static(shape, layer: int, x, gate_w, gate_bias, topk_ids, topk_w, token_req=None,
+                              token_block=None, sig_req=None, sig_block=None):
+    """eldr_moe_gate_topk without a workspace: the logits scratch is a static array inside the library (no allocation)."""
+    s = make_shape(shape)
+    T = x.shape[0]
+    _check(load().eldr_moe_gate_topk_static(
+        C.byref(s), C.c_int32(layer), C.c_int32(T), _ptr(x, torch.bfloat16), _ptr(gate_w, torch.float32),
+        _ptr(gate_bias, torch.float32), _ptr(topk_ids, torch.int32), _ptr(topk_w, torch.float32),
+        _ptr(token_req, torch.int32), _ptr(token_block, torch.int32), _ptr(sig_req, torch.int32),
+        _ptr(sig_block, torch.int8), _stream()), "eldr_moe_gate_topk_static")
 
 
 def eldr_moe_decode_layer(shape, layer: int, x, gate_w, gate_bias, w13, w2, shared_w13, shared_w2, out,

@@ -39,6 +39,12 @@ std::atomic<int> g_coop{1};
 std::atomic<int> g_head_first{0};
 std::atomic<int> g_xs_min_np{48};
 
+// Scratch of eldr_moe_gate_topk_static (the entry point that allocates nothing): the gate logits z [T,E] fp32.  File
+// scope, so every GPU that loads the library holds these bytes until the process exits.  In HOST code this name is a
+// host-side stand-in, not a device address: the entry point asks cudaGetSymbolAddress for the device address, once per
+// device, and hands that to the kernels.
+static __device__ __align__(256) unsigned char g_static_scratch[ELDR_STATIC_SCRATCH_BYTES];
+
 thread_local char g_err[256] = "";
 thread_local int g_launches = 0;
 
@@ -146,6 +152,7 @@ struct DevState {
   std::atomic<int> sms{0};
   std::atomic<int> fused_ok{-1};          // -1 unknown, 0 the persistent grid cannot be co-resident, 1 it can
   std::atomic<int> coop_pdl_ok{-1};       // -1 unknown, 1 cooperative + programmatic launch compose on this driver, 0 they do not
+  std::atomic<void*> static_scratch{nullptr};   // device address of g_static_scratch on this device (cudaGetSymbolAddress)
   std::atomic<bool> attr[kAttrCount];
   DevState() { for (auto& a : attr) a.store(false); }
 };
@@ -541,6 +548,40 @@ int32_t eldr_moe_gate_topk(const eldr_moe_shape_t* s, int32_t layer, int32_t T, 
   TopkArgs a{z, topk_ids, topk_w, token_req, token_block, sig_req, sig_block,
              T, s->n_experts, s->top_k, s->n_layers, layer, s->renormalize};
   return launch_gate_topk(s, T, x, gate_w, gate_bias, z, workspace_bytes, a, st);
+}
+
+int32_t eldr_moe_gate_topk_static(const eldr_moe_shape_t* s, int32_t layer, int32_t T, const eldr_bf16* x,
+                                  const float* gate_w, const float* gate_bias, int32_t* topk_ids, float* topk_w,
+                                  const int32_t* token_req, const int32_t* token_block, int32_t* sig_req,
+                                  int8_t* sig_block, eldr_stream_t stream) {
+  g_launches = 0;
+  int32_t rc = check_shape(s);
+  if (rc != ELDR_OK) return rc;
+  if (T < 0 || layer < 0 || layer >= s->n_layers) return ELDR_ERR_INVALID_ARG;
+  if (T == 0) return ELDR_OK;
+  if (!x || !gate_w || !topk_ids || !topk_w) return ELDR_ERR_INVALID_ARG;
+  if (!aligned16(x) || !aligned16(gate_w) || !aligned16(sig_block)) return ELDR_ERR_INVALID_ARG;
+  const size_t z_bytes = (size_t)T * s->n_experts * 4;
+  if (z_bytes > (size_t)ELDR_STATIC_SCRATCH_BYTES) {
+    snprintf(g_err, sizeof(g_err), "eldr_moe_gate_topk_static: T * n_experts * 4 = %zu bytes of logits exceed the static scratch (%u bytes)",
+             z_bytes, (unsigned)ELDR_STATIC_SCRATCH_BYTES);
+    return ELDR_ERR_WORKSPACE_SMALL;
+  }
+  // device address of the file-scope array: resolved once per device, with that device current (it is: the call runs
+  // on the current device).  No allocation: the array is part of the loaded module.
+  DevState& dv = g_dev[current_device()];
+  void* scratch = dv.static_scratch.load(std::memory_order_acquire);
+  if (!scratch) {
+    if (!cuda_ok(cudaGetSymbolAddress(&scratch, g_static_scratch), "cudaGetSymbolAddress(g_static_scratch)")) return ELDR_ERR_CUDA;
+    dv.static_scratch.store(scratch, std::memory_order_release);
+  }
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  float* z = static_cast<float*>(scratch);
+  TopkArgs a{z, topk_ids, topk_w, token_req, token_block, sig_req, sig_block,
+             T, s->n_experts, s->top_k, s->n_layers, layer, s->renormalize};
+  // z_bytes = one logit tensor: every element of z[0 .. T*E) is written by the logits kernel before the top-k reads it,
+  // so nothing left by an earlier call is ever read and nothing has to be cleared
+  return launch_gate_topk(s, T, x, gate_w, gate_bias, z, z_bytes, a, st);
 }
 
 int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t T, const eldr_bf16* x,
