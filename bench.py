@@ -874,7 +874,7 @@ def main():
     ap.add_argument("--config", default="2", choices=["2", "3", "4", "5", "prefill", "route", "mxfp4", "fit", "gemv"])
     ap.add_argument("--unions", default="", help="config 2: subset of the union sizes, e.g. 16,128")
     ap.add_argument("--prefill-T", default="2048,4096,8192,16384")
-    ap.add_argument("--timeline", default="", help="T:U[,U...]  e.g. 64:16,128 -- print the fused kernel's in-kernel timeline (markdown)")
+    ap.add_argument("--timeline", default="", help="T:U[,U...]  e.g. 64:16,128, or c5 (the config-5 layer, fused path) -- print the fused kernel's in-kernel timeline (markdown)")
     ap.add_argument("--steady", action="store_true", help="--timeline: trace the last of 12 back-to-back steps instead of an isolated one")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -885,8 +885,11 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if args.timeline:
         from paper_2607_00466_b200 import timeline
-        T, us = args.timeline.split(":")
-        timeline.run(int(T), [int(u) for u in us.split(",")], steady=args.steady)
+        if args.timeline == "c5":
+            timeline.run(256, [], steady=args.steady, config5=True)
+        else:
+            T, us = args.timeline.split(":")
+            timeline.run(int(T), [int(u) for u in us.split(",")], steady=args.steady)
         return
     if args.impl == "reference":
         if args.config not in ("2", "3", "4", "5"):

@@ -72,7 +72,7 @@ typedef struct {
   size_t off;        /* int32   [E+1]            exclusive scan of cnt                                   */
   size_t perm;       /* int32   [T*k]            pair index (t*k+slot) at each sorted position           */
   size_t pair_pos;   /* int32   [T*k]            inverse of perm                                         */
-  size_t work;       /* int32x4 [E+n_shared]     {expert, x_row0, out_row0, m} per streamed expert       */
+  size_t work;       /* int32x4 [E+n_shared]     {expert, x_row0, out_row0, m} per streamed expert: routed experts in id order; the shared ones (ids E..) before them (one-launch step) or after them (staged step) */
   size_t n_work;     /* int32   [1]              n_active + n_shared                                     */
   size_t sync;       /* uint32  [...]            epoch flags + generation words (internal); offset 0                       */
   size_t x_perm;     /* bf16    [T*k + T, H]     x gathered in sorted order, then a plain copy of x      */
@@ -262,9 +262,8 @@ int32_t eldr_moe_workspace_layout(const eldr_moe_shape_t* shape, int32_t T, eldr
 #define ELDR_OPT_PDL      1   /* 1 (default): programmatic dependent launch between the step's kernels; 0: plain */
 #define ELDR_OPT_STEP_PATH 2  /* ELDR_STEP_FUSED: the whole step in ONE persistent launch (T <= 256, H,I % 64 == 0);
                                  ELDR_STEP_STAGED: one launch per stage (gate+route, gather, w1/w3, w2, combine), also
-                                 the path for shapes the fused kernel does not take; ELDR_STEP_AUTO (default): fused,
-                                 except for layers with shared experts at T >= 224 (every token goes through a shared
-                                 expert, and the staged path handles such wide activation tiles faster) */
+                                 the path for shapes the fused kernel does not take; ELDR_STEP_AUTO (default): fused
+                                 whenever the shape allows it */
 #define ELDR_OPT_RING_KB  3   /* fused step: cap on the shared-memory stage ring in KiB per SM (bytes in flight);
                                  32..208; default 208 (all of it) */
 #define ELDR_OPT_DP_MIN_ROUNDS 4 /* fused step: a phase whose tile count is at least this many rounds of the grid runs its

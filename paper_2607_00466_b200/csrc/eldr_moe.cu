@@ -621,10 +621,11 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
   float* ybuf = reinterpret_cast<float*>(ws + L.y);
 
   // ------------------------------------------------------------------ whole step in one persistent launch
-  // AUTO: shared experts receive every token, so from ~224 tokens their activation tiles are as wide as the weight
-  // tiles and the staged path (rows gathered once, plain TMA boxes) is faster: config-5 shape at T = 256 280 -> 257 us
+  // AUTO = the one-launch step whenever the shape allows it.  (Round 1 sent layers with shared experts and T >= 224 to
+  // the staged path; with the expert-sorted copy of x and the shared experts first in the work list the one-launch
+  // step is faster there too: config-5 shape, T = 256: 223.6 vs 258.6 us.)
   const int step_path = g_step_path.load();
-  const bool want_fused = step_path == ELDR_STEP_FUSED || (step_path == ELDR_STEP_AUTO && !(ns > 0 && T >= 224));
+  const bool want_fused = step_path == ELDR_STEP_FUSED || step_path == ELDR_STEP_AUTO;
   const int ffn_path = g_ffn_path.load();
   if (want_fused && ffn_path == ELDR_FFN_TCGEN05 && H % 64 == 0 && I % 64 == 0 &&
       T <= kFusedMaxT && num_sms() <= 256) {

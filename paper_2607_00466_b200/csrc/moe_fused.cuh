@@ -475,19 +475,24 @@ __device__ __forceinline__ void fused_route_a(const FusedArgs& a, const FusedSme
     const int coff = cbase + cinc - c;
     const int aoff = abase + __popc(act_ballot & ((1u << lane) - 1u));
     s_off[tid] = coff;
-    s_ent[tid] = c > 0 ? aoff : -1;
+    // Work-list order: the SHARED experts first, then the active routed experts in id order.  The shared experts
+    // take every token, so their tiles are the widest (128 columns per pass) and every token's combine needs them:
+    // first in the list they are whole tiles of the first rounds -- never split between SMs, h and y ready early --
+    // and the tail of each phase is the narrow routed experts, whose fix-ups and epilogues are cheap.  (Shared last:
+    // config-5 shape, T = 256: the last 35 us of the step were 128-column fix-ups and a combine that could not start.)
+    s_ent[tid] = c > 0 ? aoff + ns : -1;
     if (is_cta0) { a.off[tid] = coff; a.cnt[tid] = c; }
     if (c > 0) {
       const int4 wk = make_int4(tid, coff, coff, c);
-      sm.work[aoff] = wk;
-      if (is_cta0) { a.active[aoff] = tid; a.work[aoff] = wk; }
+      sm.work[aoff + ns] = wk;
+      if (is_cta0) { a.active[aoff] = tid; a.work[aoff + ns] = wk; }
     }
     if (is_cta0 && tid >= n_act) a.active[tid] = -1;
   }
   if (tid < ns) {
     const int4 wk = make_int4(E + tid, T * k, T * k + tid * T, T);
-    sm.work[n_act + tid] = wk;
-    if (is_cta0) a.work[n_act + tid] = wk;
+    sm.work[tid] = wk;
+    if (is_cta0) a.work[tid] = wk;
   }
   if (tid == 0) {
     const int np = (min(cmax, kNPCap) + 15) & ~15;
@@ -680,7 +685,6 @@ __device__ __forceinline__ void fused_combine(const FusedArgs& a, const FusedSme
     const int32_t* s_ent = reinterpret_cast<const int32_t*>(sm.route_scratch + (size_t)E * ((T + 31) >> 5) * 8);
     const int q_per_row = H >> 2;
     const int n_units = T * tilesB;
-    const int n_act_ = n_work - ns;
     // Two units per iteration: both units' flag polls, then both units' k row loads, are in flight together (one
     // unit at a time cost a poll + fence + load round trip each: 13 us of combine at T = 256).
     const int u_step = G * (kFusedThreads / 32);
@@ -704,7 +708,7 @@ __device__ __forceinline__ void fused_combine(const FusedArgs& a, const FusedSme
             if (a.force_routing) wt_[q] = __ldcg(a.tk.w + t * k + lane);
             else wsrc_[q] = a.wtag + (size_t)t * kMaxTopK + lane;
           } else if (lane < k + ns) {
-            const int ent = n_act_ + (lane - k);
+            const int ent = lane - k;                       // shared experts lead the work list
             pos_[q] = T * k + (lane - k) * T + t;
             fl_[q] = (sm.cumpass[ent] + t / kNPCap) * tilesB + rt;
             wt_[q] = 1.0f;

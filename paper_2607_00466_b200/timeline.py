@@ -31,28 +31,36 @@ ROW1 = [(8, "kernel entry (before barrier init / TMEM alloc)"), (12, "prelude: o
         (7, "route_a: scan, work list, pass table (warp 0)"), (15, "prelude: routing tables built (route_a)")]
 
 
-def run(T: int, unions, steady: bool = False):
+def run(T: int, unions, steady: bool = False, config5: bool = False):
+    """unions: the config-2/3 union sizes to trace at batch T (Qwen3-30B-A3B-shaped layer); config5 = True traces the
+    config-5 layer instead (64 routed top-6 + 2 shared experts, I = 1408, T = 256, fused path forced; `unions` ignored)."""
     import torch
     from paper_2607_00466_b200 import build as b
     from paper_2607_00466_b200 import api, synth
     lib = api.load(path=b.build(trace=True))
-    shape = synth.SHAPE_QWEN
-    lw = synth.make_layer_weights(shape, synth.WEIGHT_SEED)
+    shape = synth.SHAPE_C5 if config5 else synth.SHAPE_QWEN
+    lw = synth.make_layer_weights(shape, 5 if config5 else synth.WEIGHT_SEED)
+    if config5:
+        T, unions = 256, [shape.n_experts]
+        api.eldr_moe_set_option(api.OPT_STEP_PATH, api.STEP_FUSED)
     dl = api.DecodeLayer(shape, lw, max_T=T)
     copies = [(dl.w13, dl.w2)] + [(dl.w13.clone(), dl.w2.clone()) for _ in range(3)]
-    cmd = "python bench.py --timeline %d:%s%s" % (T, ",".join(str(u) for u in unions), " --steady" if steady else "")
+    cmd = "python bench.py --timeline %s%s" % ("c5" if config5 else "%d:%s" % (T, ",".join(str(u) for u in unions)), " --steady" if steady else "")
     print("# In-kernel timeline of `moe_fused_kernel` (`%s`)\n" % cmd)
     print("%s; -DELDR_TRACE build; microseconds since the first CTA passed its prologue; min / median / max over the CTAs that "
           "hit the stamp.  %s (4 rotating weight copies).\n" %
           (torch.cuda.get_device_name(0), "The last of 12 back-to-back steps is the one traced" if steady else
            "The sixth step of each case, alone on the device, is the one traced"))
     for u in unions:
-        try:
-            seed = synth.accepted_union_seed(T, u)
-        except KeyError:
-            seed = 1000
-        xb, bias = synth.union_case(shape, T, u, seed)
-        x, bias_t = api.bf16_from_bits(xb), torch.from_numpy(bias).cuda()
+        if config5:
+            x, bias_t = api.bf16_from_bits(synth.make_hidden(T, shape.hidden, 5)), None
+        else:
+            try:
+                seed = synth.accepted_union_seed(T, u)
+            except KeyError:
+                seed = 1000
+            xb, bias = synth.union_case(shape, T, u, seed)
+            x, bias_t = api.bf16_from_bits(xb), torch.from_numpy(bias).cuda()
         for it in range(12 if steady else 6):
             if it == 5 and not steady:
                 torch.cuda.synchronize()

@@ -82,7 +82,11 @@ def run_case(gpu, oracle, shape, lw, x_bits, bias=None, token_req=None, token_bl
     n_work = int(dl.ws_view("n_work", T).item())
     assert n_work == n_active + ns
     assert n_work * shape.expert_bytes == (len(np.unique(ids_gpu)) + ns) * 3 * H * I * 2
-    assert np.array_equal(work[:n_active, 0], active[:n_active])
+    # routed entries in expert order; the ns shared entries (ids E..E+ns-1) lead the list on the fused path and close it
+    # on the staged path
+    ent_ids = work[:n_work, 0]
+    assert np.array_equal(ent_ids[ent_ids < shape.n_experts], active[:n_active])
+    assert sorted(ent_ids[ent_ids >= shape.n_experts].tolist()) == list(range(shape.n_experts, shape.n_experts + ns))
 
     # Kernels F13 / F2: per-pair intermediates, indexed by (token, slot) through the permutation
     if check_pairs:
@@ -303,11 +307,11 @@ def test_c5_shared_experts_layer(gpu, oracle):
     token_req, token_block = synth.decode_maps(256)
     r = run_case(gpu, oracle, shape, lw, x, None, token_req, token_block, n_req=256, n_blk=256, check_pairs=False)
     assert r["n_active"] == 64
-    assert gpu.eldr_moe_last_launch_count() == 5      # ELDR_STEP_AUTO: shared experts at T >= 224 take the staged path
-    gpu.eldr_moe_set_option(gpu.OPT_STEP_PATH, gpu.STEP_FUSED)
+    assert gpu.eldr_moe_last_launch_count() == 1      # ELDR_STEP_AUTO: the one-launch step (shared experts lead its work list)
+    gpu.eldr_moe_set_option(gpu.OPT_STEP_PATH, gpu.STEP_STAGED)
     try:
         r = run_case(gpu, oracle, shape, lw, x, None, token_req, token_block, n_req=256, n_blk=256, check_pairs=False)
-        assert r["n_active"] == 64 and gpu.eldr_moe_last_launch_count() == 1
+        assert r["n_active"] == 64 and gpu.eldr_moe_last_launch_count() == 5
     finally:
         gpu.eldr_moe_set_option(gpu.OPT_STEP_PATH, gpu.STEP_AUTO)
 
@@ -520,8 +524,8 @@ def test_fused_kernel_back_to_back_steps_and_graph_capture(gpu, oracle, qwen_lay
 def test_graph_replay_with_new_inputs_matches_oracle(gpu, oracle, case):
     """A captured step must route from the x it finds at replay time, not from the capture-time step: x is
     overwritten in place between replays, ids / weights / signatures are zeroed, and every replay is compared with
-    the oracle on that replay's x.  Covers the staged path (T = 300; config-5 shape at T = 256, which
-    ELDR_STEP_AUTO sends to the staged kernels) -- whose election epoch used to be a host counter frozen into the
+    the oracle on that replay's x.  Covers the staged path (T = 300; config-5 shape at T = 256 with
+    ELDR_STEP_STAGED) -- whose election epoch used to be a host counter frozen into the
     captured launch, so replays silently reused the first step's routing -- and the fused launch."""
     import torch
     if case == "small_T300":
@@ -536,6 +540,17 @@ def test_graph_replay_with_new_inputs_matches_oracle(gpu, oracle, case):
         shape = synth.SHAPE_QWEN
         lw = synth.make_layer_weights(shape, synth.WEIGHT_SEED)
         T, want_launches = 64, 1
+    E, k = shape.n_experts, shape.top_k
+    if case == "c5_T256":
+        gpu.eldr_moe_set_option(gpu.OPT_STEP_PATH, gpu.STEP_STAGED)
+    try:
+        _graph_replay_case(gpu, oracle, shape, lw, T, want_launches)
+    finally:
+        gpu.eldr_moe_set_option(gpu.OPT_STEP_PATH, gpu.STEP_AUTO)
+
+
+def _graph_replay_case(gpu, oracle, shape, lw, T, want_launches):
+    import torch
     E, k = shape.n_experts, shape.top_k
     dl = gpu.DecodeLayer(shape, lw, max_T=T)
     xs = [synth.make_hidden(T, shape.hidden, 900 + i) for i in range(3)]
