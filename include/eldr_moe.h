@@ -266,9 +266,10 @@ int32_t eldr_moe_workspace_layout(const eldr_moe_shape_t* shape, int32_t T, eldr
                                  whenever the shape allows it */
 #define ELDR_OPT_RING_KB  3   /* fused step: cap on the shared-memory stage ring in KiB per SM (bytes in flight);
                                  32..208; default 208 (all of it) */
-#define ELDR_OPT_DP_MIN_ROUNDS 4 /* fused step: a phase whose tile count is at least this many rounds of the grid runs its
-                                 whole rounds round-robin (no split tiles) and only the remainder as stream-K; below it the
-                                 whole phase is stream-K.  1..2^20; default 4 */
+#define ELDR_OPT_DP_MIN_ROUNDS 4 /* fused step: a phase (w1/w3 or w2, decided for each) whose tile count is at least this many
+                                 rounds of the grid runs whole tiles (first tile = the CTA's index, then drawn from a counter),
+                                 its remainder per ELDR_OPT_SK_MAX_SPLIT; below it the whole phase is one stream-K cut.
+                                 1..2^20; default 1 (round 2 started at 4: |U| = 32 74.5 -> 70.1 us, T = 256 98.8 -> 91.2) */
 #define ELDR_OPT_SK_SPLIT_PCT 6 /* fused step, small unions (w1/w3 phase shorter than ELDR_OPT_DP_MIN_ROUNDS rounds of tiles): the
                                  active experts are cut into two groups and the step runs w1/w3(g0) w1/w3(g1) w2(g0) w2(g1);
                                  value = percentage of the experts in g0 (0 or 100: one group).  0..100; default 0: measured on
@@ -285,6 +286,10 @@ int32_t eldr_moe_workspace_layout(const eldr_moe_shape_t* shape, int32_t T, eldr
                                  streams its whole tiles (every range ends without a fix-up).  Measured on B200: 1 is SLOWER
                                  (|U| = 16: 66.6 vs 61.2 us, 32: 82.2 vs 76.4) -- the early fix-up waits for a partner whose
                                  head piece is longer than ours while the ring is still filling */
+#define ELDR_OPT_SK_MAX_SPLIT 10 /* fused step, large unions: the stream-K remainder of a phase (the tiles past the last whole round)
+                                 is cut over at most this many CTAs per tile; the other CTAs go straight on to the next part.
+                                 0 = over the whole grid (round 1).  0..64; default 1 = whole tiles (|U| = 128: 205.8 us at 0,
+                                 203.9 at 2, 197.3 at 1; config-5 shape 221.9 / 215.5 / 216.5) */
 #define ELDR_OPT_XS_MIN_NP 9  /* fused step: when some expert receives at least this many tokens (padded to 16) the w1/w3 phase reads
                                  its activations from an expert-sorted copy of x written inside the step (16 rows per TMA
                                  instruction) instead of gathering token rows from x (4 rows per instruction) for every stage;

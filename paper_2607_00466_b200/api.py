@@ -35,6 +35,7 @@ OPT_SK_SPLIT_PCT = 6
 OPT_COOPERATIVE = 7
 OPT_HEAD_FIRST = 8
 OPT_XS_MIN_NP = 9
+OPT_SK_MAX_SPLIT = 10
 PROFILE_SLOTS = ("gate", "route", "gather", "ffn13", "ffn2", "combine")
 
 

@@ -33,11 +33,12 @@ std::atomic<int> g_ffn_path{ELDR_FFN_TCGEN05};
 std::atomic<int> g_pdl{1};
 std::atomic<int> g_step_path{ELDR_STEP_AUTO};
 std::atomic<int> g_ring_kb{208};
-std::atomic<int> g_dp_min_rounds{4};
+std::atomic<int> g_dp_min_rounds{1};
 std::atomic<int> g_sk_split_pct{0};
 std::atomic<int> g_coop{1};
 std::atomic<int> g_head_first{0};
 std::atomic<int> g_xs_min_np{48};
+std::atomic<int> g_sk_max_split{1};
 
 // Scratch of eldr_moe_gate_topk_static (the entry point that allocates nothing): the gate logits z [T,E] fp32.  File
 // scope, so every GPU that loads the library holds these bytes until the process exits.  In HOST code this name is a
@@ -470,6 +471,10 @@ int32_t eldr_moe_set_option(int32_t key, int32_t value) {
     g_dp_min_rounds = value;
     return ELDR_OK;
   }
+  if (key == ELDR_OPT_SK_MAX_SPLIT && value >= 0 && value <= 64) {
+    g_sk_max_split = value;
+    return ELDR_OK;
+  }
   if (key == ELDR_OPT_XS_MIN_NP && value >= 16 && value <= 144) {
     g_xs_min_np = value;
     return ELDR_OK;
@@ -655,6 +660,7 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
     fa.sk_split_pct = g_sk_split_pct.load();
     fa.head_first = g_head_first.load();
     fa.xs_min_np = g_xs_min_np.load();
+    fa.sk_max_split = g_sk_max_split.load();
     fa.xs = x_perm;
     const size_t smem = fixed + fa.stage_area;
     if ((size_t)fa.stage_area >= min_area) {

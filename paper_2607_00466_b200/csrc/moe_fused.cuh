@@ -110,6 +110,7 @@ struct FusedArgs {
   int dp_min_rounds;           // hybrid schedule: data-parallel part only if a phase has at least this many tile rounds
   int sk_split_pct;            // small unions (whole phase stream-K): share of the accumulator passes in the first expert group
   int xs_min_np;               // experts with this many token columns or more (np, padded to 16): phase A reads the sorted copy of x
+  int sk_max_split;            // large unions: at most this many pieces per tile of a stream-K remainder (0: cut over the whole grid)
   int head_first;              // static ranges: head piece first and parked, split tiles finished by the owner of their last stage
 };
 
@@ -569,15 +570,19 @@ __device__ __forceinline__ void fused_route_b(const FusedArgs& a, const FusedSme
 struct Piece {
   int tile, k0, k1, ent, pass, rt;
 };
-// Hybrid schedule.  Per phase the tile list (entry-major, so experts come in order) is cut at R0 = the largest
-// multiple of gridDim.x:
-//   part 0 ("data-parallel"): tiles [0, R0) go round-robin, whole, tile r*G + c to CTA c in round r -- no split,
-//           no fix-up, and experts FINISH IN ORDER over the phase;
-//   part 1 ("stream-K remainder"): the stages of tiles [R0, end) are cut into gridDim.x equal contiguous ranges.
+// Schedule, decided PER PHASE from its tile count n (tile list entry-major, so experts come in order), R0 = the
+// largest multiple of gridDim.x <= n:
+//   n >= min_rounds * G (default: at least one whole round):
+//     part 0 ("data-parallel"): tiles [0, R0) whole -- the first one of CTA c is tile c, the following ones are drawn
+//             from the phase's counter -- no split, no fix-up, and experts FINISH IN ORDER over the phase;
+//     part 1 (remainder): tiles [R0, n) cut over at most max_split CTAs per tile (default 1: whole tiles on n - R0
+//             CTAs); the other CTAs go straight on to the next phase / the combine.  Measured: every further piece of
+//             a tile costs more (park, publish, the finisher's serial adds) than the idle SMs of a partial round --
+//             |U| = 128: 205.8 us with the remainder cut over the whole grid, 197.4 with whole tiles.
+//   n < min_rounds * G: the whole phase is one static stream-K cut (equal contiguous stage ranges over the grid).
 // Sub-phase order A0 A1 B0 B1: B0 starts on the first experts, whose h tiles were all produced in A0 (several
 // microseconds earlier), so the w1/w3 -> w2 hand-over costs no pipeline drain; B1 needs the last experts, finished
-// a whole B0 earlier.  (With equal contiguous ranges over the WHOLE phase every expert had a tile finished in the
-// last microsecond of A, and every CTA stalled ~9 us at the hand-over.)
+// a whole B0 earlier.
 struct PieceWalker {
   int tpe, kit;          // row tiles per (entry, pass); k-chunks per tile
   long long g, hi, P;    // remainder part: current / end stage of this CTA, total stages
@@ -587,25 +592,31 @@ struct PieceWalker {
   const int32_t* cumpass;
   int tile0;             // remainder part: first tile (R0)
   int dp_tile, dp_end, G;
+  int Gs;                // CTAs that share the static (stream-K) part: 0 .. Gs-1, the others skip it
   bool dp;
   __device__ __forceinline__ void init(int sp, int tilesA, int tilesB, int kitA, int kitB, int total_pass,
-                                       const int32_t* cp, int cta, int G_, int min_rounds, int split_pct, bool head_first_) {
+                                       const int32_t* cp, int cta, int G_, int min_rounds, int split_pct, bool head_first_, int max_split) {
     const int ph = sp >> 1;
     head_first = head_first_;
     tpe = ph == 0 ? tilesA : tilesB;
     kit = ph == 0 ? kitA : kitB;
     G = G_;
+    Gs = G_;
     const int n_tiles = total_pass * tpe;
     ent = 0;
     cumpass = cp;
     dp_tile = cta;
-    if (total_pass * tilesA / G >= min_rounds) {
-      // large union: sub-phases A-dp, A-remainder, B-dp, B-remainder
-      const int R0 = (n_tiles / G >= min_rounds) ? (n_tiles / G) * G : 0;   // few rounds: all stream-K
+    if (n_tiles / G >= min_rounds) {
+      // a phase with at least min_rounds whole rounds of tiles (decided per phase): whole rounds, then the remainder
+      const int R0 = (n_tiles / G) * G;
       dp = (sp & 1) == 0;
       dp_end = R0;
       tile0 = R0;
       P = (long long)(n_tiles - R0) * kit;
+      // a remainder of few tiles is not cut over the whole grid: every further piece of a tile is one more parked
+      // partial the tile's finisher adds in series (config-5 shape: 16 tiles over 148 CTAs = nine pieces per tile, the
+      // finishers 25 us behind); at most max_split pieces per tile, the other CTAs go straight on to the next part
+      if (max_split > 0 && R0 > 0) Gs = min(G, max(1, (n_tiles - R0) * max_split));
     } else {
       // small union (phase A shorter than min_rounds rounds of tiles): the accumulator passes -- experts, in order --
       // are cut into two groups and the sub-phases run A(g0) A(g1) B(g0) B(g1), each a static stream-K cut of its own
@@ -620,8 +631,8 @@ struct PieceWalker {
       tile0 = t_lo;
       P = (long long)(t_hi - t_lo) * kit;
     }
-    g = P * cta / G;
-    hi = P * (cta + 1) / G;
+    g = cta < Gs ? P * cta / Gs : 0;
+    hi = cta < Gs ? P * (cta + 1) / Gs : 0;
     hi_walk = hi;
     head_pending = head_first && !dp;
   }
@@ -1018,7 +1029,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
       for (int sp = 0; sp < 4; ++sp) {
         const int ph = sp >> 1;
         PieceWalker pw;
-        pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds, a.sk_split_pct, a.head_first != 0);
+        pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds, a.sk_split_pct, a.head_first != 0, a.sk_max_split);
         Piece p;
         auto stream_piece = [&]() {
           const int4 wk = sm.work[p.ent];
@@ -1047,10 +1058,12 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
               while (flag_acquire(a.sync + kSyncCntReady) != epoch) { __nanosleep(40); if (++spins > (1u << 24)) __trap(); }
               cnt_ready = true;
             }
-            int cur = (int)atomicAdd(a.sync + kSyncTileCnt + ph, 1u);
+            // first tile: the CTA's own index (no draw, no round trip before the first byte); the counter hands out
+            // tiles G, G+1, ...
+            int cur = cta;
             claim_push(cur);
             while (pw.next(p, cur)) {
-              const int nxt = (int)atomicAdd(a.sync + kSyncTileCnt + ph, 1u);     // in flight while this tile streams
+              const int nxt = G + (int)atomicAdd(a.sync + kSyncTileCnt + ph, 1u);     // in flight while this tile streams
               stream_piece();
               claim_push(nxt);
               cur = nxt;
@@ -1089,7 +1102,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     for (int sp = 0; sp < 4; ++sp) {
       const int ph = sp >> 1;
       PieceWalker pw;
-      pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds, a.sk_split_pct, a.head_first != 0);
+      pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds, a.sk_split_pct, a.head_first != 0, a.sk_max_split);
       Piece p;
       int ready_ent = -1;
       while (consumer_next(pw, p, cn)) {
@@ -1172,7 +1185,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     bool first = true;
     for (int sp = 0; sp < 4; ++sp) {
       PieceWalker pw;
-      pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds, a.sk_split_pct, a.head_first != 0);
+      pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds, a.sk_split_pct, a.head_first != 0, a.sk_max_split);
       Piece p;
       while (consumer_next(pw, p, cn)) {
         const int4 wk = sm.work[p.ent];
@@ -1206,8 +1219,9 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     for (int sp = 0; sp < 4; ++sp) {
       const int ph = sp >> 1;
       PieceWalker pw;
-      pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds, a.sk_split_pct, a.head_first != 0);
+      pw.init(sp, tilesA, tilesB, kitA, kitB, total_pass, sm.cumpass, cta, G, a.dp_min_rounds, a.sk_split_pct, a.head_first != 0, a.sk_max_split);
       const long long P = pw.P;
+      const int Gs = pw.Gs;
       Piece p;
       while (consumer_next(pw, p, cn)) {
         const int4 wk = sm.work[p.ent];
@@ -1245,8 +1259,8 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
             const long long tile_end = ((long long)(p.tile - pw.tile0) + 1) * pw.kit;
             long long covered = (long long)(p.tile - pw.tile0) * pw.kit + p.k1;
             int j = cta + 1;
-            while (covered < tile_end && j < G) {
-              const long long hj = P * (j + 1) / G;
+            while (covered < tile_end && j < Gs) {
+              const long long hj = P * (j + 1) / Gs;
               if (hj > covered) {                              // CTA j owns a non-empty piece of this tile
                 wait_partner(j);
                 covered = min(hj, tile_end);
@@ -1257,7 +1271,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
           } else {
             const long long tile_start = (long long)(p.tile - pw.tile0) * pw.kit;
             for (int j = cta - 1; j >= 0; --j) {
-              const long long lj = P * j / G, hj = P * (j + 1) / G;
+              const long long lj = P * j / Gs, hj = P * (j + 1) / Gs;
               if (hj <= lj) continue;                          // empty range: parked nothing
               if (hj <= tile_start) break;
               wait_partner(j);
@@ -1266,7 +1280,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
             }
           }
           __syncwarp();
-          pf_valid = n_partner >= 1 && (P * (cta + dir + 1) / G > P * (cta + dir) / G);
+          pf_valid = n_partner >= 1 && (P * (cta + dir + 1) / Gs > P * (cta + dir) / Gs);
         }
         // parked partials: [slot][column / 4][row] float4 -- the 32 lanes of a warp (consecutive rows) touch 512
         // contiguous bytes per access
@@ -1328,7 +1342,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
             }
             for (int j = pf_valid ? 2 : 1; j <= n_partner; ++j) {
               // CTAs with an empty range parked nothing; their slot is skipped by the same test as above
-              const long long lj = P * (cta + dir * j) / G, hj = P * (cta + dir * j + 1) / G;
+              const long long lj = P * (cta + dir * j) / Gs, hj = P * (cta + dir * j + 1) / Gs;
               if (hj <= lj) continue;
               const float4* srcp = reinterpret_cast<const float4*>(a.partial) + (size_t)(sp * G + cta + dir * j) * 128 * (kNPCap / 4) + row;
 #pragma unroll

@@ -585,10 +585,12 @@ def _graph_replay_case(gpu, oracle, shape, lw, T, want_launches):
             assert int(dl.n_active.item()) == ora["n_active"]
 
 
-@pytest.mark.parametrize("min_rounds", [1, 1 << 20])
-def test_schedule_variants_match_oracle_and_each_other(gpu, oracle, qwen_layer, min_rounds):
-    """The fused kernel's two schedules -- whole tile rounds drawn dynamically from a global counter (forced here
-    for every phase with at least ONE round) and the static stream-K cut of the whole phase -- must pass the same
+@pytest.mark.parametrize("min_rounds,max_split", [(1, 1), (1 << 20, 1), (4, 3), (1, 0)])
+def test_schedule_variants_match_oracle_and_each_other(gpu, oracle, qwen_layer, min_rounds, max_split):
+    """The fused kernel's schedules -- whole tiles (first one static, then drawn from a global counter) for every
+    phase with at least ONE round, the remainder as whole tiles (the default), the static stream-K cut of the whole
+    phase, round 2's hybrid (whole rounds from 4 rounds on, remainder cut over at most 3 CTAs per tile) and the remainder
+    cut over the whole grid -- must pass the same
     parity gates, and each must be run-to-run bit-identical: the K order inside a tile and the fix-up order are
     fixed, so it does not matter WHICH CTA draws a tile.  (Across the two schedules the fp32 sums are grouped
     differently -- a tile is whole in one and split in the other -- so they agree to rounding, not bit for bit.)
@@ -598,6 +600,7 @@ def test_schedule_variants_match_oracle_and_each_other(gpu, oracle, qwen_layer, 
     shape, lw, dl = qwen_layer
     T = 64
     gpu.eldr_moe_set_option(gpu.OPT_DP_MIN_ROUNDS, min_rounds)
+    gpu.eldr_moe_set_option(gpu.OPT_SK_MAX_SPLIT, max_split)
     try:
         for u in (16, 96):
             xb, bias = synth.union_case(shape, T, u, synth.accepted_union_seed(T, u))
@@ -613,7 +616,8 @@ def test_schedule_variants_match_oracle_and_each_other(gpu, oracle, qwen_layer, 
         run_case(gpu, oracle, small, slw, synth.make_hidden(200, small.hidden, 77))
         assert gpu.eldr_moe_last_launch_count() == 1
     finally:
-        gpu.eldr_moe_set_option(gpu.OPT_DP_MIN_ROUNDS, 4)
+        gpu.eldr_moe_set_option(gpu.OPT_DP_MIN_ROUNDS, 1)
+        gpu.eldr_moe_set_option(gpu.OPT_SK_MAX_SPLIT, 1)
 
 
 def test_head_first_piece_order_matches_oracle(gpu, oracle, qwen_layer):
