@@ -753,7 +753,7 @@ def run_mxfp4(args):
                                              "union sweep (realised unions reported; no rejection sampling)",
                                  "l2": "rotating %d weight copies (1.7 GB each)" % N_COPIES},
                       "frac_of_peak": round(value / peak, 3), "peak_GBps": peak, "peak_kind": kind, "sweep": rows,
-                      "roofline": {"bound": "hbm", "kernel": "ffn_mx_kernel<0> (w1/w3: packed-code streaming + in-smem decode + tcgen05)",
+                      "roofline": {"bound": "hbm", "kernel": "ffn_mx_kernel<0> (w1/w3: packed-code streaming + register decode -> TMEM A operand + tcgen05)",
                                    "achieved": round(top_gbs, 1), "peak": peak, "unit": "GB/s", "frac": round(top_gbs / peak, 3), "traffic": None,
                                    "avg_launch_us": round(top_ms * 1e3, 2), "algorithmic_bytes_per_launch": round(kb13 / n_prof),
                                    "kernel_us": {n_: round(v / n_prof * 1e3, 2) for n_, v in kern.items()}},

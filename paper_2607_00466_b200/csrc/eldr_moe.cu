@@ -979,12 +979,12 @@ int32_t eldr_moe_decode_layer_mxfp4(const eldr_moe_shape_t* s, int32_t layer, in
   m13.scales = w13_scales;
   m2.scales = w2_scales;
   m13.np = m2.np = T <= 64 ? 64 : 128;
-  m13.stages = m2.stages = 3;
-  m13.raw_stages = m2.raw_stages = 5;
+  m13.stages = m2.stages = kMxMaxStages;               // decoded tiles: TMEM ring
+  m13.raw_stages = m2.raw_stages = 8;
   m13.act_stages = m2.act_stages = T <= 64 ? 8 : 4;
   const size_t smem = mx_smem_bytes(m13.np, m13.stages, m13.raw_stages, m13.act_stages);
   if (!once_per_device(kAttrMx, [] {
-        const size_t a_ = mx_smem_bytes(64, 3, 5, 8), b_ = mx_smem_bytes(128, 3, 5, 4);
+        const size_t a_ = mx_smem_bytes(64, kMxMaxStages, 8, 8), b_ = mx_smem_bytes(128, kMxMaxStages, 8, 4);
         const size_t mx = a_ > b_ ? a_ : b_;
         return set_smem(ffn_mx_kernel<0>, mx) && set_smem(ffn_mx_kernel<1>, mx);
       })) return ELDR_ERR_CUDA;

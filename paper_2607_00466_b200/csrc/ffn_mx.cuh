@@ -3,8 +3,11 @@
 // (element 2i in the low nibble), one E8M0 scale byte per 32 elements of the contraction axis, value =
 // e2m1(code) * 2^(scale - 127).  Every decoded value is exactly a bf16 number, and the activations stay bf16, so the
 // layer is BY DEFINITION the plain layer on the decoded weights: the kernel streams the packed bytes from HBM
-// (17/64 of the bf16 bytes), decodes them to bf16 in shared memory and feeds the same tcgen05 swap-AB MMAs as
-// ffn_umma.cuh -- nothing is approximated, the activations are not quantised.
+// (17/64 of the bf16 bytes), decodes them to bf16 in registers, stores the decoded tile into TENSOR MEMORY
+// (tcgen05.st) and issues the swap-AB MMAs with the A operand read from TMEM -- nothing is approximated, the
+// activations are not quantised.  (Round 2's first version wrote the decoded tiles to shared memory: decoded data is
+// four times the packed bytes, written once and read once by the tensor core -- at HBM speed that alone is ~180 bytes
+// per clock against the 128 bytes per clock of an SM's shared memory.  TMEM ring: 1.49 -> 1.75 TB/s of packed bytes.)
 //
 // One persistent CTA per SM, 11 warps:
 //   warp 0   TMA producer, packed weights: 128 rows x 128 bytes (256 codes per row = FOUR 64-element k-chunks) per RAW
@@ -12,16 +15,17 @@
 //            version fetched one k-chunk = 32 bytes per row per stage: 32-byte pieces of 1440-byte rows ran HBM at
 //            1.2 TB/s even with the decode switched off.)
 //   warp 1   TMA producer, activations (as ffn_umma.cuh)
-//   warp 2   MMA issuer: 4 x tcgen05.mma (M=128, N=n_pad, K=16) per stage, fp32 in TMEM
+//   warp 2   MMA issuer: 4 x tcgen05.mma (M=128, N=n_pad, K=16; A = 8 TMEM columns of the decoded ring, B = shared
+//            memory descriptor) per stage, fp32 accumulators in TMEM
 //   warps 3-6  epilogue: TMEM -> SiLU*mul -> h (MODE 0) / y (MODE 1)
 //   warps 7-10 decoders: thread r owns row r of the 128-row tile.  Per k-chunk it reads 32 raw bytes of its row and the
 //            row's two scale bytes (the eight scale bytes of a raw stage are fetched three raw stages ahead with 4-byte
 //            cp.async into a per-thread ring: the scale rows are K/32 bytes long, neither 16-byte aligned nor
 //            TMA-addressable), decodes 64 codes with two
 //            byte-permute look-ups per four codes (magnitudes 0, .5, 1, 1.5, 2, 3, 4, 6 need five distinct bf16 bytes),
-//            ORs in the signs, multiplies by the scale as a bf16x2 power of two (exact) and writes its 128-byte row of
-//            the K-major SWIZZLE_128B operand tile; MODE 0 rows land in the 4 x [16 rows of w1 | 16 of w3] order
-//            the SiLU*mul epilogue expects.  20 operations per 8 codes, 14-16 of them on the ALU pipe (byte permutes,
+//            ORs in the signs, multiplies by the scale as a bf16x2 power of two (exact) and stores its 16 columns
+//            (32 bf16) of the tile row = TMEM lane it owns (a warp reaches the lanes of its quarter, warp % 4); MODE 0
+//            rows land in the 4 x [16 rows of w1 | 16 of w3] order the SiLU*mul epilogue expects.  20 operations per 8 codes, 14-16 of them on the ALU pipe (byte permutes,
 //            logic): 8192 codes per stage -> ~256 SM cycles of ALU-pipe time against ~180 cycles a 4 KiB stage lasts
 //            at HBM speed, so the decode -- not HBM -- bounds this kernel (measured 1.5 TB/s of packed bytes, 2.2 TB/s
 //            with the decode switched off; every role's loop nest is written out with incremental ring cursors
@@ -41,6 +45,8 @@ constexpr int kMxDecWarps = 4 * kMxParts;
 constexpr int kMxThreads = (7 + kMxDecWarps) * 32;
 constexpr int kMxRawBytes = 128 * 128;         // packed codes of one raw stage: 128 rows x 4 k-chunks
 constexpr int kMxRawChunks = 4;                // 64-element k-chunks per raw stage
+constexpr int kMxATmemCol = 256;               // first TMEM column of the decoded-tile ring (accumulators: 2 x np <= 256 columns)
+constexpr int kMxMaxStages = 8;                // decoded-tile ring: 8 x 32 columns
 constexpr int kMxScaleAhead = 3;               // raw stages of scale prefetch per decoder thread (16-byte slot each)
 
 struct MxArgs {
@@ -53,7 +59,8 @@ struct MxArgs {
 // activations (L2 latency: their own ring -- sharing the weight tiles' four stages bounded the pipeline at four stages
 // per L2 round trip, 1.2 TB/s).
 __host__ __device__ inline size_t mx_smem_bytes(int np, int stages, int raw_stages, int act_stages) {
-  return (size_t)stages * kUmmaWBytes + (size_t)act_stages * np * 128 + (size_t)raw_stages * kMxRawBytes +
+  (void)stages;                                  // decoded tiles live in TMEM, not in shared memory
+  return (size_t)act_stages * np * 128 + (size_t)raw_stages * kMxRawBytes +
          (size_t)kMxScaleAhead * kMxDecWarps * 32 * 16 + 1024 + 1024;
 }
 
@@ -125,9 +132,8 @@ ffn_mx_kernel(const __grid_constant__ CUtensorMap tm_codes, const __grid_constan
   const uint32_t smem_base = (smem_u32(smem_dyn) + 1023u) & ~1023u;
   uint8_t* smem_gen = smem_dyn + (smem_base - smem_u32(smem_dyn));
   const int NP = a.np, S = a.stages, RS = a.raw_stages, AS = a.act_stages;
-  const uint32_t stage_bytes = kUmmaWBytes;
   const uint32_t act_bytes = NP * 128;
-  const uint32_t act_base = smem_base + S * stage_bytes;
+  const uint32_t act_base = smem_base;
   const uint32_t raw_base = act_base + AS * act_bytes;
   const uint32_t sc_base = raw_base + RS * kMxRawBytes;             // [kMxScaleAhead][128] x 16 bytes
   const uint32_t bar_base = sc_base + kMxScaleAhead * kMxDecWarps * 32 * 16;
@@ -149,7 +155,9 @@ ffn_mx_kernel(const __grid_constant__ CUtensorMap tm_codes, const __grid_constan
     for (int b = 0; b < 2; ++b) { mbar_init(tfull_bar(b), 1); mbar_init(tempty_bar(b), 4); }
     mbar_fence_init();
   }
-  const uint32_t tmem_cols = 2 * NP;
+  // TMEM: accumulators (2 x NP columns) at column 0, the ring of decoded weight tiles (S stages x 32 columns: 128 rows
+  // x 64 bf16, two per 32-bit column) from column kMxATmemCol on.  All 512 columns: one CTA per SM.
+  const uint32_t tmem_cols = 512;
   if (warp == 2) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(tmem_slot), "r"(tmem_cols) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
@@ -225,7 +233,7 @@ ffn_mx_kernel(const __grid_constant__ CUtensorMap tm_codes, const __grid_constan
     // predicated on the elected lane inside the asm (no ELECT / R2UR waterfall per instruction).
     const uint32_t leader = elect_one();
     const uint32_t uS = warp_uniform((uint32_t)S), uAS = warp_uniform((uint32_t)AS);
-    const uint32_t ubar = warp_uniform(bar_base), uw = warp_uniform(smem_base), ua = warp_uniform(act_base), uab = warp_uniform(act_bytes);
+    const uint32_t ubar = warp_uniform(bar_base), ua = warp_uniform(act_base), uab = warp_uniform(act_bytes);
     const uint32_t utmem = warp_uniform(tmem_base);
     uint32_t unit = 0, ws_ = 0, wpar = 0, as = 0, apar = 0;
     for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
@@ -242,9 +250,10 @@ ffn_mx_kernel(const __grid_constant__ CUtensorMap tm_codes, const __grid_constan
           mbar_wait(ubar + 8u * (2 * uS + 2 * RS + 4 + as), apar);                          // afull
           mbar_wait(ubar + 8u * ws_, wpar);                                                 // wfull
           tc_fence_after();
-          const uint64_t da = umma_desc_sw128(uw + ws_ * kUmmaWBytes), db = umma_desc_sw128(ua + as * uab);
+          const uint32_t a_tmem = utmem + kMxATmemCol + ws_ * 32u;
+          const uint64_t db = umma_desc_sw128(ua + as * uab);
 #pragma unroll
-          for (int k = 0; k < 4; ++k) umma_bf16_if(leader, d_tmem, da + 2 * k, db + 2 * k, idesc, (kc | k) ? 1u : 0u);
+          for (int k = 0; k < 4; ++k) umma_bf16_ts_if(leader, d_tmem, a_tmem + 8u * k, db + 2 * k, idesc, (kc | k) ? 1u : 0u);
           umma_commit_if(leader, ubar + 8u * (uS + ws_));                                   // wempty
           umma_commit_if(leader, ubar + 8u * (2 * uS + 2 * RS + 4 + uAS + as));             // aempty
           if (kc == k_iters - 1) umma_commit_if(leader, ubar + 8u * (2 * uS + 2 * RS + buf));   // tfull
@@ -301,8 +310,9 @@ ffn_mx_kernel(const __grid_constant__ CUtensorMap tm_codes, const __grid_constan
     // ================================================================ decoders: tile row d, part `part` of its 64 codes.
     // kMxParts threads share a row so that each SM sub-partition holds several decoder warps: one warp per
     // sub-partition ran the ~300 dependent-ish ALU instructions of a stage at ~3 cycles each (ncu: 1.4 IPC, 0.9 TB/s).
+    // A warp reaches only the TMEM lanes of its quarter (warp % 4): thread -> tile row d = 32 * (warp % 4) + lane.
     const int dt = threadIdx.x - 7 * 32;
-    const int d = dt & 127, part = dt >> 7;
+    const int d = 32 * (warp & 3) + lane, part = (warp - 7) >> 2;
     const int kscale = f.K / 32;                     // scale bytes per weight row
     const size_t scale_total = (size_t)f.E * f.rows_per_expert * kscale;
     // row of this thread inside the expert's weight matrix, as a function of the row tile
@@ -345,10 +355,11 @@ ffn_mx_kernel(const __grid_constant__ CUtensorMap tm_codes, const __grid_constan
       asm volatile("cp.async.commit_group;" ::: "memory");
     }
     constexpr int NW = 8 / kMxParts;                  // 32-bit words (8 codes each) per thread per stage
+    static_assert(NW == 4 || NW == 8, "a decoder thread stores whole groups of 16 TMEM columns");
     const int n_raw = (k_iters + kMxRawChunks - 1) / kMxRawChunks;
-    const uint32_t rx = src_row & 7, x7 = d & 7;
+    const uint32_t rx = src_row & 7;
     const uint32_t raw_row0 = raw_base + src_row * 128;
-    const uint32_t op_row0 = smem_base + (d >> 3) * 1024 + (d & 7) * 128;
+    const uint32_t a_row0 = tmem_base + kMxATmemCol + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)(4 * NW * part);
     const uint32_t sc_stride = kMxDecWarps * 32;      // uint4 per scale slot
     uint32_t ws_ = 0, wpar = 1, rs = 0, rpar = 0, slot = 0;
     for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
@@ -391,15 +402,18 @@ ffn_mx_kernel(const __grid_constant__ CUtensorMap tm_codes, const __grid_constan
               } else {
                 asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(wd[0]), "=r"(wd[1 % NW]) : "r"(addr));
               }
-              mbar_wait(wempty_bar(ws_), wpar);
-              const uint32_t row_addr = op_row0 + ws_ * stage_bytes;
+              // decode into registers, then straight into this row's TMEM lane: 4 columns (8 bf16) per word
+              uint4 o[NW];
 #pragma unroll
-              for (int i = 0; i < NW; ++i) {
-                const int c = NW * part + i;          // 16-byte chunk of the bf16 row = word index inside the k-chunk
-                const uint4 o = mx_decode8(wd[i], NW == 8 ? (i < 4 ? sc0 : sc1) : scm);
-                asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" :: "r"(row_addr + ((c ^ x7) << 4)), "r"(o.x), "r"(o.y), "r"(o.z), "r"(o.w) : "memory");
-              }
-              asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+              for (int i = 0; i < NW; ++i) o[i] = mx_decode8(wd[i], NW == 8 ? (i < 4 ? sc0 : sc1) : scm);
+              mbar_wait(wempty_bar(ws_), wpar);
+              tc_fence_after();
+              const uint32_t a_addr = a_row0 + ws_ * 32u;
+#pragma unroll
+              for (int i = 0; i < NW; i += 4)
+                tmem_st16(a_addr + 4u * i, o[i], o[(i + 1) % NW], o[(i + 2) % NW], o[(i + 3) % NW]);
+              asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+              tc_fence_before();
               __syncwarp();
               if (lane == 0) mbar_arrive(wfull_bar(ws_));
               if (++ws_ == (uint32_t)S) { ws_ = 0; wpar ^= 1u; }
