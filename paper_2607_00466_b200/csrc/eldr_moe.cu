@@ -783,7 +783,7 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
   // (Gathering inside the w1/w3 kernel by TMA tile::gather4, as the fused decode kernel does, was measured for the
   // prefill-shaped calls and rejected: 256 single-row requests per stage instead of four boxes made w1/w3 3.7x slower.)
   prof_mark(2, st);
-  launch_dep(gather_x_kernel, dim3((x_rows + 7) / 8), dim3(256), 0, st, x, perm, x_perm, T, H, k, x_rows);
+  launch_dep(gather_x_kernel, dim3((x_rows + 7) / 8), dim3(256), 0, st, x, perm, x_perm, T, H, k, x_rows, 0);
   if (!launch_ok("gather_x_kernel")) return ELDR_ERR_CUDA;
 
   // a5/a6: grouped SwiGLU FFN over the active experts
@@ -969,7 +969,7 @@ int32_t eldr_moe_decode_layer_mxfp4(const eldr_moe_shape_t* s, int32_t layer, in
   }
   const int x_rows = T * k;
   prof_mark(2, st);
-  launch_dep(gather_x_kernel, dim3((x_rows + 7) / 8), dim3(256), 0, st, x, perm, x_perm, T, H, k, x_rows);
+  launch_dep(gather_x_kernel, dim3((x_rows + 7) / 8), dim3(256), 0, st, x, perm, x_perm, T, H, k, x_rows, 1);
   if (!launch_ok("gather_x_kernel")) return ELDR_ERR_CUDA;
 
   const int max_work = E < T * k ? E : T * k;

@@ -64,32 +64,36 @@ __host__ __device__ inline size_t mx_smem_bytes(int np, int stages, int raw_stag
          (size_t)kMxScaleAhead * kMxDecWarps * 32 * 16 + 1024 + 1024;
 }
 
-// 8 codes (one 32-bit word, element j in nibble j) -> 8 bf16 values scaled by `sc` (bf16x2, both halves 2^(b-127)).
-// 20 operations: mask, 4 look-ups (high / low byte of the bf16 magnitude of codes 0-3 and 4-7), signs (2 + 2 permutes
-// that spread the nibbles' sign bits to bit 7 of a byte each + 2 masked ORs into the high bytes), 4 byte interleaves,
-// 4 bf16x2 multiplies by the power-of-two scale (exact; zero stays zero).
+// 8 codes (one 32-bit word, element j in nibble j) -> 8 bf16 values scaled by `sc` (bf16x2, both halves 2^(b-127)),
+// in the K-SLOT ORDER e0 e4 | e1 e5 | e2 e6 | e3 e7 (kMxSlot: slot j of a group of eight holds element kMxSlot[j]).
+// An E2M1 code s|ee|m placed as a bf16 with exponent field ee and top mantissa bit m IS the code's value times 2^-126
+// -- for ee = 0 a bf16 subnormal, m * 2^-127: the subnormal code 0.5 needs no special case -- so a code pair becomes
+// a bf16x2 with one mask, one integer multiply (x * (2^a + 2^b) = two shifted copies: exponent/mantissa and sign
+// each land on their bit positions) and one mask; the masks pick nibbles j and j+4 of the word, which lie exactly 16
+// bits apart: no shifts.  Then two exact bf16x2 multiplies: by 2^126, by the block scale.  Per word 9 logic
+// operations (ALU pipe) + 4 integer multiplies + 8 bf16x2 multiplies (FMA pipe); the byte-permute look-up it replaces
+// took 16 on the ALU pipe, which bounds this kernel (ncu: ALU 59 % busy at 1.6 TB/s, FMA 15 %).  The contraction does
+// not care about the order of its terms as long as BOTH operands use it: the activation rows are stored in the same
+// slot order (gather_x_kernel, the MODE 0 epilogue).
 __device__ __forceinline__ uint4 mx_decode8(uint32_t w, __nv_bfloat162 sc) {
-  constexpr uint32_t H0 = 0x3F3F3F00u, H1 = 0x40404040u;      // high bytes of the bf16 magnitudes of codes 0..7
-  constexpr uint32_t L0 = 0xC0800000u, L1 = 0xC0804000u;      // low bytes
-  const uint32_t m = w & 0x77777777u;
-  uint32_t hiA = __byte_perm(H0, H1, m), hiB = __byte_perm(H0, H1, m >> 16);
-  const uint32_t loA = __byte_perm(L0, L1, m), loB = __byte_perm(L0, L1, m >> 16);
-  const uint32_t sg = w & 0x88888888u, sg4 = sg << 4;         // sign of code 2k+1 / 2k at bit 7 of byte k
-  hiA |= __byte_perm(sg4, sg, 0x5140) & 0x80808080u;
-  hiB |= __byte_perm(sg4, sg, 0x7362) & 0x80808080u;
+  const uint32_t k126 = 0x7E807E80u;                          // bf16x2 (2^126, 2^126)
+  const __nv_bfloat162 c126 = *reinterpret_cast<const __nv_bfloat162*>(&k126);
+  const uint32_t w8 = w >> 8;
   uint32_t o[4];
-  o[0] = __byte_perm(loA, hiA, 0x5140);
-  o[1] = __byte_perm(loA, hiA, 0x7362);
-  o[2] = __byte_perm(loB, hiB, 0x5140);
-  o[3] = __byte_perm(loB, hiB, 0x7362);
+  o[0] = ((w & 0x000F000Fu) * 0x1040u) & 0x81C081C0u;         // nibbles 0, 4: value << 6, sign << 12
+  o[1] = ((w & 0x00F000F0u) * 0x0104u) & 0x81C081C0u;         // nibbles 1, 5: value << 2, sign << 8
+  o[2] = ((w8 & 0x000F000Fu) * 0x1040u) & 0x81C081C0u;        // nibbles 2, 6
+  o[3] = ((w8 & 0x00F000F0u) * 0x0104u) & 0x81C081C0u;        // nibbles 3, 7
 #pragma unroll
   for (int k = 0; k < 4; ++k) {
     __nv_bfloat162 v = *reinterpret_cast<__nv_bfloat162*>(&o[k]);
-    v = __hmul2(v, sc);
+    v = __hmul2(__hmul2(v, c126), sc);
     o[k] = *reinterpret_cast<uint32_t*>(&v);
   }
   return make_uint4(o[0], o[1], o[2], o[3]);
 }
+// slot of element e inside its group of eight (inverse of the slot order above)
+__host__ __device__ __forceinline__ int mx_slot_of(int e) { return (e & ~7) | ((e & 3) << 1) | ((e >> 2) & 1); }
 
 // Walks this CTA's (tile, pass, k-chunk) stages in the order every role uses.
 struct MxWalker {
@@ -288,7 +292,7 @@ ffn_mx_kernel(const __grid_constant__ CUtensorMap tm_codes, const __grid_constan
               const float gv = lo ? v[k] : recv;
               const float uv = lo ? recv : v[8 + k];
               const int tok = n0 + c0 + (lo ? k : 8 + k);
-              if (tok < wk.w) f.h_out[(size_t)(wk.z + tok) * f.I + i] = f32_to_bf16_rn(silu_f(gv) * uv);
+              if (tok < wk.w) f.h_out[(size_t)(wk.z + tok) * f.I + mx_slot_of(i)] = f32_to_bf16_rn(silu_f(gv) * uv);   // K-slot order of the w2 decode
             }
           } else {
             const int r = rt * 128 + 32 * qtr + lane;

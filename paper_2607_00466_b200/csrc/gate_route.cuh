@@ -436,10 +436,11 @@ __global__ void __launch_bounds__(256) gate_topk_route_kernel(GateRouteArgs a) {
 }
 
 // x_perm[row] = x[token of sorted pair row]  (rows >= T*k: plain copy of x for the shared experts)
+// slot_order != 0: elements permuted inside every group of eight for the MXFP4 decoder
 __global__ void __launch_bounds__(256) gather_x_kernel(const uint16_t* __restrict__ x,
                                                        const int32_t* __restrict__ perm,
                                                        uint16_t* __restrict__ x_perm, int T, int H, int k,
-                                                       int n_rows) {
+                                                       int n_rows, int slot_order) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int row = blockIdx.x * 8 + warp;
   pdl_launch_dependents();
@@ -448,7 +449,16 @@ __global__ void __launch_bounds__(256) gather_x_kernel(const uint16_t* __restric
   const int t = (row < T * k) ? perm[row] / k : row - T * k;
   const uint4* src = reinterpret_cast<const uint4*>(x + (size_t)t * H);
   uint4* dst = reinterpret_cast<uint4*>(x_perm + (size_t)row * H);
-  for (int c = lane; c < (H >> 3); c += 32) dst[c] = __ldg(src + c);
+  if (!slot_order) {
+    for (int c = lane; c < (H >> 3); c += 32) dst[c] = __ldg(src + c);
+  } else {
+    // MXFP4 path: every group of eight elements in the decoder's K-slot order e0 e4 e1 e5 e2 e6 e3 e7 (ffn_mx.cuh)
+    for (int c = lane; c < (H >> 3); c += 32) {
+      const uint4 v = __ldg(src + c);
+      dst[c] = make_uint4(__byte_perm(v.x, v.z, 0x5410), __byte_perm(v.x, v.z, 0x7632),
+                          __byte_perm(v.y, v.w, 0x5410), __byte_perm(v.y, v.w, 0x7632));
+    }
+  }
 }
 
 // --------------------------------------------------------------------------- a7: weighted combine

@@ -72,6 +72,8 @@ def run_mx(gpu, oracle, shape, T, seed, force=False, scale_lo=118, scale_hi=122,
                       dl.ws_view("perm", T).cpu().numpy(), pair_pos, dl.active.cpu().numpy(), int(dl.n_active.item()), op)
     if check_pairs:
         h_gpu = dl.ws_view("h", T).float().cpu().numpy()
+        # the MXFP4 step keeps h in the K-slot order of its decoder (e0 e4 e1 e5 e2 e6 e3 e7 per group of eight)
+        h_gpu = h_gpu.reshape(h_gpu.shape[0], -1, 8)[:, :, [0, 2, 4, 6, 1, 3, 5, 7]].reshape(h_gpu.shape)
         y_gpu = dl.ws_view("y", T).cpu().numpy()
         rows_g, rows_o = [], []
         for t in np.nonzero(clean)[0]:
