@@ -70,12 +70,14 @@ __host__ __device__ inline size_t mx_smem_bytes(int np, int stages, int raw_stag
 // -- for ee = 0 a bf16 subnormal, m * 2^-127: the subnormal code 0.5 needs no special case -- so a code pair becomes
 // a bf16x2 with one mask, one integer multiply (x * (2^a + 2^b) = two shifted copies: exponent/mantissa and sign
 // each land on their bit positions) and one mask; the masks pick nibbles j and j+4 of the word, which lie exactly 16
-// bits apart: no shifts.  Then two exact bf16x2 multiplies: by 2^126, by the block scale.  Per word 9 logic
-// operations (ALU pipe) + 4 integer multiplies + 8 bf16x2 multiplies (FMA pipe); the byte-permute look-up it replaces
+// bits apart: no shifts.  Then one exact bf16x2 multiply by 2^126 x the block scale.  Per word 9 logic
+// operations (ALU pipe) + 4 integer multiplies + 4 bf16x2 multiplies (FMA pipe); the byte-permute look-up it replaces
 // took 16 on the ALU pipe, which bounds this kernel (ncu: ALU 59 % busy at 1.6 TB/s, FMA 15 %).  The contraction does
 // not care about the order of its terms as long as BOTH operands use it: the activation rows are stored in the same
 // slot order (gather_x_kernel, the MODE 0 epilogue).
-__device__ __forceinline__ uint4 mx_decode8(uint32_t w, __nv_bfloat162 sc) {
+// `sc` = bf16x2 of 2^(b-1) (the 2^126 folded in) for scale bytes b <= 128; larger scales (`wide`, weights beyond 2^1 per
+// unit code: not seen in practice) take the two multiplies 2^126, 2^(b-127).
+__device__ __forceinline__ uint4 mx_decode8(uint32_t w, __nv_bfloat162 sc, bool wide) {
   const uint32_t k126 = 0x7E807E80u;                          // bf16x2 (2^126, 2^126)
   const __nv_bfloat162 c126 = *reinterpret_cast<const __nv_bfloat162*>(&k126);
   const uint32_t w8 = w >> 8;
@@ -87,7 +89,8 @@ __device__ __forceinline__ uint4 mx_decode8(uint32_t w, __nv_bfloat162 sc) {
 #pragma unroll
   for (int k = 0; k < 4; ++k) {
     __nv_bfloat162 v = *reinterpret_cast<__nv_bfloat162*>(&o[k]);
-    v = __hmul2(__hmul2(v, c126), sc);
+    if (wide) v = __hmul2(v, c126);
+    v = __hmul2(v, sc);
     o[k] = *reinterpret_cast<uint32_t*>(&v);
   }
   return make_uint4(o[0], o[1], o[2], o[3]);
@@ -387,7 +390,11 @@ ffn_mx_kernel(const __grid_constant__ CUtensorMap tm_codes, const __grid_constan
             if (sub < nsub) {
               const uint32_t sb = (sub < 2 ? sc_lo : sc_hi) >> (16 * (sub & 1));
               const uint32_t sbyte = (NW * part >= 4 ? (sb >> 8) : sb) & 0xffu;      // my codes lie in one 32-element block when NW <= 4
-              const uint32_t s0 = (sb & 0xffu) << 7, s1 = ((sb >> 8) & 0xffu) << 7, sm_ = sbyte << 7;
+              // multiplier bits: exponent field b + 126 (= 2^(b-1), the decode's 2^126 folded in) while that is a finite
+              // bf16, else b (= 2^(b-127)) and the decode multiplies by 2^126 itself
+              auto mul_bits = [](uint32_t b) -> uint32_t { return (b <= 128u ? b + 126u : b) << 7; };
+              const bool wide0 = (sb & 0xffu) > 128u, wide1 = ((sb >> 8) & 0xffu) > 128u, widem = sbyte > 128u;
+              const uint32_t s0 = mul_bits(sb & 0xffu), s1 = mul_bits((sb >> 8) & 0xffu), sm_ = mul_bits(sbyte);
               const uint32_t p0 = s0 | (s0 << 16), p1 = s1 | (s1 << 16), pm = sm_ | (sm_ << 16);
               const __nv_bfloat162 sc0 = *reinterpret_cast<const __nv_bfloat162*>(&p0);
               const __nv_bfloat162 sc1 = *reinterpret_cast<const __nv_bfloat162*>(&p1);
@@ -409,7 +416,8 @@ ffn_mx_kernel(const __grid_constant__ CUtensorMap tm_codes, const __grid_constan
               // decode into registers, then straight into this row's TMEM lane: 4 columns (8 bf16) per word
               uint4 o[NW];
 #pragma unroll
-              for (int i = 0; i < NW; ++i) o[i] = mx_decode8(wd[i], NW == 8 ? (i < 4 ? sc0 : sc1) : scm);
+              for (int i = 0; i < NW; ++i)
+                o[i] = mx_decode8(wd[i], NW == 8 ? (i < 4 ? sc0 : sc1) : scm, NW == 8 ? (i < 4 ? wide0 : wide1) : widem);
               mbar_wait(wempty_bar(ws_), wpar);
               tc_fence_after();
               const uint32_t a_addr = a_row0 + ws_ * 32u;

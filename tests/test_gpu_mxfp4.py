@@ -108,6 +108,13 @@ def test_mxfp4_scale_range_and_signs(gpu, oracle):
     run_mx(gpu, oracle, shape, 24, seed=77, scale_lo=87, scale_hi=107)
 
 
+def test_mxfp4_scales_around_and_above_one(gpu, oracle):
+    """Scale bytes 125..131 (2^-2 .. 2^4): the decoder folds its 2^126 into the block-scale multiplier while 2^(b-1) is a
+    finite bf16 (b <= 128) and multiplies twice above that -- both sides of the switch, mixed inside one row."""
+    shape = synth.MoEShape(hidden=128, inter=128, n_experts=4, top_k=2, n_layers=1)
+    run_mx(gpu, oracle, shape, 24, seed=78, scale_lo=125, scale_hi=131)
+
+
 def test_mxfp4_gpt_oss_shaped_layer(gpu, oracle):
     """GPT-OSS-120B-shaped experts (top-4, mxfp4; hidden = intermediate = 2880) with 16 of the 128 experts
     (the oracle's decoded copy of all 128 would take 6 GB): 45 k-chunks, 45 w1/w3 row tiles, 22.5 w2 row tiles."""
