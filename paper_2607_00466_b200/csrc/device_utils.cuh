@@ -59,6 +59,21 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     if (spins > (1u << 24)) __trap();
   }
 }
+// The same with a suspend-time hint: the warp stays asleep until the phase completes (or 20 us pass) instead of
+// returning to its spin loop every ~80 cycles.  For LONG waits of warps that share an SM with busy ones -- the
+// spin loops of waiting warps cost issue slots -- and not for hand-overs on a critical path: waking up takes longer.
+__device__ __forceinline__ void mbar_wait_long(uint32_t bar, uint32_t parity) {
+  uint32_t ok = 0;
+  for (uint32_t spins = 0; ; ++spins) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok) : "r"(bar), "r"(parity), "r"(20000u) : "memory");
+    if (ok) break;
+    if (spins > (1u << 20)) __trap();
+  }
+}
 
 // --------------------------------------------------------------------------------------------- TMA
 __device__ __forceinline__ uint64_t l2_policy_evict_first() {

@@ -1038,7 +1038,10 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
           const CUtensorMap* tmw = ph == 0 ? (shared ? &tm_sw13 : &tm_w13) : (shared ? &tm_sw2 : &tm_w2);
           for (int kc = p.k0; kc < p.k1; ++kc, ++it) {
             const int s = it % S;
-            FTIMED(w_wait[ph], mbar_wait(empty_bar(s), ((it / S) & 1) ^ 1));
+            // suspended wait (try_wait with a time hint: the lane sleeps until a slot is free instead of re-polling the
+            // barrier every ~80 cycles).  Measured: |U| = 128 197.7 -> 193.7 us, 64: 111.2 -> 108.6, T = 256 91.1 -> 92.5.
+            // (The same wait selected by a run-time branch between the two loops cost 8 %: |U| = 128 213 us.)
+            FTIMED(w_wait[ph], mbar_wait_long(empty_bar(s), ((it / S) & 1) ^ 1));
 #ifdef ELDR_TRACE
             const long long cw_ = clock64();
 #endif
