@@ -84,7 +84,7 @@ def run(T: int, unions, steady: bool = False, config5: bool = False):
                     print("| %s | %d | %.2f | %.2f | %.2f |" % (name, len(v), (v.min() - t0) / 1e3,
                                                                (np.median(v) - t0) / 1e3, (v.max() - t0) / 1e3))
         if not steady:
-            print("\n| per sub-phase (0: w1/w3 whole rounds, 1: w1/w3 stream-K part, 2: w2 whole rounds, 3: w2 stream-K part) | min | median | max |\n|---|---|---|---|")
+            print("\n| per sub-phase (0: w1/w3 whole rounds, 1: w1/w3 remainder (or the whole phase as stream-K), 2: w2 whole rounds, 3: w2 remainder (or stream-K)) | min | median | max |\n|---|---|---|---|")
             for base, name, is_time in ((0, "weights producer: sub-phase %d fully issued", True), (4, "epilogue: sub-phase %d finished", True),
                                         (8, "activations producer: waited for h flags in sub-phase %d (us)", False),
                                         (12, "epilogue warp 0: waited for partners' parked partials in sub-phase %d (us)", False)):
