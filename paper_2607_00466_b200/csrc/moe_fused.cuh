@@ -2,38 +2,38 @@
 // "the gate partitions the batch among experts ... each step fetches the weights of every expert the batch
 // activates"; PAPER.md:198/:253 signature counts).  One CTA per SM, 8 warps.
 //
-//   G  gate GEMV: 8-token x 8-expert logit tiles spread over the grid.  fp32 FMA on CUDA cores; a warp owns
-//      2 experts x 4 tokens (halves the shared-memory traffic of 1 x 8), gate rows are requested 8 float4 deep
-//      per row BEFORE the x tile is staged so both latencies overlap.  Each tile publishes an epoch flag.
+//   G  gate GEMV: GT-token x 8-expert logit tiles spread over the grid (GT = 8 / 16 / 32 for T <= 64 / 128 / 256: one
+//      round of tiles).  fp32 FMA on CUDA cores; a warp owns 2 experts x GT/2 tokens, gate rows are requested 8 float4
+//      deep per row BEFORE the x tile is staged so both latencies overlap.  Each tile publishes an epoch flag.
 //   K  top-k: the CTA that owns token group g polls the group's tile flags, runs a redux-based warp top-k
-//      (+ fused signature increments), publishes the group flag.
-//   R  routing, redundantly in EVERY CTA from the 4*T*k bytes of ids: membership bitmasks -> counts ->
-//      offsets -> union-compacted work list (the weights producer starts streaming here) -> token<->position
+//      (+ fused signature increments) and publishes ids and weights as epoch-tagged 64-bit words.
+//   R  routing, redundantly in EVERY CTA from the tagged ids: membership bitmasks -> counts -> offsets ->
+//      union-compacted work list (shared experts first; the weights producer starts streaming here) -> token<->position
 //      maps, all in shared memory.  No second election, no route/gather kernels, no work list in HBM.
 //      CTA 0 also writes the routing outputs of the C ABI (active list, n_active, cnt/off/perm/pair_pos).
 //   F  expert FFN on tcgen05 + TMEM, swap-AB (weights = M=128 operand, the expert's tokens = N operand).  Per
-//      phase (A: w1/w3 tiles, B: w2 tiles) the tile list is entry-major (experts in order).  HYBRID schedule:
-//      whole rounds of gridDim.x tiles are "data-parallel" -- never split, drawn tile by tile from a global counter
-//      by each CTA's weights producer (SMs get unequal shares of a saturated HBM, so fast SMs draw more) -- and the
-//      remaining < gridDim.x tiles (or the whole phase when it has fewer than `dp_min_rounds` rounds) are a STATIC
-//      stream-K schedule: the flattened sequence of 16 KiB weight stages (tile-major, k-chunk minor) is cut into
-//      gridDim.x equal contiguous ranges.  A tile cut by a range boundary is finished by the CTA that owns its k=0
-//      end: the other owner(s) -- which reach the tile FIRST, at the start of their range -- park raw fp32
-//      accumulators in a scratch slot and raise a flag; the head owner adds them in ascending CTA order (a fixed
-//      order: results are run-to-run bit-identical whichever CTA computed a whole tile).  Weights: TMA
+//      phase (A: w1/w3 tiles, B: w2 tiles) the tile list is entry-major.  Schedule (PieceWalker, below): a phase with
+//      at least one round of gridDim.x tiles runs WHOLE tiles -- CTA c's first tile is tile c, further ones are drawn
+//      from a global counter by its weights producer (SMs get unequal shares of a saturated HBM, so fast SMs draw
+//      more), the tiles past the last whole round go whole to as many CTAs while the others move on; a phase shorter
+//      than one round is a STATIC stream-K schedule: the flattened sequence of 16 KiB weight stages (tile-major,
+//      k-chunk minor) is cut into gridDim.x equal contiguous ranges.  A tile cut by a range boundary is finished by the
+//      CTA that owns its k=0 end: the other owner(s) -- which reach the tile FIRST, at the start of their range -- park
+//      raw fp32 accumulators in a scratch slot and raise a flag; the head owner adds them in ascending CTA order (a
+//      fixed order: results are run-to-run bit-identical whichever CTA computed a whole tile).  Weights: TMA
 //      (SWIZZLE_128B, evict_first).  Activations: TMA too -- tile::gather4 pulls the expert's token rows straight
-//      from x (A), 16-row boxes read h (B) -- into the swizzled K-major B tile; the permutation never exists in
-//      HBM.  Phase B waits on per-tile epoch flags of the expert's h tiles (release/acquire through L2, proxy
-//      fences around the TMA reads).  Phase A never waits on phase B and first pieces never wait on anything, so
-//      there is no cycle.  Because data-parallel tiles finish in expert order, B's first rounds find their h
-//      long finished: no pipeline drain at the hand-over when the union is large.
+//      from x (A; wide batches: 16-row boxes of an expert-sorted copy of x written at the start of the phase), 16-row
+//      boxes read h (B) -- into the swizzled K-major B tile.  Phase B waits on per-tile epoch flags of the expert's h
+//      tiles (release/acquire through L2, proxy fences around the TMA reads).  Phase A never waits on phase B and first
+//      pieces never wait on anything, so there is no cycle.  Because whole tiles finish in work-list order, B's first
+//      rounds find their h long finished: no pipeline drain at the hand-over when the union is large.
 //      The B-tile rows per stage adapt to the batch's largest tokens-per-expert count, so small-m steps get a
 //      deeper weight ring (more bytes in flight).
-//   C  ordered combine after a flag barrier over the grid: out[t] = sum_j w[t,j]*y[pos(t,j)] (+ shared) in
-//      slot order, one RNE rounding to bf16.
+//   C  flag-driven ordered combine (no grid barrier): out[t] = sum_j w[t,j]*y[pos(t,j)] (+ shared) in slot order, one
+//      RNE rounding to bf16, each (token, 128-column tile) as soon as its y tiles are flagged.
 //
 // Nothing needs zeroing by the host: flags compare against epoch = gen+1; gen lives in the workspace and is
-// bumped by CTA 0 after the last barrier (the launch is CUDA-graph capturable; a workspace of arbitrary initial
+// bumped by the last CTA to leave the step (the launch is CUDA-graph capturable; a workspace of arbitrary initial
 // contents works up to a 2^-32 flag collision).
 #pragma once
 #include "device_utils.cuh"
