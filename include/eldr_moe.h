@@ -290,6 +290,9 @@ int32_t eldr_moe_workspace_layout(const eldr_moe_shape_t* shape, int32_t T, eldr
                                  is cut over at most this many CTAs per tile; the other CTAs go straight on to the next part.
                                  0 = over the whole grid (round 1).  0..64; default 1 = whole tiles (|U| = 128: 205.8 us at 0,
                                  203.9 at 2, 197.3 at 1; config-5 shape 221.9 / 215.5 / 216.5) */
+#define ELDR_OPT_GATE_TC 11    /* prefill-shaped gate (T >= 2048, hidden % 64 == 0): 1 (default) = on the tensor cores with every fp32
+                                 gate weight as the exact sum of three bf16 terms and 256-wide K slices summed in fp32 (same
+                                 1e-5 logit gate as the CUDA-core kernels); 0 = the register-tiled fp32 CUDA-core GEMM */
 #define ELDR_OPT_XS_MIN_NP 9  /* fused step: when some expert receives at least this many tokens (padded to 16) the w1/w3 phase reads
                                  its activations from an expert-sorted copy of x written inside the step (16 rows per TMA
                                  instruction) instead of gathering token rows from x (4 rows per instruction) for every stage;

@@ -36,6 +36,7 @@ OPT_COOPERATIVE = 7
 OPT_HEAD_FIRST = 8
 OPT_XS_MIN_NP = 9
 OPT_SK_MAX_SPLIT = 10
+OPT_GATE_TC = 11
 PROFILE_SLOTS = ("gate", "route", "gather", "ffn13", "ffn2", "combine")
 
 

@@ -18,6 +18,7 @@
 #include "fit_host.cuh"
 #include "gate_route.cuh"
 #include "gate_prefill.cuh"
+#include "gate_tc.cuh"
 #include "moe_fused.cuh"
 #include "route_decide.cuh"
 #include "route_prefill.cuh"
@@ -38,6 +39,7 @@ std::atomic<int> g_sk_split_pct{0};
 std::atomic<int> g_coop{1};
 std::atomic<int> g_head_first{0};
 std::atomic<int> g_xs_min_np{48};
+std::atomic<int> g_gate_tc{1};
 std::atomic<int> g_sk_max_split{1};
 
 // Scratch of eldr_moe_gate_topk_static (the entry point that allocates nothing): the gate logits z [T,E] fp32.  File
@@ -148,7 +150,7 @@ void make_host_stage(const eldr_moe_shape_t* s, int T, size_t base, HostStage* S
 // grid are properties of the device the call runs on, so everything cached here is keyed by the device ordinal.
 constexpr int kMaxDevices = 64;
 enum { kAttrFused = 0, kAttrRouteBig, kAttrUmma, kAttrPair, kAttrStream, kAttrRouteSims, kAttrGateLogits, kAttrGateRoute,
-       kAttrRouteOnly, kAttrMx, kAttrSigLayers, kAttrGemv, kAttrCount };
+       kAttrRouteOnly, kAttrMx, kAttrSigLayers, kAttrGemv, kAttrGateTc, kAttrCount };
 struct DevState {
   std::atomic<int> sms{0};
   std::atomic<int> fused_ok{-1};          // -1 unknown, 0 the persistent grid cannot be co-resident, 1 it can
@@ -400,6 +402,25 @@ int32_t launch_gate_logits(const eldr_moe_shape_t* s, int T, const eldr_bf16* x,
 // a1-a3 as separate launches (eldr_moe_gate_topk and the prefill-shaped layer): logits, then warp top-k + signature.
 int32_t launch_gate_topk(const eldr_moe_shape_t* s, int T, const eldr_bf16* x, const float* gate_w,
                          const float* gate_bias, float* z, size_t z_bytes, const TopkArgs& a, cudaStream_t st) {
+  // prefill-shaped, H a multiple of 64: the tensor-core gate (three exact bf16 terms per fp32 weight, 256-wide K slices
+  // summed in fp32: gate_tc.cuh); the three-term split of the weights lives behind z in the workspace
+  const size_t z_sz = align_up((size_t)T * s->n_experts * 4, 1024);
+  const size_t split_sz = (size_t)3 * s->n_experts * s->hidden * 2;
+  if (g_gate_tc.load() && T >= 2048 && s->hidden % 64 == 0 && z_bytes >= z_sz + split_sz) {
+    uint16_t* wsplit = reinterpret_cast<uint16_t*>(reinterpret_cast<uint8_t*>(z) + z_sz);
+    const int n = s->n_experts * s->hidden;
+    gate_split_kernel<<<(n + 255) / 256, 256, 0, st>>>(gate_w, wsplit, n);
+    if (!launch_ok("gate_split_kernel")) return ELDR_ERR_CUDA;
+    CUtensorMap tm_x, tm_w;
+    if (!make_tmap(&tm_x, x, (uint64_t)T, s->hidden, kGtcTok)) return ELDR_ERR_CUDA;
+    if (!make_tmap(&tm_w, wsplit, (uint64_t)3 * s->n_experts, s->hidden, kGtcExp)) return ELDR_ERR_CUDA;
+    if (!once_per_device(kAttrGateTc, [] { return set_smem(gate_logits_tc_kernel, kGtcSmemBytes); })) return ELDR_ERR_CUDA;
+    launch_dep(gate_logits_tc_kernel, dim3((s->n_experts + kGtcExp - 1) / kGtcExp, (T + kGtcTok - 1) / kGtcTok), dim3(kGtcThreads),
+               (size_t)kGtcSmemBytes, st, tm_x, tm_w, gate_bias, z, T, s->hidden, s->n_experts);
+    if (!launch_ok("gate_logits_tc_kernel")) return ELDR_ERR_CUDA;
+    topk_kernel<<<(T + 7) / 8, 256, 0, st>>>(a);
+    return launch_ok("topk_kernel") ? ELDR_OK : ELDR_ERR_CUDA;
+  }
   const int S = gate_slices(s, T);
   if (S > 0 && z_bytes >= (size_t)S * T * s->n_experts * 4) {
     // prefill-shaped: register-tiled fp32 GEMM, split-K into the fewest slices of at most 256 h (accuracy, see
@@ -473,6 +494,10 @@ int32_t eldr_moe_set_option(int32_t key, int32_t value) {
   }
   if (key == ELDR_OPT_SK_MAX_SPLIT && value >= 0 && value <= 64) {
     g_sk_max_split = value;
+    return ELDR_OK;
+  }
+  if (key == ELDR_OPT_GATE_TC && (value == 0 || value == 1)) {
+    g_gate_tc = value;
     return ELDR_OK;
   }
   if (key == ELDR_OPT_XS_MIN_NP && value >= 16 && value <= 144) {

@@ -122,6 +122,7 @@ def test_tuning_options_validate_their_values(lib):
                            (api.OPT_RING_KB, [32, 208], [31, 209]),
                            (api.OPT_DP_MIN_ROUNDS, [4, 1], [0]),
                            (api.OPT_SK_MAX_SPLIT, [0, 3, 1], [-1, 65]),
+                           (api.OPT_GATE_TC, [0, 1], [-1, 2]),
                            (api.OPT_XS_MIN_NP, [16, 144, 48], [15, 145]),
                            (api.OPT_SK_SPLIT_PCT, [60, 0], [-1, 101]),
                            (api.OPT_COOPERATIVE, [0, 1], [-1, 2]),

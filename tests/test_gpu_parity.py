@@ -646,10 +646,22 @@ def test_invalid_option_values_are_rejected(gpu):
 
 @pytest.mark.parametrize("H,E,k,T,big_ws", [(2048, 128, 8, 4096, True), (2048, 128, 8, 2100, False), (320, 130, 3, 2050, True),
                                             (64, 10, 2, 2049, True), (1408, 64, 6, 3001, True)])
-def test_gate_prefill_tiled_gemm(gpu, oracle, H, E, k, T, big_ws):
-    """eldr_moe_gate_topk at prefill-shaped T (>= 2048 tokens takes the register-tiled fp32 GEMM with split-K):
+@pytest.mark.parametrize("tc", [1, 0])
+def test_gate_prefill_tiled_gemm(gpu, oracle, H, E, k, T, big_ws, tc):
+    """eldr_moe_gate_topk at prefill-shaped T (>= 2048 tokens): the tensor-core gate (every fp32 weight as three exact
+    bf16 terms, 256-wide K slices summed in fp32; ELDR_OPT_GATE_TC = 1, the default, when H % 64 == 0 and the workspace
+    holds the split weights) and the register-tiled fp32 CUDA-core GEMM with split-K (ELDR_OPT_GATE_TC = 0):
     logits within 1e-5 of the fp64 oracle, ids / weights / signatures through the same gates as the decode path;
     ragged T, E and H, with a gate bias, with a workspace that only fits one K slice, and run-to-run bit-identical."""
+    import torch
+    gpu.eldr_moe_set_option(gpu.OPT_GATE_TC, tc)
+    try:
+        _gate_prefill_case(gpu, oracle, H, E, k, T, big_ws, 3 if (tc and big_ws and H % 64 == 0) else 2)
+    finally:
+        gpu.eldr_moe_set_option(gpu.OPT_GATE_TC, 1)
+
+
+def _gate_prefill_case(gpu, oracle, H, E, k, T, big_ws, want_launches):
     import torch
     shape = synth.MoEShape(hidden=H, inter=64, n_experts=E, top_k=k, n_layers=1)
     gate_w = synth.make_gate_w(shape, 17)
@@ -665,7 +677,7 @@ def test_gate_prefill_tiled_gemm(gpu, oracle, H, E, k, T, big_ws):
             token_req, None, sig_req, None, ws)
     gpu.eldr_moe_gate_topk(*args)
     torch.cuda.synchronize()
-    assert gpu.eldr_moe_last_launch_count() == 2
+    assert gpu.eldr_moe_last_launch_count() == want_launches
     ora = oracle.gate_topk(shape, x_bits, gate_w, bias)
     z = ws[: T * E * 4].view(torch.float32).reshape(T, E).cpu().numpy().astype(np.float64)
     assert np.abs(z - ora["z"]).max() <= 1e-5
@@ -697,7 +709,8 @@ def test_prefill_shaped_layer_ragged(gpu, oracle, H, I, E, k, T, ns):
     n_blk = int(token_block.max()) + 1
     r = run_case(gpu, oracle, shape, lw, x, None, token_req, token_block, n_req=n_req, n_blk=n_blk, layer=1)
     assert r["n_active"] == len(np.unique(r["ids"]))
-    assert gpu.eldr_moe_last_launch_count() == 8             # logits, top-k, count, scatter, gather, w1/w3, w2, combine
+    # logits, top-k, count, scatter, gather, w1/w3, w2, combine (+ the gate-weight split of the tensor-core gate: T >= 2048, H % 64 == 0)
+    assert gpu.eldr_moe_last_launch_count() == (9 if (T >= 2048 and H % 64 == 0) else 8)
 
 
 @pytest.mark.gpu
@@ -737,7 +750,7 @@ def test_prefill_shaped_graph_capture(gpu, oracle):
     dl = gpu.DecodeLayer(shape, lw, max_T=T)
     ref = dl.run(x, None).clone()
     torch.cuda.synchronize()
-    assert gpu.eldr_moe_last_launch_count() == 8
+    assert gpu.eldr_moe_last_launch_count() == 9     # split, logits, top-k, count, scatter, gather, w1/w3, w2, combine
     side = torch.cuda.Stream()
     side.wait_stream(torch.cuda.current_stream())
     with torch.cuda.stream(side):
@@ -777,7 +790,7 @@ def test_prefill_shaped_layer_c5_shape_2048(gpu, oracle):
     try:
         r = run_case(gpu, oracle, shape, lw, x, check_pairs=False)
         assert r["n_active"] == shape.n_experts
-        assert gpu.eldr_moe_last_launch_count() == 8
+        assert gpu.eldr_moe_last_launch_count() == 9
     finally:
         gpu.eldr_moe_set_option(gpu.OPT_FFN_PAIR, 1)
 
