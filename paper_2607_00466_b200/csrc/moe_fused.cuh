@@ -1111,6 +1111,34 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
       while (consumer_next(pw, p, cn)) {
         const int4 wk = sm.work[p.ent];
         if (ph == 0 && use_xs && !xs_ready) {
+          // The sorted copy takes ~3 us to appear (every CTA's part, flagged).  The head of this CTA's FIRST piece --
+          // one ring's worth of stages -- is gathered from x as in the narrow case, so the MMAs start while the copy is
+          // still being written; then the flags are awaited once and the piece goes on in the regular loop below.
+          // (A loop of its own: the regular per-stage loop is sensitive to every instruction added to it.)
+          const int n0h = p.pass * kNPCap;
+          const int n_hh = min(kNPCap, wk.w - n0h);
+          const int n_padh = (n_hh + 15) & ~15;
+          int g0 = 0, g1 = 0, g2 = 0, g3 = 0;
+          if (4 * lane < n_padh) {
+            const uint16_t* tp = sm.tok_of_pos + wk.y + n0h;
+            g0 = tp[min(4 * lane, n_hh - 1)];
+            g1 = tp[min(4 * lane + 1, n_hh - 1)];
+            g2 = tp[min(4 * lane + 2, n_hh - 1)];
+            g3 = tp[min(4 * lane + 3, n_hh - 1)];
+          }
+          const int k_head = min(p.k1, p.k0 + S);
+          for (int kc = p.k0; kc < k_head; ++kc, ++it) {
+            if ((it & 1u) != xw) continue;
+            const int s = it % S;
+            if (lane == 0) {
+              mbar_wait(empty_bar(s), ((it / S) & 1) ^ 1);
+              mbar_arrive_expect_tx(full_bar(s), (uint32_t)n_padh * 128u);
+            }
+            __syncwarp();
+            if (4 * lane < n_padh)
+              tma_gather4(sm.stage_base + s * stage_bytes + kUmmaWBytes + lane * 512, &tm_x, kc * 64, g0, g1, g2, g3, full_bar(s), xpol);
+          }
+          p.k0 = k_head;
           warp_wait_flags(a.sync + kSyncXReady, G, epoch, lane);
           fence_proxy_async_all();
           __syncwarp();
