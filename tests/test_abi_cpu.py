@@ -132,3 +132,16 @@ def test_tuning_options_validate_their_values(lib):
         for v in good:                      # the last one is the default
             assert set_opt(C.c_int32(key), C.c_int32(v)) == 0
     assert set_opt(C.c_int32(99), C.c_int32(0)) == -1
+
+
+def test_option_keys_are_unique_and_mirrored_in_the_binding(lib):
+    """Every ELDR_OPT_* key of include/eldr_moe.h is a distinct integer and the Python binding carries the same value
+    under the same name (two knobs sharing a key would silently set each other)."""
+    import os, re
+    api, _ = lib
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    text = open(os.path.join(root, "include", "eldr_moe.h")).read()
+    keys = {m.group(1): int(m.group(2)) for m in re.finditer(r"#define\s+ELDR_OPT_(\w+)\s+(\d+)", text)}
+    assert len(keys) >= 10 and len(set(keys.values())) == len(keys), keys
+    for name, value in keys.items():
+        assert getattr(api, "OPT_" + name) == value, name
