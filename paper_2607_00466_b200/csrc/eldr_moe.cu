@@ -1081,8 +1081,17 @@ int32_t eldr_moe_decode_layer_host(const eldr_moe_shape_t* s, int32_t layer, int
   int32_t* d_req = static_cast<int32_t*>(mapped(h_token_req));
   int32_t* d_blk = static_cast<int32_t*>(mapped(h_token_block));
   eldr_bf16* d_out = static_cast<eldr_bf16*>(mapped(h_out));
-  int32_t* d_ids = nullptr;      // ids / weights are read back by the step's own kernels (routing, combine): they
-  float* d_w = nullptr;          // stay in device memory and are copied out
+  // ids / weights: the staged kernels read them back (routing, combine), so there they stay in device memory and a
+  // small block mirrors them into the mapped buffers; the one-launch step never reads them back (its CTAs route from
+  // the tagged words in the workspace), so when that is the path this call is expected to take its top-k owners write
+  // them straight through the mapping and the mirror launch is dropped.  (If the launch falls back to the staged
+  // kernels after all -- the grid cannot be co-resident -- those read the mapped memory: slower, still correct.)
+  const int sp_ = g_step_path.load();
+  const bool expect_fused = (sp_ == ELDR_STEP_FUSED || sp_ == ELDR_STEP_AUTO) && g_ffn_path.load() == ELDR_FFN_TCGEN05 &&
+                            s->hidden % 64 == 0 && s->inter % 64 == 0 && T <= kFusedMaxT && num_sms() <= 256 &&
+                            g_dev[current_device()].fused_ok.load(std::memory_order_relaxed) == 1;
+  int32_t* d_ids = expect_fused ? static_cast<int32_t*>(mapped(h_topk_ids)) : nullptr;
+  float* d_w = expect_fused ? static_cast<float*>(mapped(h_topk_w)) : nullptr;
   int32_t* d_na = static_cast<int32_t*>(mapped(h_n_active));
   if (!cuda_ok(cudaMemcpyAsync(ws + S.x, h_x, (size_t)T * H * 2, cudaMemcpyHostToDevice, st), "H2D x")) return ELDR_ERR_CUDA;
   if (h_token_req && !d_req) {
@@ -1102,15 +1111,15 @@ int32_t eldr_moe_decode_layer_host(const eldr_moe_shape_t* s, int32_t layer, int
                              d_req, d_blk, sig_req, sig_block, workspace, L.total, stream);
   if (rc != ELDR_OK) return rc;
   if (!d_out && !cuda_ok(cudaMemcpyAsync(h_out, ws + S.out, (size_t)T * H * 2, cudaMemcpyDeviceToHost, st), "D2H out")) return ELDR_ERR_CUDA;
-  int32_t* m_ids = static_cast<int32_t*>(mapped(h_topk_ids));
-  float* m_w = static_cast<float*>(mapped(h_topk_w));
+  int32_t* m_ids = d_ids ? nullptr : static_cast<int32_t*>(mapped(h_topk_ids));
+  float* m_w = d_w ? nullptr : static_cast<float*>(mapped(h_topk_w));
   if (m_ids || m_w) {
     mirror_to_host_kernel<<<1, 256, 0, st>>>(reinterpret_cast<const int32_t*>(ws + S.ids), m_ids,
                                              reinterpret_cast<const float*>(ws + S.w), m_w, (int)(T * k));
     if (!cuda_ok(cudaGetLastError(), "mirror_to_host_kernel")) return ELDR_ERR_CUDA;
   }
-  if (h_topk_ids && !m_ids && !cuda_ok(cudaMemcpyAsync(h_topk_ids, ws + S.ids, (size_t)T * k * 4, cudaMemcpyDeviceToHost, st), "D2H ids")) return ELDR_ERR_CUDA;
-  if (h_topk_w && !m_w && !cuda_ok(cudaMemcpyAsync(h_topk_w, ws + S.w, (size_t)T * k * 4, cudaMemcpyDeviceToHost, st), "D2H w")) return ELDR_ERR_CUDA;
+  if (h_topk_ids && !m_ids && !d_ids && !cuda_ok(cudaMemcpyAsync(h_topk_ids, ws + S.ids, (size_t)T * k * 4, cudaMemcpyDeviceToHost, st), "D2H ids")) return ELDR_ERR_CUDA;
+  if (h_topk_w && !m_w && !d_w && !cuda_ok(cudaMemcpyAsync(h_topk_w, ws + S.w, (size_t)T * k * 4, cudaMemcpyDeviceToHost, st), "D2H w")) return ELDR_ERR_CUDA;
   if (h_n_active && !d_na && !cuda_ok(cudaMemcpyAsync(h_n_active, ws + S.n_active, 4, cudaMemcpyDeviceToHost, st), "D2H n_active")) return ELDR_ERR_CUDA;
   if (!cuda_ok(cudaStreamSynchronize(st), "stream sync")) return ELDR_ERR_CUDA;
   return ELDR_OK;
