@@ -251,6 +251,13 @@ int32_t eldr_fit_kmeans_balanced(const double* h_sig, int32_t N, int32_t d, int3
                                  const int32_t* h_init_idx, int32_t max_iter,
                                  double* h_centroids, int32_t* h_assign, int32_t* h_steps, double* h_total);
 
+/* Workspace: device memory owned by the caller, 16-byte aligned, at least the number of bytes returned here; one
+ * workspace serves one call at a time (calls that overlap on the GPU need their own).  It carries state between calls:
+ * its first word is the generation of the epoch flags the kernels of a step wait on.  RECOMMENDED: zero the workspace
+ * once after allocating it (cudaMemsetAsync).  It is not required: the epoch of a step is a full-period 32-bit sequence
+ * state XOR a salt derived from the workspace address, so the stale bytes of a recycled allocation pass for a raised flag
+ * only with probability ~ (distinct stale words) / 2^32 on the first step.  Do not copy a live workspace to another
+ * address and continue there. */
 size_t  eldr_moe_workspace_bytes(const eldr_moe_shape_t* shape, int32_t max_T);
 size_t  eldr_moe_workspace_bytes_host(const eldr_moe_shape_t* shape, int32_t max_T);
 int32_t eldr_moe_workspace_layout(const eldr_moe_shape_t* shape, int32_t T, eldr_moe_ws_layout_t* layout);

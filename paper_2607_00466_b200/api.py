@@ -282,7 +282,7 @@ class DecodeLayer:
         self.shared_w13 = bf16_from_bits(lw.shared_w13, device) if lw.shared_w13 is not None else None
         self.shared_w2 = bf16_from_bits(lw.shared_w2, device) if lw.shared_w2 is not None else None
         self.max_T = max_T
-        self.workspace = torch.empty(eldr_moe_workspace_bytes_host(shape, max_T), dtype=torch.uint8, device=device)
+        self.workspace = torch.zeros(eldr_moe_workspace_bytes_host(shape, max_T), dtype=torch.uint8, device=device)   # zeroed once (include/eldr_moe.h: recommended)
         E, k, H = shape.n_experts, shape.top_k, shape.hidden
         self.out = torch.empty((max_T, H), dtype=torch.bfloat16, device=device)
         self.ids = torch.empty((max_T, k), dtype=torch.int32, device=device)
@@ -373,7 +373,7 @@ class MxDecodeLayer:
         self.w13_codes, self.w13_scales = (torch.from_numpy(np.ascontiguousarray(a)).to(device) for a in w13)
         self.w2_codes, self.w2_scales = (torch.from_numpy(np.ascontiguousarray(a)).to(device) for a in w2)
         self.max_T = max_T
-        self.workspace = torch.empty(eldr_moe_workspace_bytes(shape, max_T), dtype=torch.uint8, device=device)
+        self.workspace = torch.zeros(eldr_moe_workspace_bytes(shape, max_T), dtype=torch.uint8, device=device)
         E, k, H = shape.n_experts, shape.top_k, shape.hidden
         self.out = torch.empty((max_T, H), dtype=torch.bfloat16, device=device)
         self.ids = torch.empty((max_T, k), dtype=torch.int32, device=device)

@@ -75,6 +75,20 @@ __device__ __forceinline__ void mbar_wait_long(uint32_t bar, uint32_t parity) {
   }
 }
 
+// ------------------------------------------------------------------------------------- step epochs
+// Every flag a step waits for is compared with the step's EPOCH.  The workspace's first word holds a generation state
+// that walks a full-period 32-bit sequence (one step per call); the epoch is that state XOR a salt derived from the
+// workspace ADDRESS.  Why not simply generation + 1: a workspace handed out by a caching allocator holds the stale flags
+// of whatever workspace lived in that memory before -- at other offsets -- and with small consecutive epochs a stale
+// word equal to the new epoch is likely (found by a fuzz run: about one freshly allocated workspace in a hundred
+// produced garbage on its first step).  With the salt a stale word of another workspace matches with probability
+// (distinct stale values) / 2^32; stale words of the SAME workspace are older states of the same sequence and never
+// match.  (Callers who zero the workspace once after allocating it do not depend on any of this.)
+__device__ __forceinline__ uint32_t epoch_next_state(uint32_t state) { return state * 747796405u + 2891336453u; }
+__device__ __forceinline__ uint32_t epoch_of_state(uint32_t state, const void* ws_sync) {
+  return state ^ ((uint32_t)(reinterpret_cast<uintptr_t>(ws_sync) >> 4) * 0x9E3779B1u);
+}
+
 // --------------------------------------------------------------------------------------------- TMA
 __device__ __forceinline__ uint64_t l2_policy_evict_first() {
   uint64_t p;

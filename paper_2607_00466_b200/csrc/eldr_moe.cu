@@ -291,7 +291,9 @@ bool make_tmap_u8(CUtensorMap* out, const void* ptr, uint64_t rows, uint64_t row
 // w13 [n_exp, 2I, H] viewed as 5-D (col, row-in-16, branch{w1,w3}, 16-row group, expert) so that ONE box of
 // (64 cols, 16 rows, 2 branches, 4 groups) lands in shared memory as 4 x [16 rows of w1 | same 16 rows of w3].
 bool make_tmap_w13_5d(CUtensorMap* out, const void* ptr, uint64_t n_exp, uint64_t I, uint64_t H) {
-  const TmapKey key{ptr, n_exp * 2 * I, H, 16, 5, current_device()};
+  // (I is part of the key: two weight tensors of the same total row count and different I that the allocator placed at
+  // the same address -- one freed, the next allocated -- must not share a descriptor: found by a fuzz run)
+  const TmapKey key{ptr, n_exp * 2 * I, H | (I << 32), 16, 5, current_device()};
   if (tmap_lookup(key, out)) return true;
   encode_tiled_fn fn = get_encode_fn();
   if (!fn) { snprintf(g_err, sizeof(g_err), "cuTensorMapEncodeTiled entry point not found"); return false; }

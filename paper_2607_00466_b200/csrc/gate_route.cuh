@@ -402,7 +402,8 @@ __global__ void __launch_bounds__(256) gate_topk_route_kernel(GateRouteArgs a) {
   const int n_etiles = gridDim.x, n_groups = gridDim.y;
   ELDR_STAMP(0);
   pdl_launch_dependents();
-  const uint32_t epoch = ld_volatile_u32(a.sync) + 1u;
+  const uint32_t gen_next = epoch_next_state(ld_volatile_u32(a.sync));
+  const uint32_t epoch = epoch_of_state(gen_next, a.sync);
   gate_tile(a.x, a.gate_w, a.gate_bias, const_cast<float*>(tk.z), T, a.r.H, E, smem_raw);
   ELDR_STAMP(2);
 
@@ -431,7 +432,7 @@ __global__ void __launch_bounds__(256) gate_topk_route_kernel(GateRouteArgs a) {
   if (!publish_and_elect(group_flags, n_groups, g, elected2, epoch, &s_flag)) return;
   ELDR_STAMP(5);
   route_phases(a.r, smem_raw, 256, false);
-  if (threadIdx.x == 0) st_volatile_u32(a.sync, epoch);
+  if (threadIdx.x == 0) st_volatile_u32(a.sync, gen_next);
   ELDR_STAMP(10);
 }
 

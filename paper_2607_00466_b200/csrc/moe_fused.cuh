@@ -32,7 +32,8 @@
 //   C  flag-driven ordered combine (no grid barrier): out[t] = sum_j w[t,j]*y[pos(t,j)] (+ shared) in slot order, one
 //      RNE rounding to bf16, each (token, 128-column tile) as soon as its y tiles are flagged.
 //
-// Nothing needs zeroing by the host: flags compare against epoch = gen+1; gen lives in the workspace and is
+// Nothing needs zeroing by the host: flags compare against the step's epoch (device_utils.cuh: a full-period sequence
+// state kept in the workspace, salted with the workspace address); the state lives in the workspace and is
 // bumped by the last CTA to leave the step (the launch is CUDA-graph capturable; a workspace of arbitrary initial
 // contents works up to a 2^-32 flag collision).
 #pragma once
@@ -869,7 +870,8 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
   pdl_wait();
   if (tid == 0) FSTAMP(1);
 
-  const uint32_t epoch = __ldcg(a.sync + kSyncGen) + 1u;
+  const uint32_t gen_next = epoch_next_state(__ldcg(a.sync + kSyncGen));
+  const uint32_t epoch = epoch_of_state(gen_next, a.sync);
   if (cta == 0 && tid == 0) {
     // this step's tile counters (the previous grid has completed: pdl_wait above)
     a.sync[kSyncTileCnt] = 0u;
@@ -1479,7 +1481,7 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     // to leave publishes the new generation -- every CTA read the old one long before it got here.  One atomicAdd per
     // CTA: a compare-and-swap loop on an epoch-tagged word serialised the 148 leavers by L2 round trips and cost
     // every step 30 us (measured).
-    if (atomicAdd(a.sync + kSyncExit, 1u) == (uint32_t)G - 1u) a.sync[kSyncGen] = epoch;
+    if (atomicAdd(a.sync + kSyncExit, 1u) == (uint32_t)G - 1u) a.sync[kSyncGen] = gen_next;
   }
   if (warp == 6) {
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_base), "r"(tmem_cols) : "memory");

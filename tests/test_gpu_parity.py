@@ -638,6 +638,67 @@ def test_head_first_piece_order_matches_oracle(gpu, oracle, qwen_layer):
         gpu.eldr_moe_set_option(gpu.OPT_HEAD_FIRST, 0)
 
 
+@pytest.mark.parametrize("path", ["fused", "staged"])
+def test_recycled_workspace_with_stale_flags(gpu, oracle, path):
+    """A workspace handed out by a caching allocator holds the flags of whatever workspace lived there before, at other
+    offsets.  Reproduced deliberately: a few steps run in a workspace at offset 0 of a buffer, then the step runs in
+    'new' workspaces that START a few flag slots / pages into the used one's bytes (so the new generation word and
+    the new flag words all land on stale words of the old one), never zeroed.  Every run must be
+    bit-identical to the run in a zeroed workspace.  (With epoch = generation + 1 about one recycled workspace in a
+    hundred produced garbage on its first step -- found by a fuzz run over random shapes; the epochs are now a
+    full-period sequence salted with the workspace address: include/eldr_moe.h.)"""
+    import torch
+    shape = synth.MoEShape(hidden=256, inter=128, n_experts=24, top_k=3, n_shared=1, n_layers=1)
+    lw = synth.make_layer_weights(shape, 91, w_std=0.05, gate_std=0.2)
+    T = 40
+    dl = gpu.DecodeLayer(shape, lw, max_T=T)
+    x = gpu.bf16_from_bits(synth.make_hidden(T, shape.hidden, 92))
+    gpu.eldr_moe_set_option(gpu.OPT_STEP_PATH, gpu.STEP_FUSED if path == "fused" else gpu.STEP_STAGED)
+    try:
+        ref = dl.run(x, None).clone()
+        ref_ids = dl.ids[:T].clone()
+        n = dl.workspace.numel()
+        pad = 1 << 16
+        big = torch.zeros(n + pad, dtype=torch.uint8, device="cuda")
+        own = dl.workspace
+        for shift, steps_before in ((0, 1), (128, 1), (256, 1), (32, 1), (384, 1), (1152, 1), (4224, 1), (128, 3), (65408, 2)):
+            # (after ONE step every raised flag of the old workspace holds the first epoch and most other words are
+            # still zero: a new generation word that lands on a zero word used to start at that same first epoch)
+            big.zero_()
+            dl.workspace = big[:n]
+            for _ in range(steps_before):
+                dl.run(x, None)
+            torch.cuda.synchronize()
+            if shift:
+                dl.workspace = big[shift:shift + n]            # a 'new' allocation over the old one's bytes, at another offset
+            for _ in range(3):
+                out = dl.run(x, None)
+                torch.cuda.synchronize()
+                assert torch.equal(out.view(torch.int16), ref.view(torch.int16)), "shift %d" % shift
+                assert torch.equal(dl.ids[:T], ref_ids)
+        dl.workspace = own
+    finally:
+        gpu.eldr_moe_set_option(gpu.OPT_STEP_PATH, gpu.STEP_AUTO)
+
+
+def test_two_weight_tensors_at_one_address(gpu, oracle):
+    """Weights of one model freed, weights of another allocated at the same address with the same number of rows
+    (E * 2I) and the same H but another I: the cached TMA descriptor of the first must not serve the second (the 5-D
+    w1/w3 descriptor's strides depend on I; its cache key once did not -- found by a fuzz run over random shapes)."""
+    import torch
+    sa = synth.MoEShape(hidden=256, inter=128, n_experts=8, top_k=2, n_layers=1)
+    sb = synth.MoEShape(hidden=256, inter=64, n_experts=16, top_k=2, n_layers=1)
+    T = 24
+    buf13 = torch.empty(8 * 2 * 128 * 256, dtype=torch.bfloat16, device="cuda")
+    for shape, seed in ((sa, 301), (sb, 302), (sa, 303)):
+        lw = synth.make_layer_weights(shape, seed, w_std=0.05, gate_std=0.2)
+        dl = gpu.DecodeLayer(shape, lw, max_T=T)
+        buf13.copy_(dl.w13.reshape(-1))
+        dl.w13 = buf13.view(dl.w13.shape)
+        run_case(gpu, oracle, shape, lw, synth.make_hidden(T, shape.hidden, seed), layer_obj=dl)
+        assert gpu.eldr_moe_last_launch_count() == 1
+
+
 def test_invalid_option_values_are_rejected(gpu):
     for key, value in ((gpu.OPT_DP_MIN_ROUNDS, 0), (gpu.OPT_RING_KB, 16), (99, 1)):
         with pytest.raises(RuntimeError):
