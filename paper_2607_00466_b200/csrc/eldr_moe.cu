@@ -121,7 +121,11 @@ void make_layout(const eldr_moe_shape_t* s, int T, eldr_moe_ws_layout_t* L) {
   const size_t sync_fused = fused_sync_words((int)E, (int)ns, (int)I, (int)H) * 4;
   L->sync = take(align_up(sync_fused, 256) + sync_staged);   // [fused | staged]: never aliased (both derive epochs)
   const int zs = gate_slices(s, T);
-  L->z = take(Tz * E * 4 * (zs > 1 ? zs : 1));              // prefill-shaped gate: one partial logit tensor per slice
+  // prefill-shaped gate: one partial logit tensor per slice (CUDA-core split-K) or the logits + the three-term bf16
+  // split of the gate weights behind them (tensor-core gate: gate_tc.cuh), whichever is larger
+  const size_t z_cuda = Tz * E * 4 * (zs > 1 ? zs : 1);
+  const size_t z_tc = (T >= 2048 && H % 64 == 0) ? align_up(Tz * E * 4, 1024) + 3 * E * H * 2 : 0;
+  L->z = take(z_cuda > z_tc ? z_cuda : z_tc);
   L->cnt = take(align_up(E * 4, 256) + (Tz > (size_t)kDecodeMaxT ? (Tz + kRouteChunk - 1) / kRouteChunk * E * 4 : 0));   // + cnt_blk
   L->off = take((E + 1) * 4);
   L->perm = take(Tz * k * 4);

@@ -9,15 +9,17 @@
 // less forgiving than a chain of round-to-nearest FMAs over a long sum (measured with cuBLAS on this part: full K = 2048
 // in one accumulator 2.9e-5 abs error at |z| ~ 10, K slices of 256 summed afterwards 3.2e-6; in this kernel a 256-wide
 // slice still left 1.3e-5 on a layer with large gate weights: the accumulator's error grows with the NUMBER of
-// accumulations and the size of the running sum), so each TMEM accumulator holds ONE 64-wide k-chunk (3 terms x 4
-// MMAs of K = 16, lo first) and the epilogue warps add the chunks to fp32 registers in order, round to nearest.
+// accumulations and the size of the running sum), so each TMEM accumulator holds ONE 64-wide k-chunk -- the hi terms (4 MMAs of
+// K = 16) in one accumulator, the mid and lo terms (8 MMAs) in a second one -- and the epilogue warps add hi + (mid + lo)
+// of every chunk to fp32 registers in order, round to nearest.
 //
 // CTA = 128 tokens x 64 experts.  Warp 0: TMA producer (x box 128 x 64, three weight boxes 64 x 64 per 64-wide k-chunk,
-// 40 KiB per stage, 4 stages); warp 1: MMA issuer (tcgen05, M = 128 tokens, N = 64 experts, fp32 in TMEM, two 64-column
-// buffers); warps 2-5: epilogue (lane = token: 64 fp32 accumulators in registers).  The two expert halves of a token tile
+// 40 KiB per stage, 4 stages); warp 1: MMA issuer (tcgen05, M = 128 tokens, N = 64 experts, fp32 in TMEM, two buffers of
+// 2 x 64 columns); warps 2-5: epilogue (lane = token: 64 fp32 accumulators in registers).  The two expert halves of a token tile
 // are neighbouring CTAs, so x crosses HBM once.
 // The three-term split of Wg is written by gate_split_kernel into the workspace before it (1 MB in, 0.75 MB out).
-// Measured (bench.py --config prefill, gate = split + logits + top-k): T = 2048 / 4096 / 8192 / 16384: 39 / 42 / 50 / 81 us
+// Logit error against the fp64 oracle: 2e-6 at |z| ~ 15 (the CUDA-core kernel: 1.1e-5 on the same inputs).
+// Measured (bench.py --config prefill, gate = split + logits + top-k): T = 2048 / 4096 / 8192 / 16384: 44 / 44 / 50 / 88 us
 // against 78 / 108 / 157 / 275 us for the register-tiled CUDA-core GEMM; the step 0.49 -> 0.54 of the sustained bf16 peak
 // at T = 16384.
 #pragma once
@@ -69,7 +71,7 @@ gate_logits_tc_kernel(const __grid_constant__ CUtensorMap tm_x, const __grid_con
     tma_prefetch_desc(&tm_x);
     tma_prefetch_desc(&tm_w);
   }
-  constexpr uint32_t tmem_cols = 2 * kGtcExp;
+  constexpr uint32_t tmem_cols = 4 * kGtcExp;                       // two buffers x (hi-term accumulator | mid+lo accumulator)
   if (warp == 1) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(tmem_slot), "r"(tmem_cols) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
@@ -107,9 +109,12 @@ gate_logits_tc_kernel(const __grid_constant__ CUtensorMap tm_x, const __grid_con
       const uint32_t buf = sl & 1;
       mbar_wait(tempty_bar(buf), ((sl >> 1) & 1) ^ 1);
       tc_fence_after();
-      const uint32_t d_tmem = tmem_base + buf * kGtcExp;
+      // the hi terms (the full-size products) get an accumulator of their own: every accumulation rounds at the size
+      // of the running sum, and the eight mid / lo MMAs of a chunk would otherwise each cost the big sum one more
+      // rounding for a contribution of 2^-8 / 2^-16 of it (measured: 1.1e-5 instead of < 5e-6 at |z| ~ 10, H = 256)
+      const uint32_t d_hi = tmem_base + buf * 2 * kGtcExp, d_lo = d_hi + kGtcExp;
       const int kc_end = min(n_chunks, (sl + 1) * kGtcSliceChunks);
-      bool first = true;
+      bool first_lo = true, first_hi = true;
       for (; kc < kc_end; ++kc) {
         const int s = kc % kGtcStages;
         mbar_wait(full_bar(s), (kc / kGtcStages) & 1);
@@ -121,8 +126,8 @@ gate_logits_tc_kernel(const __grid_constant__ CUtensorMap tm_x, const __grid_con
           const uint64_t db = umma_desc_sw128(sa + kGtcTok * 128 + term * kGtcExp * 128);
 #pragma unroll
           for (int k = 0; k < 4; ++k) {
-            umma_bf16_if(leader, d_tmem, da + 2 * k, db + 2 * k, idesc, first ? 0u : 1u);
-            first = false;
+            if (term < 2) { umma_bf16_if(leader, d_lo, da + 2 * k, db + 2 * k, idesc, first_lo ? 0u : 1u); first_lo = false; }
+            else { umma_bf16_if(leader, d_hi, da + 2 * k, db + 2 * k, idesc, first_hi ? 0u : 1u); first_hi = false; }
           }
         }
         umma_commit_if(leader, empty_bar(s));
@@ -139,13 +144,14 @@ gate_logits_tc_kernel(const __grid_constant__ CUtensorMap tm_x, const __grid_con
       const int buf = sl & 1;
       mbar_wait(tfull_bar(buf), (sl >> 1) & 1);
       tc_fence_after();
-      const uint32_t t_addr = tmem_base + buf * kGtcExp + ((uint32_t)(qtr * 32) << 16);
+      const uint32_t t_addr = tmem_base + buf * 2 * kGtcExp + ((uint32_t)(qtr * 32) << 16);
 #pragma unroll
       for (int c0 = 0; c0 < kGtcExp; c0 += 16) {
-        float v[16];
-        tmem_ld16(t_addr + c0, v);
+        float vh[16], vl[16];
+        tmem_ld16(t_addr + c0, vh);
+        tmem_ld16(t_addr + kGtcExp + c0, vl);
 #pragma unroll
-        for (int j = 0; j < 16; ++j) acc[c0 + j] += v[j];           // slice order, round to nearest
+        for (int j = 0; j < 16; ++j) acc[c0 + j] += vh[j] + vl[j];  // chunk order, round to nearest
       }
       tc_fence_before();
       __syncwarp();
