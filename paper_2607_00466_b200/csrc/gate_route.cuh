@@ -522,7 +522,8 @@ __global__ void __launch_bounds__(256) sig_accumulate_kernel(const int32_t* __re
 // All layers of a prefill-shaped call in ONE launch ("Each forward accumulates the new tokens' expert picks
 // into the matching rows in a single GPU pass"): grid (token chunks of 256, layers).  A chunk's increments are first
 // combined in shared memory -- the request histogram when all 256 tokens belong to one request (the prefill case), the
-// KV-block rows per run of equal block ids (a new run at least every 64 tokens, so a byte cell cannot overflow) -- and
+// KV-block rows per run of equal block ids (a new run at least every 64 tokens, so a byte of the shared-memory
+// histogram cannot overflow) -- and
 // only the non-zero cells / words go to global memory: ~10x fewer global atomics than one per pick.  Decode-shaped
 // chunks (every token its own request) take the direct path for the request table.  Same saturating int8 semantics.
 constexpr int kSigChunk = 256;
@@ -585,15 +586,24 @@ __global__ void __launch_bounds__(256) sig_accumulate_layers_kernel(const int32_
       const int r = i / EW, wd = i - r * EW;
       const size_t cell0 = ((size_t)s_run_blk[r] * L + layer) * E + (size_t)wd * 4;
       if (word_ok) {
+        // saturating packed add as a compare-and-swap loop.  (An add followed by an undo of the excess is exact only
+        // while a byte's TRANSIENT value stays below 256: three runs of 64 picks landing on a saturated cell before
+        // any of them has undone its excess wrap the byte -- a block with more than 127 tokens, outside the int8
+        // cells' contract but reachable through the ABI; found by a fuzz run.)
         unsigned int* word = reinterpret_cast<unsigned int*>(sig_block + cell0);
-        const unsigned int old = atomicAdd(word, add);
-        unsigned int undo = 0u;
+        unsigned int seen = *reinterpret_cast<volatile unsigned int*>(word);
+        for (;;) {
+          unsigned int nw = 0u;
 #pragma unroll
-        for (int b = 0; b < 4; ++b) {
-          const unsigned int ob = (old >> (8 * b)) & 0xffu, c = (add >> (8 * b)) & 0xffu;
-          if (c && ob + c > 127u) undo |= (ob + c - max(ob, 127u)) << (8 * b);
+          for (int b = 0; b < 4; ++b) {
+            const unsigned int ob = (seen >> (8 * b)) & 0xffu, c = (add >> (8 * b)) & 0xffu;
+            nw |= min(ob + c, max(ob, 127u)) << (8 * b);
+          }
+          if (nw == seen) break;
+          const unsigned int was = atomicCAS(word, seen, nw);
+          if (was == seen) break;
+          seen = was;
         }
-        if (undo) atomicSub(word, undo);
       } else {
         for (int b = 0; b < 4 && wd * 4 + b < E; ++b)
           for (unsigned int c = (add >> (8 * b)) & 0xffu; c > 0; --c) sig_add(nullptr, sig_block, -1, s_run_blk[r], L, layer, E, wd * 4 + b);

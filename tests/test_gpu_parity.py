@@ -950,7 +950,8 @@ def test_two_layers_on_two_streams_match_serial_results(gpu, oracle):
             assert torch.equal(o.view(torch.int16), ref[i].view(torch.int16))
 
 
-@pytest.mark.parametrize("E,k,T,shaped", [(64, 6, 3000, "prefill"), (64, 6, 700, "decode"), (10, 3, 530, "prefill"), (130, 4, 257, "mixed")])
+@pytest.mark.parametrize("E,k,T,shaped", [(64, 6, 3000, "prefill"), (64, 6, 700, "decode"), (10, 3, 530, "prefill"), (130, 4, 257, "mixed"),
+                                             (64, 6, 2000, "mixed")])    # one block, 2000 picks of one expert from eight CTAs at once
 def test_signature_accumulate_layers_one_launch(gpu, oracle, E, k, T, shaped):
     """eldr_signature_accumulate_layers (all layers in one launch, chunk-level combining in shared memory) equals the
     oracle's serial loop bit for bit: prefill-shaped maps (long runs of one request, 16-token KV blocks, non-contiguous
