@@ -61,6 +61,7 @@ ffn_gemv_kernel(const uint16_t* __restrict__ w, const uint16_t* __restrict__ w_s
       for (int r = warp; r < rows_in_tile; r += kGemvThreads / 32) {
         const int row = rt * rows_in_tile + r;                   // MODE 0: intermediate index i; MODE 1: output row
         if (MODE == 1 && row >= a.H) break;
+        if (MODE == 0 && row >= a.I) break;                       // I not a multiple of 64: the last tile is partial
         const uint4* w0 = reinterpret_cast<const uint4*>(wbase + (size_t)row * K);
         const uint4* w1 = reinterpret_cast<const uint4*>(wbase + (size_t)(row + a.I) * K);     // MODE 0: the w3 row
         float acc0[kGemvTok], acc1[kGemvTok];

@@ -449,6 +449,10 @@ def test_alternate_paths_match_oracle(gpu, oracle, step_path, ffn_path, pdl):
         token_req, token_block = synth.decode_maps(150)
         r = run_case(gpu, oracle, shape, lw, x, None, token_req, token_block, n_req=150, n_blk=150, layer=1)
         assert gpu.eldr_moe_last_launch_count() == (1 if (step_path == 1 and ffn_path == 1) else 5)
+        # ragged I and H (not multiples of 64): partial last w1/w3 tile of the GEMV path, plain CUDA-core FFN of the others
+        ragged = synth.MoEShape(hidden=72, inter=40, n_experts=9, top_k=3, n_shared=1, n_layers=2)
+        rlw = synth.make_layer_weights(ragged, 33, w_std=0.05, gate_std=0.2)
+        run_case(gpu, oracle, ragged, rlw, synth.make_hidden(70, ragged.hidden, 33))
     finally:
         gpu.eldr_moe_set_option(gpu.OPT_STEP_PATH, gpu.STEP_AUTO)
         gpu.eldr_moe_set_option(gpu.OPT_FFN_PATH, gpu.FFN_TCGEN05)
