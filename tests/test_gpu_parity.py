@@ -427,10 +427,23 @@ def test_host_buffer_entry_point_matches_device_entry_point(gpu):
     h_ids = torch.empty((8, shape.top_k), dtype=torch.int32).pin_memory()
     h_w = torch.empty((8, shape.top_k), dtype=torch.float32).pin_memory()
     h_na = torch.zeros((1,), dtype=torch.int32).pin_memory()
-    gpu.eldr_moe_decode_layer_host(shape, 0, h_x, dl.gate_w, None, dl.w13, dl.w2, None, None, h_out, h_ids, h_w,
-                                   h_na, None, None, None, None, dl.workspace)
-    assert torch.equal(h_out.view(torch.int16), ref.cpu().view(torch.int16))
-    assert int(h_na.item()) == int(dl.n_active.item())
+    ref_ids, ref_w = dl.ids[:8].cpu().clone(), dl.w[:8].cpu().clone()
+    for _ in range(2):        # (ids / weights: mirrored by a small block, or written through the mapping by the one-launch step)
+        h_ids.fill_(-3); h_w.fill_(-3.0); h_out.zero_()
+        gpu.eldr_moe_decode_layer_host(shape, 0, h_x, dl.gate_w, None, dl.w13, dl.w2, None, None, h_out, h_ids, h_w,
+                                       h_na, None, None, None, None, dl.workspace)
+        assert torch.equal(h_out.view(torch.int16), ref.cpu().view(torch.int16))
+        assert torch.equal(h_ids, ref_ids) and torch.equal(h_w.view(torch.int32), ref_w.view(torch.int32))
+        assert int(h_na.item()) == int(dl.n_active.item())
+    # pageable host buffers: staged copies, same results
+    p_out = torch.empty((8, shape.hidden), dtype=torch.bfloat16)
+    p_ids = torch.full((8, shape.top_k), -3, dtype=torch.int32)
+    p_w = torch.empty((8, shape.top_k), dtype=torch.float32)
+    p_na = torch.zeros((1,), dtype=torch.int32)
+    gpu.eldr_moe_decode_layer_host(shape, 0, gpu.bf16_from_bits(x_bits, device=None), dl.gate_w, None, dl.w13, dl.w2, None, None,
+                                   p_out, p_ids, p_w, p_na, None, None, None, None, dl.workspace)
+    assert torch.equal(p_out.view(torch.int16), ref.cpu().view(torch.int16)) and torch.equal(p_ids, ref_ids)
+    assert torch.equal(p_w.view(torch.int32), ref_w.view(torch.int32)) and int(p_na.item()) == int(dl.n_active.item())
 
 
 @pytest.mark.parametrize("step_path,ffn_path,pdl", [(1, 1, 0), (0, 1, 1), (0, 0, 1), (0, 1, 0), (0, 0, 0), (1, 1, 1), (0, 2, 1), (2, 2, 0)])
