@@ -683,8 +683,9 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
     const size_t smem_max = 227 * 1024;
     const size_t fixed = fused_smem_fixed_bytes(E, ns, T, k);
     const int gate_tok = T <= 64 ? 8 : (T <= 128 ? 16 : 32);      // gate tile height: one round of tiles over the grid
-    const size_t min_area = (size_t)3 * (kUmmaWBytes + kNPCap * 128) > (size_t)gate_tok * H * 2
-                                ? (size_t)3 * (kUmmaWBytes + kNPCap * 128) : (size_t)gate_tok * H * 2;
+    // the gate tile borrows the ring's area: x rows, and for the wide tiles the eight fp32 gate rows too
+    const size_t gate_area = (size_t)gate_tok * H * 2 + (gate_tok > 8 ? (size_t)kGateExp * H * 4 : 0);
+    const size_t min_area = (size_t)3 * (kUmmaWBytes + kNPCap * 128) > gate_area ? (size_t)3 * (kUmmaWBytes + kNPCap * 128) : gate_area;
     fa.stage_area = fixed < smem_max ? (int)((smem_max - fixed) / 1024 * 1024) : 0;
     fa.ring_bytes = g_ring_kb.load() * 1024;
     fa.dp_min_rounds = g_dp_min_rounds.load();

@@ -316,6 +316,93 @@ __device__ __forceinline__ void fused_gate_tile(const FusedArgs& a, int et, int 
   }
 }
 
+// Wide tiles (GT = 16 / 32 tokens, T > 64): the x tile AND the tile's eight gate rows are brought into shared memory by
+// two bulk copies, and a warp owns 4 experts x GT/4 tokens (the narrow tile: 2 x GT/2 with the gate rows in registers).
+// Every converted x value now feeds four FMAs instead of two (the bf16 -> fp32 conversions run on the ALU pipe at half
+// the FMA rate and were half of the tile's issue time at GT = 32), and no gate-row load sits between two halves of the
+// K loop.  The per-lane summation order (column = lane + 32 j, ascending) is the narrow tile's: same logits, bit for bit.
+template <int GT>
+__device__ __forceinline__ void fused_gate_tile_wide(const FusedArgs& a, int et, int g, uint8_t* smem_raw, uint32_t gbar,
+                                                     uint32_t gpar) {
+  constexpr int TW = GT / 4;              // tokens per warp
+  const int T = a.tk.T, H = a.H, E = a.tk.E;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int t0 = g * GT;
+  const int eq = warp & 1, tg = warp >> 1;
+  const int e0 = et * kGateExp;
+  const int q_per_row = H >> 2;
+  const int rows = min(GT, T - t0), n_e = min(kGateExp, E - e0);
+  uint8_t* w_smem = smem_raw + (size_t)GT * H * 2;
+  __syncthreads();                       // the previous tile's readers are done with the tile
+  if (tid == 0) {
+    const uint32_t xb = (uint32_t)rows * (uint32_t)H * 2u, wb = (uint32_t)n_e * (uint32_t)H * 4u;
+    mbar_arrive_expect_tx(gbar, xb + wb);
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(smem_u32(smem_raw)), "l"(a.x + (size_t)t0 * H), "r"(xb), "r"(gbar) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(smem_u32(w_smem)), "l"(a.gate_w + (size_t)e0 * H), "r"(wb), "r"(gbar) : "memory");
+  }
+  {
+    uint4* xs4 = reinterpret_cast<uint4*>(smem_raw);
+    const int vec_per_row = H >> 3;
+    for (int v = rows * vec_per_row + tid; v < GT * vec_per_row; v += kFusedThreads) xs4[v] = make_uint4(0u, 0u, 0u, 0u);
+    uint4* ws4 = reinterpret_cast<uint4*>(w_smem);
+    for (int v = n_e * q_per_row + tid; v < kGateExp * q_per_row; v += kFusedThreads) ws4[v] = make_uint4(0u, 0u, 0u, 0u);
+  }
+  mbar_wait(gbar, gpar);
+  __syncthreads();
+  float acc[4][TW];
+#pragma unroll
+  for (int e = 0; e < 4; ++e)
+#pragma unroll
+    for (int t = 0; t < TW; ++t) acc[e][t] = 0.f;
+  const float4* wv = reinterpret_cast<const float4*>(w_smem) + (size_t)(4 * eq) * q_per_row;
+  const uint2* xs2 = reinterpret_cast<const uint2*>(smem_raw) + (size_t)(TW * tg) * q_per_row;
+  for (int c4 = lane; c4 < q_per_row; c4 += 32) {
+    float4 w4[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) w4[e] = wv[(size_t)e * q_per_row + c4];
+#pragma unroll
+    for (int t = 0; t < TW; ++t) {
+      const uint2 xv = xs2[t * q_per_row + c4];
+      const float x0 = bf16_lo(xv.x), x1 = bf16_hi(xv.x), x2 = bf16_lo(xv.y), x3 = bf16_hi(xv.y);
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        float s = acc[e][t];
+        s = fmaf(w4[e].x, x0, s);
+        s = fmaf(w4[e].y, x1, s);
+        s = fmaf(w4[e].z, x2, s);
+        s = fmaf(w4[e].w, x3, s);
+        acc[e][t] = s;
+      }
+    }
+  }
+#pragma unroll
+  for (int e = 0; e < 4; ++e)
+#pragma unroll
+    for (int t = 0; t < TW; ++t) {
+      float s = acc[e][t];
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+      acc[e][t] = s;
+    }
+  if (lane == 0) {
+    float* z = const_cast<float*>(a.tk.z);
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      const int ee = e0 + 4 * eq + e;
+      if (ee < E) {
+        const float b = a.gate_bias ? a.gate_bias[ee] : 0.f;
+#pragma unroll
+        for (int t = 0; t < TW; ++t) {
+          const int tt = t0 + TW * tg + t;
+          if (tt < T) z[(size_t)tt * E + ee] = acc[e][t] + b;
+        }
+      }
+    }
+  }
+}
+
 // ------------------------------------------------------------------------------- K: redux-based warp top-k
 // Same order as warp_topk (z descending, lower id on ties), but each of the k rounds is two warp reductions
 // (redux.sync max on an order-preserving uint key, redux.sync min on the candidate id) instead of ten shuffles.
@@ -888,7 +975,8 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     uint32_t gpar = 0;
     for (int tile = cta; tile < n_tiles; tile += G, gpar ^= 1u) {
       const int g = tile / n_et, et = tile - g * n_et;
-      fused_gate_tile<GT>(a, et, g, scratch, sm.bar_base + 400u, gpar);
+      if constexpr (GT > 8) fused_gate_tile_wide<GT>(a, et, g, scratch, sm.bar_base + 400u, gpar);
+      else fused_gate_tile<GT>(a, et, g, scratch, sm.bar_base + 400u, gpar);
       __syncthreads();
       if (tid == 0) flag_release(a.sync + kSyncTile + g * 32 + et, epoch);    // cumulative over the barrier
     }
