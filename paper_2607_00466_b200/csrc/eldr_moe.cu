@@ -684,7 +684,9 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
     const size_t fixed = fused_smem_fixed_bytes(E, ns, T, k);
     const int gate_tok = T <= 64 ? 8 : (T <= 128 ? 16 : 32);      // gate tile height: one round of tiles over the grid
     // the gate tile borrows the ring's area: x rows, and for the wide tiles the eight fp32 gate rows too
-    const size_t gate_area = (size_t)gate_tok * H * 2 + (gate_tok > 8 ? (size_t)kGateExp * H * 4 : 0);
+    const size_t gate_area_wide = (size_t)gate_tok * H * 2 + (size_t)kGateExp * H * 4;
+    const bool gate_wide8 = gate_tok == 8 && fixed < smem_max && gate_area_wide <= (smem_max - fixed) / 1024 * 1024;
+    const size_t gate_area = (gate_tok > 8 || gate_wide8) ? gate_area_wide : (size_t)gate_tok * H * 2;
     const size_t min_area = (size_t)3 * (kUmmaWBytes + kNPCap * 128) > gate_area ? (size_t)3 * (kUmmaWBytes + kNPCap * 128) : gate_area;
     fa.stage_area = fixed < smem_max ? (int)((smem_max - fixed) / 1024 * 1024) : 0;
     fa.ring_bytes = g_ring_kb.load() * 1024;
@@ -710,10 +712,11 @@ int32_t eldr_moe_decode_layer(const eldr_moe_shape_t* s, int32_t layer, int32_t 
         tm_sw2 = tm_w2;
       }
       if (!once_per_device(kAttrFused, [] {
-            return set_smem(moe_fused_kernel<8>, 227 * 1024) && set_smem(moe_fused_kernel<16>, 227 * 1024) &&
-                   set_smem(moe_fused_kernel<32>, 227 * 1024);
+            return set_smem(moe_fused_kernel<8, true>, 227 * 1024) && set_smem(moe_fused_kernel<8, false>, 227 * 1024) &&
+                   set_smem(moe_fused_kernel<16, true>, 227 * 1024) && set_smem(moe_fused_kernel<32, true>, 227 * 1024);
           })) return ELDR_ERR_CUDA;
-      auto kern = gate_tok == 8 ? moe_fused_kernel<8> : (gate_tok == 16 ? moe_fused_kernel<16> : moe_fused_kernel<32>);
+      auto kern = gate_tok == 8 ? (gate_wide8 ? moe_fused_kernel<8, true> : moe_fused_kernel<8, false>)
+                                : (gate_tok == 16 ? moe_fused_kernel<16, true> : moe_fused_kernel<32, true>);
       // The persistent grid's CTAs wait on one another (tile flags, tagged ids, h / y flags): they must all be
       // resident.  (1) Once per device: the occupancy calculator must grant one CTA of this size on every SM, else the
       // call takes the staged path (no grid-wide waits there).  (2) Every launch is a COOPERATIVE launch: the driver

@@ -316,8 +316,10 @@ __device__ __forceinline__ void fused_gate_tile(const FusedArgs& a, int et, int 
   }
 }
 
-// Wide tiles (GT = 16 / 32 tokens, T > 64): the x tile AND the tile's eight gate rows are brought into shared memory by
-// two bulk copies, and a warp owns 4 experts x GT/4 tokens (the narrow tile: 2 x GT/2 with the gate rows in registers).
+// Shared-memory gate tile (every tile that fits the ring area: all of T > 64, and 8-token tiles up to H ~ 4300): the x
+// tile AND the tile's eight gate rows are brought into shared memory by two bulk copies, and a warp owns 4 experts x
+// GT/4 tokens (the register-staged tile below: 2 x GT/2 with the gate rows in registers).  Measured at T = 64: every
+// config-2 point 1.2-1.5 us faster (one L2 round trip for everything instead of rows -> x -> second half of the rows).
 // Every converted x value now feeds four FMAs instead of two (the bf16 -> fp32 conversions run on the ALU pipe at half
 // the FMA rate and were half of the tile's issue time at GT = 32), and no gate-row load sits between two halves of the
 // K loop.  The per-lane summation order (column = lane + 32 j, ascending) is the narrow tile's: same logits, bit for bit.
@@ -880,7 +882,10 @@ __device__ __forceinline__ void fused_combine(const FusedArgs& a, const FusedSme
 }
 
 // ------------------------------------------------------------------------------------------- the kernel
-template <int GT>
+// GT: tokens per gate tile (8 / 16 / 32 for T <= 64 / 128 / 256).  GW: the gate tile staged in shared memory (always for
+// GT > 8; for GT = 8 whenever it fits the ring area, else the register-staged tile).  Template parameters, not run-time
+// branches: with both tile kinds inlined into one kernel every config-2 point lost the microsecond the new tile gains.
+template <int GT, bool GW = true>
 __global__ void __launch_bounds__(kFusedThreads, 1)
 moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_constant__ CUtensorMap tm_sw13,
                  const __grid_constant__ CUtensorMap tm_w2, const __grid_constant__ CUtensorMap tm_sw2,
@@ -975,7 +980,8 @@ moe_fused_kernel(const __grid_constant__ CUtensorMap tm_w13, const __grid_consta
     uint32_t gpar = 0;
     for (int tile = cta; tile < n_tiles; tile += G, gpar ^= 1u) {
       const int g = tile / n_et, et = tile - g * n_et;
-      if constexpr (GT > 8) fused_gate_tile_wide<GT>(a, et, g, scratch, sm.bar_base + 400u, gpar);
+      // (the register-staged tile only where the shared-memory one does not fit: 8-token tiles at H > ~4300)
+      if constexpr (GT > 8 || GW) fused_gate_tile_wide<GT>(a, et, g, scratch, sm.bar_base + 400u, gpar);
       else fused_gate_tile<GT>(a, et, g, scratch, sm.bar_base + 400u, gpar);
       __syncthreads();
       if (tid == 0) flag_release(a.sync + kSyncTile + g * 32 + et, epoch);    // cumulative over the barrier

@@ -698,6 +698,18 @@ def test_recycled_workspace_with_stale_flags(gpu, oracle, path):
         gpu.eldr_moe_set_option(gpu.OPT_STEP_PATH, gpu.STEP_AUTO)
 
 
+@pytest.mark.parametrize("H,T,want_launches", [(4608, 20, 1), (8192, 40, 1), (4096, 64, 1), (4608, 130, 5)])
+def test_large_hidden_sizes_pick_the_gate_tile_that_fits(gpu, oracle, H, T, want_launches):
+    """The one-launch step stages its 8-token gate tile (x rows + eight fp32 gate rows, 48 bytes per hidden unit) in the
+    ring's shared memory when that fits (H = 4096) and falls back to the register-staged tile (16 bytes per hidden unit)
+    above (H = 4608, 8192: another instantiation of the kernel); wide batches at such H have no tile that fits and
+    take the staged launches."""
+    shape = synth.MoEShape(hidden=H, inter=64, n_experts=6, top_k=2, n_layers=1)
+    lw = synth.make_layer_weights(shape, 41, w_std=0.02, gate_std=0.05)
+    run_case(gpu, oracle, shape, lw, synth.make_hidden(T, H, 42))
+    assert gpu.eldr_moe_last_launch_count() == want_launches
+
+
 def test_two_weight_tensors_at_one_address(gpu, oracle):
     """Weights of one model freed, weights of another allocated at the same address with the same number of rows
     (E * 2I) and the same H but another I: the cached TMA descriptor of the first must not serve the second (the 5-D
